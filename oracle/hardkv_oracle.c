@@ -1,0 +1,310 @@
+/*
+ * hardkv_oracle.c -- TEST INFRASTRUCTURE ONLY (see hardkv_oracle.h).
+ *
+ * Plain nested loops in the paper's order.  No blocking, no fusion, no SIMD
+ * intrinsics; the only library routines are exp/log/ceil/nearbyint and qsort.
+ * Citations are PAPER.md line numbers (L...) and DESIGN.md readings (C...).
+ */
+#include "hardkv_oracle.h"
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+static uint32_t f32_bits(float x) { uint32_t b; memcpy(&b, &x, 4); return b; }
+
+/* Pool = Tier-2 address range [c_lo, n-W) (L72, DESIGN "tiers"); empty if n-W <= c_lo. */
+static int32_t pool_hi(const hko_config *c, const hko_unit *u) {
+  int32_t hi = u->n - c->recent;
+  return hi > u->c_lo ? hi : u->c_lo;
+}
+
+/* ---- Step 1 (L78): "linearly append KV pairs to the Tier 1 Dense Cache" -------- */
+void hko_append(const hko_config *c, hko_unit *u, const float *k_new, const float *v_new) {
+  memcpy(u->K + (size_t)u->n * c->d, k_new, sizeof(float) * c->d);
+  memcpy(u->V + (size_t)u->n * c->d, v_new, sizeof(float) * c->d);
+  u->n += 1;
+}
+
+/* ---- Step 4 (L78) / Tier 3 (L76) / vote ranking (L86), reading C7 --------------
+ * While the pool exceeds l_upper, its oldest token t = c_lo retires.  The
+ * condensed tier has C_cap constant slots; a free slot takes t; otherwise the
+ * resident with the lexicographically smallest (votes, pos) is the candidate
+ * victim and t replaces it iff votes[t] >= its votes (t is newer, so it wins
+ * ties); else t is evicted for good. */
+int hko_retire(const hko_config *c, hko_unit *u) {
+  int retired = 0;
+  while (u->n - c->recent - u->c_lo > u->l_upper) {
+    int32_t t = u->c_lo;
+    int32_t slot = -1;
+    if (u->cond_count < c->cond_cap) {
+      slot = u->cond_count;
+      u->cond_count += 1;
+    } else if (c->cond_cap > 0) {
+      int32_t m = 0;
+      for (int32_t j = 1; j < c->cond_cap; ++j) {
+        if (u->cond_votes[j] < u->cond_votes[m] ||
+            (u->cond_votes[j] == u->cond_votes[m] && u->cond_pos[j] < u->cond_pos[m]))
+          m = j;
+      }
+      if (u->votes[t] >= u->cond_votes[m]) slot = m;
+    }
+    if (slot >= 0) {
+      memcpy(u->cond_k + (size_t)slot * c->d, u->K + (size_t)t * c->d, sizeof(float) * c->d);
+      memcpy(u->cond_v + (size_t)slot * c->d, u->V + (size_t)t * c->d, sizeof(float) * c->d);
+      u->cond_pos[slot] = t;
+      u->cond_votes[slot] = u->votes[t];
+    }
+    u->c_lo += 1;
+    retired += 1;
+  }
+  return retired;
+}
+
+/* ---- score: exponent of Eq. 4 (L735-739) with the scale of reading C1 ---------- */
+void hko_score(const hko_config *c, hko_unit *u, const float *q) {
+  int32_t hi = pool_hi(c, u);
+  for (int32_t g = 0; g < c->G; ++g) {
+    for (int32_t i = u->c_lo; i < hi; ++i) {
+      double dot = 0.0;
+      for (int32_t e = 0; e < c->d; ++e)
+        dot += (double)q[(size_t)g * c->d + e] * (double)u->K[(size_t)i * c->d + e];
+      u->logits[(size_t)g * c->max_ctx + i] = (float)((double)c->sm_scale * dot);
+    }
+  }
+}
+
+/* ---- Logits Calibration, apply-T (L120 "S_hat = S(g(z/T))", g = identity for
+ * VANILLA L276; H2O-style averaging L124 for ACCUM, reading C4).  One score per
+ * KV head = mean over the GQA group of per-query-head softmax probabilities
+ * (reading C2), softmax taken over the pool only (reading C3). */
+void hko_calibrate(const hko_config *c, hko_unit *u) {
+  int32_t lo = u->c_lo, hi = pool_hi(c, u);
+  if (hi <= lo) return;
+  double T = (double)u->T;
+  double *P = (double *)calloc((size_t)(hi - lo), sizeof(double));
+  for (int32_t g = 0; g < c->G; ++g) {
+    const float *z = u->logits + (size_t)g * c->max_ctx;
+    double m = -INFINITY;
+    for (int32_t i = lo; i < hi; ++i) { double x = (double)z[i] / T; if (x > m) m = x; }
+    double s = 0.0;
+    for (int32_t i = lo; i < hi; ++i) s += exp((double)z[i] / T - m);
+    for (int32_t i = lo; i < hi; ++i) P[i - lo] += exp((double)z[i] / T - m) / s;
+  }
+  for (int32_t i = lo; i < hi; ++i) P[i - lo] /= (double)c->G;
+
+  if (u->score_mode == 0) {
+    for (int32_t i = lo; i < hi; ++i) u->probs[i] = (float)P[i - lo];
+  } else {
+    /* ACCUM (reading C4): sliding sum of the last accum_window per-step rows, kept
+     * incrementally: acc <- max(0, acc - ring[slot] + P_t); ring[slot] <- P_t;
+     * then renormalised over the current pool. acc and ring are fp32 state. */
+    float *ring = u->ring + (size_t)u->ring_slot * c->max_ctx;
+    double tot = 0.0;
+    for (int32_t i = lo; i < hi; ++i) {
+      float pt = (float)P[i - lo];
+      double a = ((double)u->acc[i] - (double)ring[i]) + (double)pt;
+      if (a < 0.0) a = 0.0;
+      u->acc[i] = (float)a;
+      ring[i] = pt;
+      tot += (double)u->acc[i];
+    }
+    u->ring_slot = (u->ring_slot + 1) % c->accum_window;
+    for (int32_t i = lo; i < hi; ++i)
+      u->probs[i] = tot > 0.0 ? (float)((double)u->acc[i] / tot) : 0.0f;
+  }
+  free(P);
+}
+
+/* ---- Top-p nucleus (L108: "Top-p sampling over {S_i} yield k tokens"), made a
+ * single well-defined result by reading C5: integer mass w_i = rn(P_i * 2^32),
+ * total order (P as fp32 bit pattern descending, position ascending), shortest
+ * prefix whose mass >= Theta = ceil(p * Wtot).  Reading C6: k = min(k_topp, k_cap),
+ * the clamp keeps the best of the same order (L233 "k as the maximum block usage
+ * for Top-p pruned each head"). */
+typedef struct { uint32_t bits; int32_t pos; } hko_key;
+static int hko_key_cmp(const void *a, const void *b) {
+  const hko_key *x = (const hko_key *)a, *y = (const hko_key *)b;
+  if (x->bits != y->bits) return x->bits > y->bits ? -1 : 1;   /* P descending  */
+  if (x->pos != y->pos) return x->pos < y->pos ? -1 : 1;       /* pos ascending */
+  return 0;
+}
+static int hko_i32_cmp(const void *a, const void *b) {
+  int32_t x = *(const int32_t *)a, y = *(const int32_t *)b;
+  return (x > y) - (x < y);
+}
+
+void hko_topp_select(const hko_config *c, hko_unit *u, float p, int count_votes) {
+  int32_t lo = u->c_lo, hi = pool_hi(c, u);
+  int32_t N = hi - lo;
+  for (int32_t j = 0; j < c->k_cap; ++j) u->sel_idx[j] = -1;
+  u->sel_count = 0; u->k_topp = 0; u->tau_bits = 0;
+  if (N <= 0) return;
+
+  hko_key *keys = (hko_key *)malloc(sizeof(hko_key) * (size_t)N);
+  for (int32_t i = 0; i < N; ++i) { keys[i].bits = f32_bits(u->probs[lo + i]); keys[i].pos = lo + i; }
+  qsort(keys, (size_t)N, sizeof(hko_key), hko_key_cmp);   /* total order: no ties left */
+
+  int32_t k_topp;
+  if (p >= 1.0f || N <= u->l_lower) {
+    k_topp = N;                                      /* no sparsity yet (L197, C8) */
+  } else {
+    uint64_t Wtot = 0;
+    for (int32_t i = 0; i < N; ++i)
+      Wtot += (uint64_t)nearbyint((double)u->probs[lo + i] * 4294967296.0);
+    uint64_t Theta = (uint64_t)ceil((double)p * (double)Wtot);
+    if (Theta < 1) Theta = 1;
+    uint64_t cum = 0;
+    k_topp = N;
+    for (int32_t j = 0; j < N; ++j) {
+      float Pj; memcpy(&Pj, &keys[j].bits, 4);
+      cum += (uint64_t)nearbyint((double)Pj * 4294967296.0);
+      if (cum >= Theta) { k_topp = j + 1; break; }
+    }
+  }
+  int32_t k = k_topp < c->k_cap ? k_topp : c->k_cap;
+  u->k_topp = k_topp;
+  u->sel_count = k;
+  if (k > 0) u->tau_bits = keys[k - 1].bits;
+  for (int32_t j = 0; j < k; ++j) u->sel_idx[j] = keys[j].pos;
+  qsort(u->sel_idx, (size_t)k, sizeof(int32_t), hko_i32_cmp);   /* I ascending (C9) */
+  if (count_votes)
+    for (int32_t j = 0; j < k; ++j) u->votes[u->sel_idx[j]] += 1;   /* L86 cumulative mask */
+  free(keys);
+}
+
+/* ---- Rewrite Cache (L172: "read the selected blocks and write them into a
+ * regularized, contiguous range"); ascending position, tail of the last valid
+ * page zero (reading C9). */
+void hko_rewrite(const hko_config *c, hko_unit *u) {
+  int32_t k = u->sel_count;
+  for (int32_t j = 0; j < k; ++j) {
+    memcpy(u->sel_k + (size_t)j * c->d, u->K + (size_t)u->sel_idx[j] * c->d, sizeof(float) * c->d);
+    memcpy(u->sel_v + (size_t)j * c->d, u->V + (size_t)u->sel_idx[j] * c->d, sizeof(float) * c->d);
+  }
+  int32_t end = ((k + c->page - 1) / c->page) * c->page;
+  for (int32_t j = k; j < end; ++j) {
+    memset(u->sel_k + (size_t)j * c->d, 0, sizeof(float) * c->d);
+    memset(u->sel_v + (size_t)j * c->d, 0, sizeof(float) * c->d);
+  }
+}
+
+/* ---- Appendix F.  Attention state of an index set I (Eq. 5):
+ * o(I) = sum_i SE_i v_i / SE(I), SE(I) = sum_i exp(x_i), x_i = sm_scale q.k_i,
+ * carried as (o, m, l) with SE = l*exp(m) (max-shifted, mathematically identical;
+ * reading C1).  Rows come from K/V at K + idx[j]*d (idx NULL => rows 0..n_idx-1). */
+void hko_state_of_set(const hko_config *c, const float *q_g, const float *K, const float *V,
+                      const int32_t *idx, int32_t n_idx, double *o, double *m, double *l) {
+  int32_t d = c->d;
+  for (int32_t e = 0; e < d; ++e) o[e] = 0.0;
+  *m = -INFINITY; *l = 0.0;
+  if (n_idx <= 0) return;
+  double *x = (double *)malloc(sizeof(double) * (size_t)n_idx);
+  for (int32_t j = 0; j < n_idx; ++j) {
+    size_t r = (size_t)(idx ? idx[j] : j) * d;
+    double dot = 0.0;
+    for (int32_t e = 0; e < d; ++e) dot += (double)q_g[e] * (double)K[r + e];
+    x[j] = (double)c->sm_scale * dot;
+    if (x[j] > *m) *m = x[j];
+  }
+  for (int32_t j = 0; j < n_idx; ++j) {
+    size_t r = (size_t)(idx ? idx[j] : j) * d;
+    double w = exp(x[j] - *m);
+    *l += w;
+    for (int32_t e = 0; e < d; ++e) o[e] += w * (double)V[r + e];
+  }
+  for (int32_t e = 0; e < d; ++e) o[e] /= *l;
+  free(x);
+}
+
+/* Merge operator of Eq. 6 (L748-762): o = (o_a SE_a + o_b SE_b)/(SE_a+SE_b),
+ * SE = SE_a + SE_b, with SE = l*exp(m).  An empty state has l = 0 (identity). */
+void hko_merge(int32_t d, double *o_a, double *m_a, double *l_a,
+               const double *o_b, double m_b, double l_b) {
+  if (l_b == 0.0) return;
+  if (*l_a == 0.0) { for (int32_t e = 0; e < d; ++e) o_a[e] = o_b[e]; *m_a = m_b; *l_a = l_b; return; }
+  double m = *m_a > m_b ? *m_a : m_b;
+  double sa = *l_a * exp(*m_a - m), sb = l_b * exp(m_b - m);
+  for (int32_t e = 0; e < d; ++e) o_a[e] = (o_a[e] * sa + o_b[e] * sb) / (sa + sb);
+  *m_a = m; *l_a = sa + sb;
+}
+
+/* ---- attention over D u I u C (L84: "exact full-sequence attention from the
+ * partial attention outputs of three tiers").  D = sinks [0,min(s,n)) and recent
+ * [max(s,n-W), n) read from the base rows; I = the rewritten selected tier;
+ * C = condensed residents.  The calibration temperature is NOT applied here. */
+void hko_attend(const hko_config *c, hko_unit *u, const float *q) {
+  int32_t d = c->d;
+  int32_t s_end = c->sink < u->n ? c->sink : u->n;
+  int32_t r_lo = u->n - c->recent; if (r_lo < s_end) r_lo = s_end;
+  int32_t n_dense = s_end + (u->n - r_lo);
+  int32_t *didx = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_dense > 0 ? n_dense : 1));
+  int32_t t = 0;
+  for (int32_t i = 0; i < s_end; ++i) didx[t++] = i;
+  for (int32_t i = r_lo; i < u->n; ++i) didx[t++] = i;
+  double *o = (double *)malloc(sizeof(double) * (size_t)d * 2);
+  double *o2 = o + d;
+  for (int32_t g = 0; g < c->G; ++g) {
+    const float *qg = q + (size_t)g * d;
+    double m, l, m2, l2;
+    hko_state_of_set(c, qg, u->K, u->V, didx, n_dense, o, &m, &l);               /* Tier 1 */
+    hko_state_of_set(c, qg, u->sel_k, u->sel_v, NULL, u->sel_count, o2, &m2, &l2); /* Tier 2 */
+    hko_merge(d, o, &m, &l, o2, m2, l2);
+    hko_state_of_set(c, qg, u->cond_k, u->cond_v, NULL, u->cond_count, o2, &m2, &l2); /* Tier 3 */
+    hko_merge(d, o, &m, &l, o2, m2, l2);
+    for (int32_t e = 0; e < d; ++e) u->out[(size_t)g * d + e] = (float)o[e];
+    u->lse[g] = (float)(m + log(l));
+  }
+  free(o); free(didx);
+}
+
+/* ---- one decode step in the order of L78 (Step 1 append; Step 4 compaction of the
+ * oldest "before new dense blocks are allocated"; Step 2 calibrated Top-p; Step 3
+ * rewrite) followed by the tiered attention of L84.  do_select = 0 reproduces the
+ * steps between two compressions (L274 "every 128 steps"): the previous selected
+ * tier is reused. */
+void hko_decode_step(const hko_config *c, hko_unit *u, const float *q,
+                     const float *k_new, const float *v_new, float p, int do_select) {
+  hko_append(c, u, k_new, v_new);
+  hko_retire(c, u);
+  if (do_select) {
+    hko_score(c, u, q);
+    hko_calibrate(c, u);
+    hko_topp_select(c, u, p, 1);
+    hko_rewrite(c, u);
+  }
+  hko_attend(c, u, q);
+}
+
+int hko_decode_step_batch(const hko_config *c, hko_unit *units, int32_t n_units,
+                          const float *q, const float *k_new, const float *v_new,
+                          float p, int do_select) {
+  int nthreads = 1;
+#ifdef _OPENMP
+  nthreads = omp_get_max_threads();
+#pragma omp parallel for schedule(dynamic, 1)
+#endif
+  for (int32_t i = 0; i < n_units; ++i)
+    hko_decode_step(c, &units[i], q + (size_t)i * c->G * c->d,
+                    k_new + (size_t)i * c->d, v_new + (size_t)i * c->d, p, do_select);
+  return nthreads;
+}
+
+/* Head-wise block table of the selected tier (L207-209, Fig. 6; reading C9):
+ * entry j is the static physical page id while j < ceil(k/page), else -1. */
+void hko_sel_table(const hko_config *c, const hko_unit *u, const int32_t *sel_pages, int32_t *sel_table) {
+  int32_t used = (u->sel_count + c->page - 1) / c->page;
+  for (int32_t j = 0; j < c->k_cap / c->page; ++j) sel_table[j] = j < used ? sel_pages[j] : -1;
+}
+
+/* Head-wise mask over the whole sequence "packed in uint8 format" (L439):
+ * bit (i % 8) of byte (i / 8), LSB first, set iff position i is selected. */
+void hko_sel_mask(const hko_config *c, const hko_unit *u, uint8_t *mask) {
+  memset(mask, 0, (size_t)(c->max_ctx / 8));
+  for (int32_t j = 0; j < u->sel_count; ++j) {
+    int32_t i = u->sel_idx[j];
+    mask[i / 8] |= (uint8_t)(1u << (i % 8));
+  }
+}

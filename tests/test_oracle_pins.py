@@ -1,0 +1,357 @@
+"""Pins P1-P12 of the CPU oracle: the oracle is checked
+against what the paper and the mathematics fix, never against itself or the CUDA path.
+
+Citations are PAPER.md lines: Top-p/M_k L108, order invariance L116 + Thm D.3,
+budget vs temperature L72-74/L100, exact tiered attention L84, Eq. 4-6,
+votes L86, Tier 3 L76.
+"""
+import itertools
+import math
+
+import numpy as np
+import pytest
+import scipy.special
+import scipy.stats
+import torch
+
+from oracle.oracle import OracleConfig, Unit, merge, state_of_set
+
+
+def _unit(G=4, d=64, n0=200, max_ctx=256, s=4, W=16, k_cap=256, C=8, l_upper=10**6, seed=0, T=1.0, mode=0,
+          l_lower=0, sm_scale=None):
+    rng = np.random.default_rng(seed)
+    cfg = OracleConfig(G=G, d=d, max_ctx=max_ctx, sink=s, recent=W, k_cap=k_cap, cond_cap=C, sm_scale=sm_scale)
+    K0 = rng.standard_normal((n0, d)).astype(np.float32)
+    V0 = rng.standard_normal((n0, d)).astype(np.float32)
+    return cfg, Unit(cfg, K0, V0, l_upper=l_upper, l_lower=l_lower, T=T, score_mode=mode), rng
+
+
+def _set_logits(u: Unit, z):
+    """Write a [G][N] logit block onto the pool of u."""
+    lo, hi = u.pool
+    z = np.atleast_2d(np.asarray(z, np.float32))
+    assert z.shape[1] == hi - lo
+    u.logits[:, lo:hi] = z
+
+
+def _w(P):
+    return np.rint(P.astype(np.float64) * 4294967296.0).astype(np.uint64)
+
+
+# ---- P1: p = 1 => selected = whole pool and the tiered output is dense attention (L84) ---------
+@pytest.mark.parametrize("G,d", [(4, 64), (7, 128)])
+def test_p1_dense_equivalence(G, d):
+    cfg, u, rng = _unit(G=G, d=d, n0=200, max_ctx=256, W=16, k_cap=256)
+    for t in range(5):
+        q = (rng.standard_normal((G, d)) * 1.7).astype(np.float32)
+        kn, vn = rng.standard_normal(d).astype(np.float32), rng.standard_normal(d).astype(np.float32)
+        u.decode_step(q, kn, vn, p=1.0)
+        n = u.n
+        lo, hi = u.pool
+        assert u.sel_count == hi - lo and list(u.sel_idx[:u.sel_count]) == list(range(lo, hi))
+        Kt = torch.tensor(u.K[:n], dtype=torch.float64)[None]
+        Vt = torch.tensor(u.V[:n], dtype=torch.float64)[None]
+        qt = torch.tensor(q, dtype=torch.float64)[:, None, :]
+        ref = torch.nn.functional.scaled_dot_product_attention(qt, Kt.expand(G, -1, -1), Vt.expand(G, -1, -1))
+        np.testing.assert_allclose(u.out, ref[:, 0].numpy(), rtol=0, atol=1e-5)
+        x = (qt[:, 0] @ Kt[0].T) / math.sqrt(d)
+        np.testing.assert_allclose(u.lse, torch.logsumexp(x, -1).numpy(), rtol=0, atol=1e-5)
+
+
+def test_p1_with_condensed_and_retired_is_not_dense_but_subset_exact():
+    """With retirement on, the output is exact attention over D u I u C (L84), checked by SDPA on that set."""
+    cfg, u, rng = _unit(G=2, d=64, n0=120, max_ctx=160, W=8, k_cap=160, C=4, l_upper=60)
+    for t in range(6):
+        q = rng.standard_normal((2, 64)).astype(np.float32)
+        u.decode_step(q, rng.standard_normal(64).astype(np.float32), rng.standard_normal(64).astype(np.float32), p=1.0)
+    live = list(range(cfg.sink)) + list(range(u.c_lo, u.n)) + list(u.cond_pos[:u.cond_count])
+    assert len(set(live)) == len(live)
+    Kt = torch.tensor(u.K[live], dtype=torch.float64)[None].expand(2, -1, -1)
+    Vt = torch.tensor(u.V[live], dtype=torch.float64)[None].expand(2, -1, -1)
+    ref = torch.nn.functional.scaled_dot_product_attention(torch.tensor(q, dtype=torch.float64)[:, None], Kt, Vt)
+    np.testing.assert_allclose(u.out, ref[:, 0].numpy(), atol=1e-5, rtol=0)
+
+
+# ---- score: closed forms (unit-vector queries; LSE identity with the pinned attention state) ---
+def test_score_closed_forms():
+    cfg, u, rng = _unit(G=4, d=64, n0=100, max_ctx=128, W=10, sm_scale=0.25)
+    lo, hi = u.pool
+    q = np.zeros((4, 64), np.float32)
+    for g, (j, a) in enumerate([(0, 1.0), (5, -2.0), (63, 0.5), (17, 3.0)]):
+        q[g, j] = a
+    u.score(q)
+    for g, (j, a) in enumerate([(0, 1.0), (5, -2.0), (63, 0.5), (17, 3.0)]):
+        np.testing.assert_array_equal(u.logits[g, lo:hi], (np.float64(0.25) * a * u.K[lo:hi, j].astype(np.float64)).astype(np.float32))
+    q = rng.standard_normal((4, 64)).astype(np.float32)
+    u.score(q)
+    for g in range(4):   # log-sum-exp of the scores == LSE of the attention state over the same rows
+        _, m, l = state_of_set(cfg, q[g], u.K, u.V, np.arange(lo, hi))
+        assert abs(scipy.special.logsumexp(u.logits[g, lo:hi].astype(np.float64)) - (m + math.log(l))) < 1e-5
+
+
+# ---- calibrate: reduces to a library softmax; group mean; temperature; ACCUM window -------------
+@pytest.mark.parametrize("G,T", [(1, 1.0), (4, 1.0), (5, 0.5), (3, 2.5)])
+def test_calibrate_is_mean_of_library_softmax(G, T):
+    cfg, u, rng = _unit(G=G, d=64, n0=300, max_ctx=320, W=20, T=T)
+    lo, hi = u.pool
+    z = rng.standard_normal((G, hi - lo)) * 3
+    _set_logits(u, z)
+    u.calibrate()
+    ref = scipy.special.softmax(u.logits[:, lo:hi].astype(np.float64) / T, axis=1).mean(0)
+    np.testing.assert_allclose(u.probs[lo:hi], ref, rtol=2e-7, atol=0)
+    assert abs(u.probs[lo:hi].astype(np.float64).sum() - 1) < 1e-5
+
+
+def test_accum_is_sliding_window_sum():
+    """ACCUM == 'accumulated attention over the last w steps' (BASELINE config 4, reading C4), renormalised."""
+    w = 4
+    rng = np.random.default_rng(3)
+    cfg = OracleConfig(G=2, d=64, max_ctx=128, sink=2, recent=8, k_cap=128, cond_cap=4, accum_window=w)
+    u = Unit(cfg, rng.standard_normal((60, 64)).astype(np.float32), rng.standard_normal((60, 64)).astype(np.float32),
+             l_upper=55, score_mode=1)
+    rows = []
+    for t in range(11):
+        u.append(rng.standard_normal(64).astype(np.float32), rng.standard_normal(64).astype(np.float32))
+        u.retire()
+        lo, hi = u.pool
+        z = rng.standard_normal((2, hi - lo)) * 2
+        _set_logits(u, z)
+        u.calibrate()
+        row = np.zeros(cfg.max_ctx)
+        row[lo:hi] = scipy.special.softmax(u.logits[:, lo:hi].astype(np.float64), axis=1).mean(0)
+        rows.append(row)
+        ref = np.sum(rows[-w:], axis=0)[lo:hi]
+        np.testing.assert_allclose(u.probs[lo:hi], ref / ref.sum(), rtol=5e-6, atol=1e-9)
+
+
+# ---- P2: brute force minimality on tiny pools (L108) --------------------------------------------
+@pytest.mark.parametrize("seed", range(12))
+def test_p2_bruteforce_minimal_nucleus(seed):
+    rng = np.random.default_rng(100 + seed)
+    N = int(rng.integers(3, 13))
+    W = 4
+    cfg, u, _ = _unit(G=1, d=64, n0=4 + N + W, max_ctx=64, s=4, W=W, k_cap=64)
+    P = rng.dirichlet(np.ones(N) * rng.choice([0.2, 1.0, 5.0])).astype(np.float32)
+    if seed % 3 == 0:
+        P[rng.integers(0, N, 3)] = P[0]      # force ties
+    lo, hi = u.pool
+    assert hi - lo == N
+    u.probs[lo:hi] = P
+    p = np.float32(rng.choice([0.5, 0.8, 0.9, 0.95]))
+    u.topp_select(float(p), count_votes=False)
+    w = _w(P)
+    theta = max(1, math.ceil(float(np.float64(p) * np.float64(int(w.sum())))))
+    sel = np.array(u.sel_idx[:u.sel_count]) - lo
+    k = len(sel)
+    assert int(w[sel].sum()) >= theta                                             # mass >= p
+    for r in range(k):                                                            # no smaller subset reaches it
+        for sub in itertools.combinations(range(N), r):
+            assert int(w[list(sub)].sum()) < theta
+    unsel = np.setdiff1d(np.arange(N), sel)
+    if len(unsel):
+        assert P[sel].min() >= P[unsel].max()                                     # a prefix of the sorted order
+        ties = unsel[P[unsel] == P[sel].min()]
+        sel_ties = sel[P[sel] == P[sel].min()]
+        if len(ties):
+            assert sel_ties.max() < ties.min()                                    # ties: position ascending
+    assert int(w[sel].sum()) - int(w[sel].min()) < theta                          # dropping the last falls below
+    assert list(sel) == sorted(sel)
+
+
+# ---- P3 ties, P4 degenerate, P5 closed form -----------------------------------------------------
+def test_p3_all_equal():
+    cfg, u, _ = _unit(G=1, d=64, n0=4 + 1000 + 16, max_ctx=1024, W=16, k_cap=1024)
+    _set_logits(u, np.zeros((1, 1000)))
+    u.calibrate()
+    u.topp_select(0.9)
+    lo, _ = u.pool
+    assert u.sel_count == 900 and list(u.sel_idx[:900]) == list(range(lo, lo + 900))
+    assert (u.votes[lo:lo + 900] == 1).all() and u.votes.sum() == 900
+
+
+def test_p4_one_dominant():
+    cfg, u, rng = _unit(G=1, d=64, n0=4 + 500 + 16, max_ctx=528, W=16, k_cap=528)
+    z = rng.standard_normal((1, 500)); z[0, 123] += 40
+    _set_logits(u, z)
+    u.calibrate(); u.topp_select(0.9)
+    assert u.sel_count == 1 and u.sel_idx[0] == u.pool[0] + 123
+
+
+@pytest.mark.parametrize("p,expect", [(0.9, 231), (0.95, 300)])
+def test_p5_geometric_closed_form(p, expect):
+    lam, N = 0.01, 2000
+    r = math.exp(-lam)
+    assert math.ceil(math.log(1 - p * (1 - r ** N)) / math.log(r)) == expect
+    cfg, u, _ = _unit(G=1, d=64, n0=4 + N + 16, max_ctx=2048, W=16, k_cap=2048)
+    _set_logits(u, -lam * np.arange(N)[None, :])
+    u.calibrate(); u.topp_select(p)
+    assert u.sel_count == expect and list(u.sel_idx[:expect]) == list(range(4, 4 + expect))
+
+
+# ---- P6: order invariance under T > 0 (Constraint 1 L116, Thm D.3) and nesting in p -------------
+def test_p6_temperature_and_p_nesting():
+    rng = np.random.default_rng(6)
+    N = 3000
+    z = rng.standard_normal((1, N)) * 2
+    sets, ks = [], []
+    for T in (0.5, 1.0, 2.0, 4.0):
+        cfg, u, _ = _unit(G=1, d=64, n0=4 + N + 16, max_ctx=3072, W=16, k_cap=3072, T=T)
+        _set_logits(u, z)
+        u.calibrate(); u.topp_select(0.9)
+        sets.append(set(u.sel_idx[:u.sel_count])); ks.append(u.sel_count)
+        order = np.argsort(-u.probs[4:4 + N], kind="stable")       # Top-k set == k largest raw logits
+        assert sets[-1] == set(4 + np.argsort(-u.logits[0, 4:4 + N], kind="stable")[:ks[-1]]) == set(4 + order[:ks[-1]])
+    assert all(a <= b + 1 for a, b in zip(ks, ks[1:])) and ks[0] < ks[-1]          # k(T) non-decreasing
+    assert all(a <= b for a, b in zip(sets, sets[1:]))                             # nested prefixes of one order
+    cfg, u, _ = _unit(G=4, d=64, n0=4 + N + 16, max_ctx=3072, W=16, k_cap=3072)
+    _set_logits(u, rng.standard_normal((4, N)) * 2)
+    u.calibrate()
+    prev = set()
+    for p in (0.5, 0.8, 0.9, 0.95, 0.99, 1.0):
+        u.topp_select(p, count_votes=False)
+        cur = set(u.sel_idx[:u.sel_count])
+        assert prev <= cur
+        prev = cur
+    assert len(prev) == N
+
+
+# ---- P7: per-head budgets follow the logit temperature (L72-74, L100) ---------------------------
+@pytest.mark.parametrize("p,sigma", [(0.95, 1.0), (0.95, 2.0), (0.9, 0.5), (0.9, 1.5)])
+def test_p7_gaussian_budget_law(p, sigma):
+    """iid N(0,sigma^2) logits: k/N -> Phi(Phi^-1(p) - sigma) (lognormal weights, size-biased tail)."""
+    N = 16384
+    rng = np.random.default_rng(int(sigma * 10) + int(p * 100))
+    cfg, u, _ = _unit(G=1, d=64, n0=4 + N + 16, max_ctx=16416, W=16, k_cap=16416)
+    _set_logits(u, rng.standard_normal((1, N)) * sigma)
+    u.calibrate(); u.topp_select(p)
+    expect = scipy.stats.norm.cdf(scipy.stats.norm.ppf(p) - sigma)
+    assert abs(u.sel_count / N - expect) < 0.03          # 3 % of N (heavy lognormal tail at sigma=2)
+
+
+# ---- P8: merge operator algebra (Eq. 6) -----------------------------------------------------------
+def test_p8_merge_algebra():
+    rng = np.random.default_rng(8)
+    d, n = 64, 90
+    cfg = OracleConfig(G=1, d=d, max_ctx=128, sink=0, recent=0, k_cap=16, cond_cap=0)
+    K = (rng.standard_normal((n, d)) * 2).astype(np.float32); V = rng.standard_normal((n, d)).astype(np.float32)
+    q = rng.standard_normal(d).astype(np.float32)
+    full = state_of_set(cfg, q, K, V, np.arange(n))
+    ref = torch.nn.functional.scaled_dot_product_attention(
+        torch.tensor(q, dtype=torch.float64)[None, None], torch.tensor(K, dtype=torch.float64)[None],
+        torch.tensor(V, dtype=torch.float64)[None])[0, 0].numpy()
+    np.testing.assert_allclose(full[0], ref, atol=1e-12)
+    for trial in range(5):
+        lab = rng.integers(0, 3, n)
+        parts = [state_of_set(cfg, q, K, V, np.flatnonzero(lab == j)) for j in range(3)]
+        for order in itertools.permutations(range(3)):                     # commutative + associative
+            left = merge(merge(parts[order[0]], parts[order[1]]), parts[order[2]])
+            right = merge(parts[order[0]], merge(parts[order[1]], parts[order[2]]))
+            for st in (left, right):
+                np.testing.assert_allclose(st[0], full[0], rtol=1e-9, atol=1e-12)
+                assert abs(st[1] + math.log(st[2]) - (full[1] + math.log(full[2]))) < 1e-9
+    empty = state_of_set(cfg, q, K, V, np.zeros(0, np.int32))
+    assert empty[2] == 0.0
+    for st in (merge(full, empty), merge(empty, full)):                    # identity
+        np.testing.assert_array_equal(st[0], full[0]); assert st[1:] == full[1:]
+
+
+# ---- P9: rewrite copies, pads and table (L172, reading C9) ---------------------------------------
+def test_p9_rewrite_and_table():
+    cfg, u, rng = _unit(G=2, d=64, n0=300, max_ctx=320, W=16, k_cap=128)
+    u.score(rng.standard_normal((2, 64)).astype(np.float32) * 3); u.calibrate(); u.topp_select(0.7)
+    u.sel_k[:] = 7.0; u.sel_v[:] = 7.0
+    u.rewrite()
+    k = u.sel_count
+    assert 0 < k < 128 and k % 16 != 0
+    idx = u.sel_idx[:k]
+    assert (np.diff(idx) > 0).all() and (u.sel_idx[k:] == -1).all()
+    assert u.sel_k[:k].tobytes() == u.K[idx].tobytes() and u.sel_v[:k].tobytes() == u.V[idx].tobytes()
+    end = -(-k // 16) * 16
+    assert (u.sel_k[k:end] == 0).all() and (u.sel_v[k:end] == 0).all() and (u.sel_k[end:] == 7.0).all()
+    pages = np.arange(100, 108, dtype=np.int32)
+    tab = u.sel_table(pages)
+    assert list(tab[:end // 16]) == list(pages[:end // 16]) and (tab[end // 16:] == -1).all()
+    mask = u.sel_mask()
+    bits = np.unpackbits(mask, bitorder="little")
+    assert set(np.flatnonzero(bits)) == set(idx)
+
+
+# ---- P10 / P11: condensed tier == top-C_cap of the retirement log; bookkeeping invariants ---------
+def test_p10_p11_condensed_and_bookkeeping():
+    C = 6
+    cfg, u, rng = _unit(G=2, d=64, n0=150, max_ctx=256, s=4, W=12, k_cap=48, C=C, l_upper=100)
+    log = []                                     # (votes at retirement, pos)
+    total_sel = 0
+    for t in range(70):
+        q = rng.standard_normal((2, 64)).astype(np.float32) * 4
+        c_before, votes_before = u.c_lo, u.votes.copy()
+        u.decode_step(q, rng.standard_normal(64).astype(np.float32), rng.standard_normal(64).astype(np.float32), p=0.6)
+        for pos in range(c_before, u.c_lo):
+            log.append((int(votes_before[pos]), pos))
+        total_sel += u.sel_count
+        lo, hi = u.pool
+        # P11
+        assert hi - lo <= 100 and u.sel_count <= cfg.k_cap and u.cond_count <= C
+        sel = u.sel_idx[:u.sel_count]
+        assert ((sel >= lo) & (sel < hi)).all() and u.votes.sum() == total_sel
+        dense = set(range(cfg.sink)) | set(range(hi, u.n))
+        assert dense | set(range(lo, hi)) | {p for _, p in log} == set(range(u.n))
+        assert len(dense) + (hi - lo) + len(log) == u.n
+        # P10
+        want = sorted(log, reverse=True)[:C]
+        have = sorted(zip(u.cond_votes[:u.cond_count].tolist(), u.cond_pos[:u.cond_count].tolist()), reverse=True)
+        assert have == want
+        for j in range(u.cond_count):
+            assert u.cond_k[j].tobytes() == u.K[u.cond_pos[j]].tobytes()
+            assert u.cond_v[j].tobytes() == u.V[u.cond_pos[j]].tobytes()
+    assert len(log) > 3 * C and u.sel_count == cfg.k_cap or u.k_topp <= cfg.k_cap
+
+
+def test_k_cap_clamp_keeps_best_of_same_order():
+    cfg, u, rng = _unit(G=1, d=64, n0=4 + 400 + 16, max_ctx=432, W=16, k_cap=32)
+    _set_logits(u, rng.standard_normal((1, 400)) * 0.3)
+    u.calibrate(); u.topp_select(0.95)
+    assert u.k_topp > 32 and u.sel_count == 32
+    best = 4 + np.argsort(-u.probs[4:404], kind="stable")[:32]
+    assert set(u.sel_idx[:32]) == set(best)
+
+
+def test_l_lower_selects_everything():
+    cfg, u, rng = _unit(G=1, d=64, n0=4 + 100 + 16, max_ctx=128, W=16, k_cap=128, l_lower=100)
+    _set_logits(u, rng.standard_normal((1, 100)) * 3)
+    u.calibrate(); u.topp_select(0.5)
+    assert u.sel_count == 100
+
+
+# ---- P12: integer mass vs fp64 sorted cumsum ----------------------------------------------------
+@pytest.mark.parametrize("seed", range(4))
+def test_p12_integer_mass_vs_real(seed):
+    rng = np.random.default_rng(1200 + seed)
+    N = 5000
+    cfg, u, _ = _unit(G=2, d=64, n0=4 + N + 16, max_ctx=5024, W=16, k_cap=5024)
+    _set_logits(u, rng.standard_normal((2, N)) * rng.choice([0.5, 1.5, 3.0]))
+    u.calibrate(); u.topp_select(0.9, count_votes=False)
+    P = np.sort(u.probs[4:4 + N].astype(np.float64))[::-1]
+    cum = np.cumsum(P) / P.sum()
+    k_real = int(np.searchsorted(cum, 0.9) + 1)
+    k_int = u.sel_count
+    a, b = sorted((k_real, k_int))
+    assert all(abs(cum[j - 1] - 0.9) <= N * 2.0 ** -33 + 1e-7 for j in range(a, b + 1)) or a == b
+
+
+def test_empty_pool_and_short_context():
+    cfg = OracleConfig(G=2, d=64, max_ctx=64, sink=4, recent=16, k_cap=32, cond_cap=4)
+    rng = np.random.default_rng(0)
+    u = Unit(cfg, rng.standard_normal((3, 64)).astype(np.float32), rng.standard_normal((3, 64)).astype(np.float32), l_upper=8)
+    for t in range(30):
+        q = rng.standard_normal((2, 64)).astype(np.float32)
+        u.decode_step(q, rng.standard_normal(64).astype(np.float32), rng.standard_normal(64).astype(np.float32), p=0.9)
+        lo, hi = u.pool
+        assert hi - lo == max(0, min(u.n - 16 - 4, 8))
+        if u.n <= 20:
+            assert u.sel_count == 0
+            n = u.n
+            Kt = torch.tensor(u.K[:n], dtype=torch.float64)[None].expand(2, -1, -1)
+            Vt = torch.tensor(u.V[:n], dtype=torch.float64)[None].expand(2, -1, -1)
+            ref = torch.nn.functional.scaled_dot_product_attention(torch.tensor(q, dtype=torch.float64)[:, None], Kt, Vt)
+            np.testing.assert_allclose(u.out, ref[:, 0].numpy(), atol=1e-5, rtol=0)
