@@ -1,0 +1,126 @@
+/*
+ * hardkv.h -- C ABI of libhardkv.so: the per-decode-step hot path of HARD-KV
+ * (arxiv/paper_2606_28831) as hand-written sm_100a CUDA kernels.
+ *
+ * One call = one stage of the paper's pipeline ("linearly append KV
+ * pairs to the Tier 1 Dense Cache" -> "Logits Calibration ... Top-p sampling" ->
+ * "Index Regularization" -> eviction of the oldest blocks) followed by the tiered
+ * attention of L84 / Appendix F, for ONE layer, for every (sequence b, KV head h).
+ *
+ * Conventions (all entry points)
+ *  - Every pointer inside hardkv_state, and q / k_new / v_new / out / lse, is a
+ *    DEVICE pointer owned by the caller.  hardkv_config / hardkv_state structs
+ *    themselves and `bytes`/`out` arguments of the create calls are HOST memory.
+ *  - The library allocates nothing, never synchronises, never reads device data
+ *    back to the host, and launches only on the stream passed in: every stage call
+ *    is CUDA-Graph capturable (L53, L63, L168: static shapes, persistent pointers).
+ *    Data-dependent sizes (per-head budget k_h, context length) stay on the device;
+ *    grids are sized for the static capacities and exit early.
+ *  - Return value: HARDKV_OK or an error detectable on the host (bad config,
+ *    unsupported (dtype, head_dim, G), NULL required pointer, workspace too small,
+ *    a failed launch).  Nothing throws across the ABI.  Inconsistencies only the
+ *    device can see (ctx_len >= max_ctx on append) set *err_flag != 0 and leave the
+ *    unit untouched; the caller reads the flag after synchronising.
+ *  - Layouts (row = head_dim elements of kv_dtype; page = page_size rows):
+ *      k_pool, v_pool         [n_pages][page][d]
+ *      base_table             [B][Hkv][max_ctx/page]   physical page of logical page j
+ *      sel_k_pool, sel_v_pool [n_sel_pages][page][d]
+ *      sel_pages              [B][Hkv][k_cap/page]     static physical ids (L207-209, L498:
+ *                                                      the same id addresses every layer)
+ *      cond_k, cond_v         [B][Hkv][cond_cap][d]
+ *      q                      [B][Hq][d] kv_dtype, query head g of KV head h is h*G+g
+ *      out                    [B][Hq][d] f32,  lse [B][Hq] f32
+ *      logits                 [B][Hq][max_ctx] f32 (valid on the pool)
+ *      probs                  [B][Hkv][max_ctx] f32 (valid on the pool)
+ *  - "pool" of sequence b = positions [c_lo[b], max(c_lo[b], ctx_len[b]-recent)):
+ *    Tier-2 candidates (L72); dense tier = [0,sink) u [ctx_len-recent, ctx_len) (L71).
+ */
+#ifndef HARDKV_H
+#define HARDKV_H
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hardkv_ctx hardkv_ctx;        /* opaque, host-side only */
+typedef struct CUstream_st *hardkv_stream;   /* == cudaStream_t */
+
+typedef enum {
+  HARDKV_OK = 0,
+  HARDKV_ERR_INVALID_ARG = 1,
+  HARDKV_ERR_UNSUPPORTED = 2,   /* (kv_dtype, head_dim, G, page_size) not built */
+  HARDKV_ERR_WORKSPACE = 3,
+  HARDKV_ERR_CUDA = 4
+} hardkv_status;
+
+typedef enum { HARDKV_F32 = 0, HARDKV_BF16 = 1 } hardkv_dtype;
+typedef enum { HARDKV_SCORE_RAW = 0, HARDKV_SCORE_ACCUM = 1 } hardkv_score_mode;
+
+/* Static for the lifetime of a ctx (and of any graph captured with it). */
+typedef struct {
+  int32_t batch, num_q_heads, num_kv_heads, head_dim, page_size; /* page_size must be 16            */
+  int32_t max_ctx;        /* static capacity in tokens per sequence, multiple of page_size          */
+  int32_t sink, recent;   /* s, W: dense tier (L71, L276-277 "sinks + local window")                */
+  int32_t k_cap;          /* selected-tier capacity in tokens, multiple of page_size (L233)         */
+  int32_t cond_cap;       /* C_cap: constant size of the condensed tier (L76)                       */
+  int32_t accum_window;   /* ring depth of SCORE_ACCUM heads (<= 0: no ACCUM state)                 */
+  int32_t kv_dtype;       /* hardkv_dtype of q, K, V                                                */
+  float   sm_scale;       /* <= 0: 1/sqrt(head_dim)                                                 */
+} hardkv_config;
+
+/* Caller-owned device state of one layer.  Pointers marked (opt) may be NULL. */
+typedef struct {
+  void *k_pool, *v_pool;            const int32_t *base_table;
+  void *sel_k_pool, *sel_v_pool;    const int32_t *sel_pages;
+  void *cond_k, *cond_v;            int32_t *cond_pos, *cond_votes, *cond_count; /* [B][Hkv][C], [B][Hkv]  */
+  int32_t *ctx_len, *c_lo;          const int32_t *l_lower, *l_upper;           /* [B] each               */
+  int32_t *votes;                                                               /* [B][Hkv][max_ctx]      */
+  const float *temperature;         const uint8_t *score_mode;                  /* [B][Hkv], [Hkv]        */
+  float *acc, *ring;                int32_t *ring_slot;  /* (opt) ACCUM: [B][Hkv][max_ctx], [B][Hkv][win][max_ctx], [B][Hkv] */
+  int32_t *sel_idx, *sel_count, *sel_table;  /* [B][Hkv][k_cap] asc. positions pad -1, [B][Hkv], [B][Hkv][k_cap/page] */
+  uint8_t *sel_mask;                /* (opt) [B][Hkv][max_ctx/8], bit i%8 of byte i/8 (L439)                */
+  float *logits, *probs;
+  int32_t *err_flag;                /* one device int                                                    */
+} hardkv_state;
+
+/* Scratch the caller must provide to hardkv_create (device memory, 256-byte aligned). */
+hardkv_status hardkv_workspace_bytes(const hardkv_config *cfg, size_t *bytes);
+/* Validates cfg and records the workspace.  The caller zeroes the workspace once
+ * (it holds arrival counters) before the first stage call; kernels restore the zeros. */
+hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t bytes, hardkv_ctx **out);
+void          hardkv_destroy(hardkv_ctx *ctx);
+const char   *hardkv_status_string(hardkv_status s);
+/* Kernel variant switch for A/B measurements: 0 = generic FMA kernels, 1 = tuned paths (default). */
+hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant);
+
+/* Step 1 + Step 4 of L78.  Writes (k_new, v_new) [B][Hkv][d] at position ctx_len[b];
+ * ctx_len += 1; while the pool exceeds l_upper[b] its oldest token retires into the
+ * condensed tier of every head, ranked on its Cautious-Update votes (L76, L86). */
+hardkv_status hardkv_append_kv(hardkv_ctx *, const hardkv_state *, const void *k_new, const void *v_new,
+                               hardkv_stream);
+/* logits[b][h*G+g][i] = sm_scale * q . K[i] over the pool (exponent of Eq. 4). */
+hardkv_status hardkv_score(hardkv_ctx *, const hardkv_state *, const void *q, hardkv_stream);
+/* Logits Calibration (apply-T) -> probs, then hardkv_topp_select. */
+hardkv_status hardkv_calibrate_topp(hardkv_ctx *, const hardkv_state *, float p, hardkv_stream);
+/* Top-p nucleus (L108) on state->probs as given: integer mass w_i = rn(P_i 2^32),
+ * order (P bits desc, position asc), minimal prefix with mass >= ceil(p * sum w),
+ * clamped to k_cap (L233).  Writes sel_idx, sel_count, sel_table, (sel_mask), votes += 1. */
+hardkv_status hardkv_topp_select(hardkv_ctx *, const hardkv_state *, float p, hardkv_stream);
+/* Rewrite Cache (L172): gather the selected rows into the contiguous selected tier. */
+hardkv_status hardkv_rewrite(hardkv_ctx *, const hardkv_state *, hardkv_stream);
+/* Split-K decode attention over dense + selected + condensed tiers merged by Eq. 6 (L748-762). */
+hardkv_status hardkv_decode_attn(hardkv_ctx *, const hardkv_state *, const void *q, float *out,
+                                 float *lse /* nullable */, hardkv_stream);
+/* The whole step on one stream: append, retire, score, calibrate + Top-p, rewrite fused
+ * with attention (selected rows are read once).  do_select = 0 skips score/select/rewrite
+ * and attends over the previous selected tier (the steps between two compressions, L274). */
+hardkv_status hardkv_decode_step(hardkv_ctx *, const hardkv_state *, const void *q, const void *k_new,
+                                 const void *v_new, float p, int32_t do_select, float *out,
+                                 float *lse /* nullable */, hardkv_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

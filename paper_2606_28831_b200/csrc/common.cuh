@@ -1,0 +1,82 @@
+// common.cuh -- shared device helpers of libhardkv (sm_100a). Product code: never includes oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/hardkv.h"
+
+namespace hardkv {
+
+constexpr int PAGE = 16;
+
+// Everything a kernel needs, passed by value (no device-side config object to keep in sync).
+struct Params {
+  int B, Hq, Hkv, G, d, max_ctx, sink, recent, k_cap, cond_cap, accum_window;
+  int ppu;        // base pages per unit  = max_ctx / PAGE
+  int spu;        // selected pages per unit = k_cap / PAGE
+  int att_chunks; // static number of attention chunks per unit
+  float sm_scale;
+  hardkv_state st;
+  // workspace
+  float *part;          // [units][att_chunks][G][d + 2] split-K partial states (m, l, acc[d])
+  int32_t *att_arrive;  // [units] arrival counters of the split-K merge (zero between launches)
+  float *stat_part;     // [units][G][score_chunks][2] per-chunk softmax statistics (m, s)
+  int score_chunks;
+};
+
+// ---- 16-byte vector access -------------------------------------------------------------------
+__device__ __forceinline__ uint4 ldg_nc(const void *p) {   // streaming read-only data (K, V rows)
+  uint4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ uint4 ldg_ca(const void *p) { return *reinterpret_cast<const uint4 *>(p); }
+__device__ __forceinline__ void stg(void *p, uint4 v) { *reinterpret_cast<uint4 *>(p) = v; }
+
+// Elements per 16-byte vector and their widening to fp32 (bf16 -> fp32 is exact: a 16-bit shift).
+template <typename T> struct Elem;
+template <> struct Elem<float> {
+  static constexpr int EPL = 4;
+  __device__ static __forceinline__ void unpack(const uint4 &r, float (&f)[4]) {
+    f[0] = __uint_as_float(r.x); f[1] = __uint_as_float(r.y);
+    f[2] = __uint_as_float(r.z); f[3] = __uint_as_float(r.w);
+  }
+};
+struct bf16_t { uint16_t bits; };
+template <> struct Elem<bf16_t> {
+  static constexpr int EPL = 8;
+  __device__ static __forceinline__ void unpack(const uint4 &r, float (&f)[8]) {
+    f[0] = __uint_as_float(r.x << 16); f[1] = __uint_as_float(r.x & 0xffff0000u);
+    f[2] = __uint_as_float(r.y << 16); f[3] = __uint_as_float(r.y & 0xffff0000u);
+    f[4] = __uint_as_float(r.z << 16); f[5] = __uint_as_float(r.z & 0xffff0000u);
+    f[6] = __uint_as_float(r.w << 16); f[7] = __uint_as_float(r.w & 0xffff0000u);
+  }
+};
+
+// Address of row `pos` of a unit in a paged pool (table holds the physical page of logical page pos/16).
+template <typename T, int D>
+__device__ __forceinline__ const char *paged_row(const void *pool, const int32_t *table_unit, int pos) {
+  int page = __ldg(table_unit + (pos >> 4));
+  return reinterpret_cast<const char *>(pool) + ((size_t)page * PAGE + (pos & 15)) * (D * sizeof(T));
+}
+
+// Pool bounds of sequence b (Tier-2 address range): [lo, hi).
+__device__ __forceinline__ void pool_bounds(const Params &P, int b, int &n, int &lo, int &hi) {
+  n = P.st.ctx_len[b];
+  lo = P.st.c_lo[b];
+  hi = n - P.recent;
+  if (hi < lo) hi = lo;
+}
+
+__device__ __forceinline__ unsigned long long shfl_xor_u64(unsigned long long v, int off) {
+  unsigned lo = __shfl_xor_sync(0xffffffffu, (unsigned)v, off);
+  unsigned hi = __shfl_xor_sync(0xffffffffu, (unsigned)(v >> 32), off);
+  return ((unsigned long long)hi << 32) | lo;
+}
+__device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {
+#pragma unroll
+  for (int o = 16; o; o >>= 1) v += shfl_xor_u64(v, o);
+  return v;
+}
+
+}  // namespace hardkv

@@ -1,0 +1,244 @@
+// hardkv.cu -- C ABI of libhardkv.so (include/hardkv.h): argument checks, kernel dispatch on
+// (kv_dtype, head_dim, G), stream-ordered launches only.  No allocation, no synchronisation.
+#include <math.h>
+#include <new>
+#include <string.h>
+
+#include "common.cuh"
+#include "select_kernel.cuh"
+#include "stage_kernels.cuh"
+
+using namespace hardkv;
+
+struct hardkv_ctx {
+  hardkv_config cfg;
+  Params base;      // config-derived fields + workspace pointers; `st` is filled per call
+  int variant;
+  size_t ws_bytes;
+};
+
+namespace {
+
+size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
+struct WsLayout { size_t part, arrive, total; };
+
+int att_chunks_of(const hardkv_config &c) {
+  return (c.sink + c.recent + c.k_cap + c.cond_cap + ATT_CHUNK - 1) / ATT_CHUNK;
+}
+
+WsLayout ws_layout(const hardkv_config &c) {
+  const size_t units = (size_t)c.batch * c.num_kv_heads;
+  const int G = c.num_q_heads / c.num_kv_heads;
+  WsLayout w;
+  size_t off = 0;
+  w.arrive = off; off += align256(units * sizeof(int32_t));
+  w.part = off;   off += align256(units * att_chunks_of(c) * G * (c.head_dim + 2) * sizeof(float));
+  w.total = off;
+  return w;
+}
+
+hardkv_status check_config(const hardkv_config *c) {
+  if (!c) return HARDKV_ERR_INVALID_ARG;
+  if (c->batch <= 0 || c->num_q_heads <= 0 || c->num_kv_heads <= 0 || c->head_dim <= 0) return HARDKV_ERR_INVALID_ARG;
+  if (c->num_q_heads % c->num_kv_heads) return HARDKV_ERR_INVALID_ARG;
+  if (c->max_ctx <= 0 || c->k_cap <= 0 || c->sink < 0 || c->recent < 0 || c->cond_cap < 0) return HARDKV_ERR_INVALID_ARG;
+  if (c->page_size != PAGE) return HARDKV_ERR_UNSUPPORTED;
+  if (c->max_ctx % PAGE || c->k_cap % PAGE) return HARDKV_ERR_INVALID_ARG;
+  const int G = c->num_q_heads / c->num_kv_heads;
+  const bool gok = G == 1 || G == 2 || G == 4 || G == 5 || G == 7 || G == 8;
+  const bool tok = (c->kv_dtype == HARDKV_F32 && c->head_dim == 64) ||
+                   (c->kv_dtype == HARDKV_BF16 && (c->head_dim == 64 || c->head_dim == 128));
+  if (!gok || !tok) return HARDKV_ERR_UNSUPPORTED;
+  return HARDKV_OK;
+}
+
+hardkv_status launch_status() { return cudaPeekAtLastError() == cudaSuccess ? HARDKV_OK : HARDKV_ERR_CUDA; }
+
+bool state_ok(const hardkv_ctx *ctx, const hardkv_state *s) {
+  if (!ctx || !s) return false;
+  return s->k_pool && s->v_pool && s->base_table && s->sel_k_pool && s->sel_v_pool && s->sel_pages &&
+         s->cond_count && s->ctx_len && s->c_lo && s->l_lower && s->l_upper && s->votes && s->temperature &&
+         s->score_mode && s->sel_idx && s->sel_count && s->sel_table && s->logits && s->probs && s->err_flag &&
+         (ctx->cfg.cond_cap == 0 || (s->cond_k && s->cond_v && s->cond_pos && s->cond_votes));
+}
+
+Params params_of(const hardkv_ctx *ctx, const hardkv_state *s) {
+  Params P = ctx->base;
+  P.st = *s;
+  return P;
+}
+
+// Dispatch on (dtype, head_dim) and on G where the kernel keeps per-head registers.
+#define HK_DISPATCH_TD(cfg, ...)                                                                   \
+  do {                                                                                             \
+    if ((cfg).kv_dtype == HARDKV_F32) { using T = float; constexpr int D = 64; __VA_ARGS__; }      \
+    else if ((cfg).head_dim == 128) { using T = bf16_t; constexpr int D = 128; __VA_ARGS__; }      \
+    else { using T = bf16_t; constexpr int D = 64; __VA_ARGS__; }                                  \
+  } while (0)
+
+#define HK_DISPATCH_G(Gv, ...)                                                                     \
+  do {                                                                                             \
+    switch (Gv) {                                                                                  \
+      case 1: { constexpr int G = 1; __VA_ARGS__; } break;                                         \
+      case 2: { constexpr int G = 2; __VA_ARGS__; } break;                                         \
+      case 4: { constexpr int G = 4; __VA_ARGS__; } break;                                         \
+      case 5: { constexpr int G = 5; __VA_ARGS__; } break;                                         \
+      case 7: { constexpr int G = 7; __VA_ARGS__; } break;                                         \
+      default: { constexpr int G = 8; __VA_ARGS__; } break;                                        \
+    }                                                                                              \
+  } while (0)
+
+void launch_append(const hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, cudaStream_t st) {
+  HK_DISPATCH_TD(ctx->cfg, (append_retire_kernel<T, D><<<P.B, 256, 0, st>>>(P, k_new, v_new)));
+}
+
+void launch_score(const hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
+  dim3 grid((P.ppu + SCORE_PAGES_PER_CTA - 1) / SCORE_PAGES_PER_CTA, P.B * P.Hkv);
+  HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (score_generic_kernel<T, D, G><<<grid, 256, 0, st>>>(P, q))));
+}
+
+void launch_select(const hardkv_ctx *, const Params &P, float p, bool calibrate, cudaStream_t st) {
+  if (calibrate) select_kernel<1><<<P.B * P.Hkv, SEL_NT, SEL_SMEM, st>>>(P, p);
+  else select_kernel<0><<<P.B * P.Hkv, SEL_NT, SEL_SMEM, st>>>(P, p);
+}
+
+void launch_rewrite(const hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
+  dim3 grid((P.k_cap + RW_ROWS_PER_CTA - 1) / RW_ROWS_PER_CTA, P.B * P.Hkv);
+  HK_DISPATCH_TD(ctx->cfg, (rewrite_kernel<T, D><<<grid, 256, 0, st>>>(P)));
+}
+
+void launch_attend(const hardkv_ctx *ctx, const Params &P, const void *q, float *out, float *lse, bool fused,
+                   cudaStream_t st) {
+  dim3 grid(P.att_chunks, P.B * P.Hkv);
+  if (fused)
+    HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, true><<<grid, 256, 0, st>>>(P, q, out, lse))));
+  else
+    HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, false><<<grid, 256, 0, st>>>(P, q, out, lse))));
+}
+
+}  // namespace
+
+extern "C" {
+
+const char *hardkv_status_string(hardkv_status s) {
+  switch (s) {
+    case HARDKV_OK: return "ok";
+    case HARDKV_ERR_INVALID_ARG: return "invalid argument";
+    case HARDKV_ERR_UNSUPPORTED: return "unsupported (kv_dtype, head_dim, G, page_size)";
+    case HARDKV_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
+    case HARDKV_ERR_CUDA: return "CUDA launch error";
+  }
+  return "unknown status";
+}
+
+hardkv_status hardkv_workspace_bytes(const hardkv_config *cfg, size_t *bytes) {
+  if (!bytes) return HARDKV_ERR_INVALID_ARG;
+  hardkv_status s = check_config(cfg);
+  if (s != HARDKV_OK) return s;
+  *bytes = ws_layout(*cfg).total;
+  return HARDKV_OK;
+}
+
+hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t bytes, hardkv_ctx **out) {
+  if (!out) return HARDKV_ERR_INVALID_ARG;
+  *out = nullptr;
+  hardkv_status s = check_config(cfg);
+  if (s != HARDKV_OK) return s;
+  const WsLayout w = ws_layout(*cfg);
+  if (!workspace || ((uintptr_t)workspace & 255) || bytes < w.total) return HARDKV_ERR_WORKSPACE;
+  hardkv_ctx *ctx = new (std::nothrow) hardkv_ctx;
+  if (!ctx) return HARDKV_ERR_INVALID_ARG;
+  memset(ctx, 0, sizeof(*ctx));
+  ctx->cfg = *cfg;
+  ctx->variant = 1;
+  ctx->ws_bytes = w.total;
+  Params &P = ctx->base;
+  P.B = cfg->batch; P.Hq = cfg->num_q_heads; P.Hkv = cfg->num_kv_heads; P.G = P.Hq / P.Hkv;
+  P.d = cfg->head_dim; P.max_ctx = cfg->max_ctx; P.sink = cfg->sink; P.recent = cfg->recent;
+  P.k_cap = cfg->k_cap; P.cond_cap = cfg->cond_cap; P.accum_window = cfg->accum_window;
+  P.ppu = cfg->max_ctx / PAGE; P.spu = cfg->k_cap / PAGE;
+  P.att_chunks = att_chunks_of(*cfg);
+  P.sm_scale = cfg->sm_scale > 0.f ? cfg->sm_scale : 1.0f / sqrtf((float)cfg->head_dim);
+  char *base = reinterpret_cast<char *>(workspace);
+  P.att_arrive = reinterpret_cast<int32_t *>(base + w.arrive);
+  P.part = reinterpret_cast<float *>(base + w.part);
+  // opt in to the large dynamic shared memory of the select kernel (host-side attribute, no stream work)
+  if (cudaFuncSetAttribute(select_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SEL_SMEM) != cudaSuccess ||
+      cudaFuncSetAttribute(select_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SEL_SMEM) != cudaSuccess) {
+    cudaGetLastError();
+    delete ctx;
+    return HARDKV_ERR_CUDA;
+  }
+  *out = ctx;
+  return HARDKV_OK;
+}
+
+void hardkv_destroy(hardkv_ctx *ctx) { delete ctx; }
+
+hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant) {
+  if (!ctx || variant < 0 || variant > 1) return HARDKV_ERR_INVALID_ARG;
+  ctx->variant = variant;
+  return HARDKV_OK;
+}
+
+hardkv_status hardkv_append_kv(hardkv_ctx *ctx, const hardkv_state *s, const void *k_new, const void *v_new,
+                               hardkv_stream st) {
+  if (!state_ok(ctx, s) || !k_new || !v_new) return HARDKV_ERR_INVALID_ARG;
+  launch_append(ctx, params_of(ctx, s), k_new, v_new, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_score(hardkv_ctx *ctx, const hardkv_state *s, const void *q, hardkv_stream st) {
+  if (!state_ok(ctx, s) || !q) return HARDKV_ERR_INVALID_ARG;
+  launch_score(ctx, params_of(ctx, s), q, st);
+  return launch_status();
+}
+
+static bool accum_ok(const hardkv_ctx *ctx, const hardkv_state *s) {
+  // ACCUM heads need their state; score_mode lives on the device, so require the buffers
+  // whenever the config declares a window.
+  return ctx->cfg.accum_window <= 0 || (s->acc && s->ring && s->ring_slot);
+}
+
+hardkv_status hardkv_calibrate_topp(hardkv_ctx *ctx, const hardkv_state *s, float p, hardkv_stream st) {
+  if (!state_ok(ctx, s) || !(p > 0.f) || !accum_ok(ctx, s)) return HARDKV_ERR_INVALID_ARG;
+  launch_select(ctx, params_of(ctx, s), p, true, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_topp_select(hardkv_ctx *ctx, const hardkv_state *s, float p, hardkv_stream st) {
+  if (!state_ok(ctx, s) || !(p > 0.f)) return HARDKV_ERR_INVALID_ARG;
+  launch_select(ctx, params_of(ctx, s), p, false, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_rewrite(hardkv_ctx *ctx, const hardkv_state *s, hardkv_stream st) {
+  if (!state_ok(ctx, s)) return HARDKV_ERR_INVALID_ARG;
+  launch_rewrite(ctx, params_of(ctx, s), st);
+  return launch_status();
+}
+
+hardkv_status hardkv_decode_attn(hardkv_ctx *ctx, const hardkv_state *s, const void *q, float *out, float *lse,
+                                 hardkv_stream st) {
+  if (!state_ok(ctx, s) || !q || !out) return HARDKV_ERR_INVALID_ARG;
+  launch_attend(ctx, params_of(ctx, s), q, out, lse, false, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const void *q, const void *k_new,
+                                 const void *v_new, float p, int32_t do_select, float *out, float *lse,
+                                 hardkv_stream st) {
+  if (!state_ok(ctx, s) || !q || !k_new || !v_new || !out || !(p > 0.f) || !accum_ok(ctx, s))
+    return HARDKV_ERR_INVALID_ARG;
+  const Params P = params_of(ctx, s);
+  launch_append(ctx, P, k_new, v_new, st);
+  if (do_select) {
+    launch_score(ctx, P, q, st);
+    launch_select(ctx, P, p, true, st);
+  }
+  launch_attend(ctx, P, q, out, lse, do_select != 0, st);
+  return launch_status();
+}
+
+}  // extern "C"

@@ -1,0 +1,415 @@
+// stage_kernels.cuh -- append/retire, generic score, rewrite and split-K attention kernels.
+// Generic = fp32 FMA arithmetic for every (dtype, head_dim, G); the bf16 tensor-core paths
+// live in fast_kernels.cuh.  Citations are PAPER.md lines.
+#pragma once
+#include "common.cuh"
+
+namespace hardkv {
+
+// =============================================================================================
+// Step 1 + Step 4 of L78: append the new (k, v) row; retire the oldest pool tokens into the
+// constant-size condensed tier (L76), ranked on Cautious-Update votes (L86).
+// One CTA per sequence, one warp per KV head (ctx_len / c_lo are per sequence: they are read by
+// every warp before the barrier and written by thread 0 after it).
+// =============================================================================================
+template <typename T, int D>
+__global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void *k_new, const void *v_new) {
+  constexpr int ROWB = D * sizeof(T);
+  constexpr int LPR = ROWB / 16;  // 16-byte vectors per row
+  const int b = blockIdx.x, lane = threadIdx.x & 31;
+  const int n = P.st.ctx_len[b];
+  const int clo0 = P.st.c_lo[b];
+  const int lup = P.st.l_upper[b];
+  if (n >= P.max_ctx) {  // device-detected inconsistency: flag and leave the sequence untouched
+    if (threadIdx.x == 0) atomicExch(P.st.err_flag, 1);
+    return;
+  }
+  const int n1 = n + 1;
+  int clo = clo0;
+  for (int h = threadIdx.x >> 5; h < P.Hkv; h += blockDim.x >> 5) {
+    const int unit = b * P.Hkv + h;
+    const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
+    // Step 1: "linearly append KV pairs to the Tier 1 Dense Cache" (L78)
+    {
+      char *dk = const_cast<char *>(paged_row<T, D>(P.st.k_pool, tab, n));
+      char *dv = const_cast<char *>(paged_row<T, D>(P.st.v_pool, tab, n));
+      const char *sk = reinterpret_cast<const char *>(k_new) + (size_t)unit * ROWB;
+      const char *sv = reinterpret_cast<const char *>(v_new) + (size_t)unit * ROWB;
+      for (int c = lane; c < LPR; c += 32) {
+        stg(dk + c * 16, ldg_ca(sk + c * 16));
+        stg(dv + c * 16, ldg_ca(sv + c * 16));
+      }
+    }
+    // Step 4: while the pool exceeds l_upper its oldest token t = c_lo retires.
+    int cnt = P.st.cond_count[unit];
+    int32_t *cpos = P.st.cond_pos + (size_t)unit * P.cond_cap;
+    int32_t *cvot = P.st.cond_votes + (size_t)unit * P.cond_cap;
+    const int32_t *votes = P.st.votes + (size_t)unit * P.max_ctx;
+    clo = clo0;
+    while (n1 - P.recent - clo > lup) {
+      const int t = clo;
+      int slot = -1;
+      if (cnt < P.cond_cap) {
+        slot = cnt++;
+      } else if (P.cond_cap > 0) {
+        // resident with the lexicographically smallest (votes, pos)
+        unsigned long long best = ~0ull;
+        int best_slot = 0;
+        for (int j = lane; j < P.cond_cap; j += 32) {
+          unsigned long long key = ((unsigned long long)(uint32_t)cvot[j] << 32) | (uint32_t)cpos[j];
+          if (key < best) { best = key; best_slot = j; }
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+          unsigned long long ob = shfl_xor_u64(best, o);
+          int os = __shfl_xor_sync(0xffffffffu, best_slot, o);
+          if (ob < best) { best = ob; best_slot = os; }
+        }
+        if (votes[t] >= (int32_t)(best >> 32)) slot = best_slot;  // newcomer wins ties (it is newer)
+      }
+      if (slot >= 0) {
+        const char *sk = paged_row<T, D>(P.st.k_pool, tab, t);
+        const char *sv = paged_row<T, D>(P.st.v_pool, tab, t);
+        char *dk = reinterpret_cast<char *>(P.st.cond_k) + ((size_t)unit * P.cond_cap + slot) * ROWB;
+        char *dv = reinterpret_cast<char *>(P.st.cond_v) + ((size_t)unit * P.cond_cap + slot) * ROWB;
+        for (int c = lane; c < LPR; c += 32) {
+          stg(dk + c * 16, ldg_ca(sk + c * 16));
+          stg(dv + c * 16, ldg_ca(sv + c * 16));
+        }
+        if (lane == 0) { cpos[slot] = t; cvot[slot] = votes[t]; }
+      }
+      __syncwarp();
+      ++clo;
+    }
+    if (lane == 0) P.st.cond_count[unit] = cnt;
+  }
+  // every warp computed the same final c_lo (or ran no head: recompute it arithmetically)
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int c = clo0;
+    if (n1 - P.recent - c > lup) c = n1 - P.recent - lup;
+    P.st.ctx_len[b] = n1;
+    P.st.c_lo[b] = c;
+  }
+}
+
+// =============================================================================================
+// score (generic): z[g][i] = sm_scale * q_g . k_i over the pool (exponent of Eq. 4).
+// A warp streams one 16-row page per iteration: each load instruction covers 512 contiguous
+// bytes (32 lanes x 16 B); the LPR lanes that share a row reduce with xor-shuffles.
+// =============================================================================================
+constexpr int SCORE_PAGES_PER_CTA = 32;  // 8 warps x 4 pages = 512 tokens = 128 KiB of K
+
+template <typename T, int D, int G>
+__global__ void __launch_bounds__(256) score_generic_kernel(Params P, const void *q_) {
+  constexpr int EPL = Elem<T>::EPL, LPR = D / EPL, RPW = 32 / LPR, NIT = PAGE / RPW;
+  const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
+  int n, lo, hi;
+  pool_bounds(P, b, n, lo, hi);
+  if (hi <= lo) return;
+  const int first_page = lo >> 4, last_page = (hi - 1) >> 4;
+  const int pg0 = blockIdx.x * SCORE_PAGES_PER_CTA;
+  if (pg0 > last_page || pg0 + SCORE_PAGES_PER_CTA <= first_page) return;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int lr = lane % LPR, rw = lane / LPR;
+
+  float qf[G][EPL];
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    const char *qp = reinterpret_cast<const char *>(q_) + ((size_t)(b * P.Hq + h * G + g) * D) * sizeof(T);
+    Elem<T>::unpack(ldg_ca(qp + lr * 16), qf[g]);
+  }
+  const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
+  float *lg = P.st.logits + ((size_t)(b * P.Hq + h * G)) * P.max_ctx;
+
+  for (int pi = warp; pi < SCORE_PAGES_PER_CTA; pi += 8) {
+    const int pg = pg0 + pi;
+    if (pg < first_page || pg > last_page) continue;
+    const char *src = reinterpret_cast<const char *>(P.st.k_pool) + (size_t)__ldg(tab + pg) * PAGE * D * sizeof(T);
+    uint4 raw[NIT];
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) raw[it] = ldg_nc(src + (it * 32 + lane) * 16);
+#pragma unroll
+    for (int it = 0; it < NIT; ++it) {
+      float kf[EPL];
+      Elem<T>::unpack(raw[it], kf);
+      float acc[G];
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        float a = 0.f;
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) a = fmaf(qf[g][e], kf[e], a);
+        acc[g] = a;
+      }
+#pragma unroll
+      for (int o = LPR / 2; o; o >>= 1)
+#pragma unroll
+        for (int g = 0; g < G; ++g) acc[g] += __shfl_xor_sync(0xffffffffu, acc[g], o);
+      const int pos = pg * PAGE + it * RPW + rw;
+      if (lr == 0 && pos >= lo && pos < hi) {
+#pragma unroll
+        for (int g = 0; g < G; ++g) lg[(size_t)g * P.max_ctx + pos] = acc[g] * P.sm_scale;
+      }
+    }
+  }
+}
+
+// =============================================================================================
+// Rewrite Cache (L172): "read the selected blocks and write them into a regularized, contiguous
+// range".  Slot j of the selected tier <- base row sel_idx[j]; rows k .. 16*ceil(k/16)-1 zero.
+// =============================================================================================
+constexpr int RW_ROWS_PER_CTA = 64;
+
+template <typename T, int D>
+__global__ void __launch_bounds__(256) rewrite_kernel(Params P) {
+  constexpr int ROWB = D * sizeof(T), LPR = ROWB / 16;
+  constexpr int NV = RW_ROWS_PER_CTA * LPR / 256;  // vectors per thread
+  const int unit = blockIdx.y;
+  const int k = P.st.sel_count[unit];
+  const int kend = (k + PAGE - 1) & ~(PAGE - 1);
+  const int j0 = blockIdx.x * RW_ROWS_PER_CTA;
+  if (j0 >= kend) return;
+  const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
+  const int32_t *stab = P.st.sel_pages + (size_t)unit * P.spu;
+  const int32_t *idx = P.st.sel_idx + (size_t)unit * P.k_cap;
+  uint4 kv[NV], vv[NV];
+  size_t dst[NV];
+  bool ok[NV];
+#pragma unroll
+  for (int u = 0; u < NV; ++u) {
+    const int vec = threadIdx.x + u * 256;
+    const int j = j0 + vec / LPR, c = vec % LPR;
+    ok[u] = j < kend;
+    kv[u] = make_uint4(0, 0, 0, 0);
+    vv[u] = make_uint4(0, 0, 0, 0);
+    dst[u] = 0;
+    if (ok[u]) {
+      dst[u] = ((size_t)__ldg(stab + (j >> 4)) * PAGE + (j & 15)) * ROWB + c * 16;
+      if (j < k) {
+        const int pos = __ldg(idx + j);
+        kv[u] = ldg_nc(paged_row<T, D>(P.st.k_pool, tab, pos) + c * 16);
+        vv[u] = ldg_nc(paged_row<T, D>(P.st.v_pool, tab, pos) + c * 16);
+      }
+    }
+  }
+#pragma unroll
+  for (int u = 0; u < NV; ++u)
+    if (ok[u]) {
+      stg(reinterpret_cast<char *>(P.st.sel_k_pool) + dst[u], kv[u]);
+      stg(reinterpret_cast<char *>(P.st.sel_v_pool) + dst[u], vv[u]);
+    }
+}
+
+// =============================================================================================
+// Split-K decode attention over the three tiers (L84; Appendix F Eq. 4-6).
+// Virtual row space of a unit: [dense: sinks, recent | selected tier | condensed residents].
+// A CTA takes ATT_CHUNK consecutive virtual rows, keeps a max-shifted state (m, l, acc) per
+// query head, and writes it as a partial; the last CTA of the unit to arrive merges the
+// partials with the operator of Eq. 6 (SE = l * e^m, o = acc / l).
+// FUSED: selected rows are gathered from the base pool through sel_idx and written through to
+// the selected tier while they are in registers (rewrite + attend read each row once).
+// =============================================================================================
+constexpr int ATT_CHUNK = 128;
+
+template <typename T, int D, int G, bool FUSED>
+__global__ void __launch_bounds__(256) attend_generic_kernel(Params P, const void *q_, float *out, float *lse) {
+  constexpr int EPL = Elem<T>::EPL, LPR = D / EPL, ROWB = D * sizeof(T);
+  constexpr int NGRP = 256 / LPR;  // row groups per CTA
+  constexpr int UNR = 4;
+  const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
+  const int n = P.st.ctx_len[b];
+  const int s_end = min(P.sink, n);
+  const int r_lo = max(n - P.recent, s_end);
+  const int n_dense = s_end + (n - r_lo);
+  const int k = P.st.sel_count[unit];
+  const int cc = P.st.cond_count[unit];
+  const int total = n_dense + k + cc;
+  const int nchunks = (total + ATT_CHUNK - 1) / ATT_CHUNK;
+  const int c = blockIdx.x;
+  if (c >= nchunks) return;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int lr = lane % LPR, grp = tid / LPR;
+
+  const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
+  const int32_t *stab = P.st.sel_pages + (size_t)unit * P.spu;
+  const int32_t *idx = P.st.sel_idx + (size_t)unit * P.k_cap;
+
+  float qf[G][EPL];
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    const char *qp = reinterpret_cast<const char *>(q_) + ((size_t)(b * P.Hq + h * G + g) * D) * sizeof(T);
+    Elem<T>::unpack(ldg_ca(qp + lr * 16), qf[g]);
+  }
+  float m[G], l[G], acc[G][EPL];
+#pragma unroll
+  for (int g = 0; g < G; ++g) {
+    m[g] = -INFINITY; l[g] = 0.f;
+#pragma unroll
+    for (int e = 0; e < EPL; ++e) acc[g][e] = 0.f;
+  }
+
+  const int v0 = c * ATT_CHUNK, v1 = min(total, v0 + ATT_CHUNK);
+  for (int vb = v0 + grp; vb < v1; vb += NGRP * UNR) {
+    uint4 kr[UNR], vr[UNR];
+    bool ok[UNR];
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) {
+      const int v = vb + u * NGRP;
+      ok[u] = v < v1;
+      kr[u] = make_uint4(0, 0, 0, 0);
+      vr[u] = make_uint4(0, 0, 0, 0);
+      if (!ok[u]) continue;
+      const char *kp, *vp;
+      if (v < n_dense) {  // Tier 1: sinks + recent window, read in place
+        const int pos = v < s_end ? v : r_lo + (v - s_end);
+        kp = paged_row<T, D>(P.st.k_pool, tab, pos);
+        vp = paged_row<T, D>(P.st.v_pool, tab, pos);
+      } else if (v < n_dense + k) {  // Tier 2: selected rows
+        const int j = v - n_dense;
+        const size_t so = ((size_t)__ldg(stab + (j >> 4)) * PAGE + (j & 15)) * ROWB;
+        if (FUSED) {
+          const int pos = __ldg(idx + j);
+          kp = paged_row<T, D>(P.st.k_pool, tab, pos);
+          vp = paged_row<T, D>(P.st.v_pool, tab, pos);
+        } else {
+          kp = reinterpret_cast<const char *>(P.st.sel_k_pool) + so;
+          vp = reinterpret_cast<const char *>(P.st.sel_v_pool) + so;
+        }
+        kr[u] = ldg_nc(kp + lr * 16);
+        vr[u] = ldg_nc(vp + lr * 16);
+        if (FUSED) {
+          stg(reinterpret_cast<char *>(P.st.sel_k_pool) + so + lr * 16, kr[u]);
+          stg(reinterpret_cast<char *>(P.st.sel_v_pool) + so + lr * 16, vr[u]);
+        }
+        continue;
+      } else {  // Tier 3: condensed residents
+        const size_t co = ((size_t)unit * P.cond_cap + (v - n_dense - k)) * ROWB;
+        kp = reinterpret_cast<const char *>(P.st.cond_k) + co;
+        vp = reinterpret_cast<const char *>(P.st.cond_v) + co;
+      }
+      kr[u] = ldg_nc(kp + lr * 16);
+      vr[u] = ldg_nc(vp + lr * 16);
+    }
+#pragma unroll
+    for (int u = 0; u < UNR; ++u) {
+      if (!ok[u]) continue;  // uniform within a row group; groups of one warp may differ -> masks below
+      float kf[EPL], vf[EPL];
+      Elem<T>::unpack(kr[u], kf);
+      Elem<T>::unpack(vr[u], vf);
+      float s[G];
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        float a = 0.f;
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) a = fmaf(qf[g][e], kf[e], a);
+        s[g] = a;
+      }
+      // reduce over the LPR lanes of this row group (lanes of other groups may be inactive)
+      const unsigned gmask = LPR == 32 ? 0xffffffffu : (((1u << LPR) - 1u) << ((lane / LPR) * LPR));
+#pragma unroll
+      for (int o = LPR / 2; o; o >>= 1)
+#pragma unroll
+        for (int g = 0; g < G; ++g) s[g] += __shfl_xor_sync(gmask, s[g], o);
+#pragma unroll
+      for (int g = 0; g < G; ++g) {
+        const float x = s[g] * P.sm_scale;
+        const float mn = fmaxf(m[g], x);
+        const float corr = __expf(m[g] - mn);
+        const float pw = __expf(x - mn);
+        l[g] = l[g] * corr + pw;
+#pragma unroll
+        for (int e = 0; e < EPL; ++e) acc[g][e] = fmaf(acc[g][e], corr, pw * vf[e]);
+        m[g] = mn;
+      }
+    }
+  }
+
+  if (FUSED && k > 0 && (n_dense + k - 1) >= v0 && (n_dense + k - 1) < v1) {
+    // zero tail of the last valid page of the selected tier (DESIGN reading C9)
+    const int kend = (k + PAGE - 1) & ~(PAGE - 1);
+    for (int vec = tid; vec < (kend - k) * LPR; vec += 256) {
+      const int j = k + vec / LPR, cch = vec % LPR;
+      const size_t so = ((size_t)__ldg(stab + (j >> 4)) * PAGE + (j & 15)) * ROWB + cch * 16;
+      stg(reinterpret_cast<char *>(P.st.sel_k_pool) + so, make_uint4(0, 0, 0, 0));
+      stg(reinterpret_cast<char *>(P.st.sel_v_pool) + so, make_uint4(0, 0, 0, 0));
+    }
+  }
+
+  // ---- combine the row groups of a warp (Eq. 6 in max-shifted form) ------------------------
+#pragma unroll
+  for (int o = LPR; o < 32; o <<= 1) {
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+      const float om = __shfl_xor_sync(0xffffffffu, m[g], o);
+      const float ol = __shfl_xor_sync(0xffffffffu, l[g], o);
+      const float mn = fmaxf(m[g], om);
+      const float ca = (m[g] == -INFINITY) ? 0.f : __expf(m[g] - mn);
+      const float cb = (om == -INFINITY) ? 0.f : __expf(om - mn);
+      l[g] = l[g] * ca + ol * cb;
+#pragma unroll
+      for (int e = 0; e < EPL; ++e) {
+        const float oa = __shfl_xor_sync(0xffffffffu, acc[g][e], o);
+        acc[g][e] = acc[g][e] * ca + oa * cb;
+      }
+      m[g] = mn;
+    }
+  }
+  // ---- combine the 8 warps through shared memory ---------------------------------------------
+  __shared__ float s_st[8][G][D + 2];
+  __shared__ int s_last;
+  if (lane < LPR) {
+#pragma unroll
+    for (int g = 0; g < G; ++g) {
+#pragma unroll
+      for (int e = 0; e < EPL; ++e) s_st[warp][g][2 + lr * EPL + e] = acc[g][e];
+      if (lr == 0) { s_st[warp][g][0] = m[g]; s_st[warp][g][1] = l[g]; }
+    }
+  }
+  __syncthreads();
+  float *part = P.part + ((size_t)unit * P.att_chunks + c) * G * (D + 2);
+  for (int it = tid; it < G * D; it += 256) {
+    const int g = it / D, e = it % D;
+    float M = -INFINITY;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) M = fmaxf(M, s_st[w][g][0]);
+    float L = 0.f, A = 0.f;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+      const float mw = s_st[w][g][0];
+      const float cw = (mw == -INFINITY) ? 0.f : __expf(mw - M);
+      L += s_st[w][g][1] * cw;
+      A += s_st[w][g][2 + e] * cw;
+    }
+    part[g * (D + 2) + 2 + e] = A;
+    if (e == 0) { part[g * (D + 2)] = M; part[g * (D + 2) + 1] = L; }
+  }
+  // ---- last CTA of the unit merges all partials ------------------------------------------------
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) {
+    const int ticket = atomicAdd(P.att_arrive + unit, 1);
+    s_last = (ticket == nchunks - 1);
+  }
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  const float *pu = P.part + (size_t)unit * P.att_chunks * G * (D + 2);
+  for (int it = tid; it < G * D; it += 256) {
+    const int g = it / D, e = it % D;
+    float M = -INFINITY;
+    for (int ch = 0; ch < nchunks; ++ch) M = fmaxf(M, __ldcg(pu + ((size_t)ch * G + g) * (D + 2)));
+    float L = 0.f, A = 0.f;
+    for (int ch = 0; ch < nchunks; ++ch) {
+      const float *pp = pu + ((size_t)ch * G + g) * (D + 2);
+      const float mw = __ldcg(pp);
+      const float cw = (mw == -INFINITY) ? 0.f : __expf(mw - M);
+      L += __ldcg(pp + 1) * cw;
+      A += __ldcg(pp + 2 + e) * cw;
+    }
+    out[((size_t)(b * P.Hq + h * G + g)) * D + e] = A / L;
+    if (e == 0 && lse) lse[b * P.Hq + h * G + g] = M + logf(L);
+  }
+  if (tid == 0) P.att_arrive[unit] = 0;  // restore for the next launch / graph replay
+}
+
+}  // namespace hardkv

@@ -1,0 +1,223 @@
+"""-m gpu parity tests: the CUDA path (called through the C ABI) against the CPU oracle, element by
+element on the same seeded inputs.  Sizes span several tiles and ragged tails of every kernel
+(score: 512-token CTA tiles; select: 512 threads / 16 warp segments; rewrite: 64 rows; attention:
+128-row chunks) and the degenerate cases (empty pool, single token, ties, k_cap clamp, p = 1).
+
+Bars (BASELINE.json north_star): selection, counts, tables, votes, rewritten rows, condensed-tier
+bookkeeping bit-exact given identical probabilities; end to end only tokens within 1e-6 of the
+threshold may differ; outputs max-abs <= 2e-2, mean-abs <= 2e-3.
+"""
+import numpy as np
+import pytest
+import torch
+
+from paper_2606_28831_b200.synth import make_workload
+
+pytestmark = pytest.mark.gpu
+
+i32 = lambda *v: np.array(v, np.int32)
+
+
+def small_workloads():
+    """Shrunk versions of BASELINE.json's five configs (same dtype, G, d, structure, parameters)."""
+    return {
+        "c0": make_workload(0),
+        "c1s": make_workload(1, n0=i32(2100), max_ctx=2176, k_cap=512, l_upper=i32(1960), cond_cap=32, steps=6),
+        "c2s": make_workload(2, B=3, n0=i32(900, 2300, 1500), max_ctx=2400, k_cap=256,
+                             l_upper=i32(900 - 132, 2300 - 132, 1500 - 132), cond_cap=24, steps=6),
+        "c3s": make_workload(3, B=2, n0=i32(300, 300), max_ctx=512, k_cap=64, l_upper=i32(48, 48), cond_cap=8,
+                             steps=40),
+        "c4s": make_workload(4, B=2, n0=i32(1500, 1500), max_ctx=1600, k_cap=384, l_upper=i32(1390, 1390),
+                             cond_cap=16, accum_window=4, steps=8),
+        "g1d64": make_workload(1, Hq=2, Hkv=2, d=64, n0=i32(700), max_ctx=720, k_cap=128, l_upper=i32(560),
+                               cond_cap=4, steps=4),
+        "g2": make_workload(1, Hq=4, Hkv=2, n0=i32(640), max_ctx=656, k_cap=160, l_upper=i32(500), cond_cap=4,
+                            steps=4),
+        "g8": make_workload(1, Hq=8, Hkv=1, n0=i32(1100), max_ctx=1120, k_cap=1120, l_upper=i32(5000), cond_cap=0,
+                            steps=3),
+    }
+
+
+WL = small_workloads()
+
+
+@pytest.fixture(scope="module")
+def P():
+    from gpu_common import Pair
+    return Pair
+
+
+@pytest.mark.parametrize("name", list(WL))
+def test_stages_teacher_forced(name, P):
+    """Each ABI stage against the matching oracle stage, every step; selection fed identical probabilities."""
+    wl = WL[name]
+    pr = P(wl)
+    eng, st, ob = pr.eng, pr.st, pr.ob
+    for t in range(min(wl.steps, 6)):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        G, d = wl.G, wl.d
+        # step 0: append + retire
+        eng.append_kv(st, knd, vnd)
+        for i, u in enumerate(ob.units):
+            u.append(kn.reshape(-1, d)[i], vn.reshape(-1, d)[i])
+            u.retire()
+        pr.check_bookkeeping()
+        # step 1: score
+        eng.score(st, qd)
+        qu = q.reshape(-1, G, d)
+        for i, u in enumerate(ob.units):
+            u.score(qu[i])
+        pr.check_logits()
+        # step 2a-2c end to end from the CUDA logits (votes restored afterwards)
+        votes0 = st.votes.clone()
+        eng.calibrate_topp(st, wl.p)
+        for u in ob.units:
+            u.calibrate()
+            u.topp_select(wl.p, True)
+        pr.check_probs()
+        pr.check_selection_band()
+        # step 2b-2c bit exact from identical probabilities
+        st.votes.copy_(votes0)
+        pr.upload_oracle_probs()
+        eng.topp_select(st, wl.p)
+        pr.check_selection_exact()
+        # step 3: rewrite
+        eng.rewrite(st)
+        for u in ob.units:
+            u.rewrite()
+        pr.check_rewrite_exact()
+        # step 4: attention over the three tiers
+        eng.decode_attn(st, qd, pr.out, pr.lse)
+        for i, u in enumerate(ob.units):
+            u.attend(qu[i])
+        pr.check_out(f"{name} step {t}")
+
+
+@pytest.mark.parametrize("name", list(WL))
+@pytest.mark.parametrize("teacher", [True, False])
+def test_fused_decode_step(name, teacher, P):
+    """hardkv_decode_step (one call per step) over a trajectory, teacher-forced and free-running."""
+    wl = WL[name]
+    pr = P(wl, want_mask=False)
+    flips = 0
+    for t in range(min(wl.steps, 12)):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)
+        pr.ob.step(q, kn, vn, wl.p)
+        pr.check_out(f"{name} step {t}")
+        if teacher or flips == 0:
+            f = pr.check_selection_band()
+            flips += f
+            if f == 0:
+                pr.check_bookkeeping()
+                pr.check_rewrite_exact()
+                pr.check_votes()
+        if teacher:
+            pr.force_discrete_state()
+
+
+def test_select_interval_reuses_selected_tier(P):
+    """do_select = 0 between compressions (L274): append + attend over the previous selected tier."""
+    wl = WL["c1s"]
+    pr = P(wl, want_mask=False)
+    for t in range(6):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        sel = (t % 3 == 0)
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse, do_select=sel)
+        pr.ob.step(q, kn, vn, wl.p, do_select=sel)
+        pr.check_out(f"step {t}")
+        assert pr.check_selection_band() == 0
+        pr.check_bookkeeping()
+
+
+@pytest.mark.parametrize("case", ["ties", "one_dominant", "p1", "l_lower", "clamp", "zeros", "n1"])
+def test_select_degenerate(case, P):
+    """Top-p edge cases on hand-made probability rows, bit exact."""
+    wl = make_workload(1, Hq=4, Hkv=1, n0=i32(1200), max_ctx=1216, k_cap=1216 if case != "clamp" else 64,
+                       l_upper=i32(5000), cond_cap=0, l_lower=i32(2000 if case == "l_lower" else 0))
+    if case == "n1":
+        wl = make_workload(1, Hq=4, Hkv=1, n0=i32(4 + 128 + 1), max_ctx=160, k_cap=16, l_upper=i32(5000), cond_cap=0)
+    pr = P(wl)
+    u = pr.ob.units[0]
+    lo, hi = u.pool
+    N = hi - lo
+    rng = np.random.default_rng(5)
+    p = 0.9
+    if case == "ties":
+        row = np.full(N, 1.0 / N, np.float32)
+    elif case == "one_dominant":
+        row = np.full(N, 1e-12, np.float32); row[N // 3] = 1.0
+    elif case == "p1":
+        row = rng.random(N).astype(np.float32); row /= row.sum(); p = 1.0
+    elif case == "zeros":
+        row = np.zeros(N, np.float32); row[5:40] = 1.0 / 35
+    elif case == "n1":
+        row = np.ones(N, np.float32)
+    else:
+        row = rng.random(N).astype(np.float32) ** 4; row /= row.sum()
+        row[100:140] = row[100]   # a run of exact ties inside the row
+    u.probs[lo:hi] = row
+    u.topp_select(p, True)
+    pr.upload_oracle_probs()
+    pr.eng.topp_select(pr.st, p)
+    pr.check_selection_exact()
+    assert u.sel_count > 0
+
+
+def test_empty_pool_and_growth(P):
+    """Context shorter than sink + recent: empty pool, dense tier only; then the pool opens."""
+    wl = make_workload(1, Hq=8, Hkv=2, n0=i32(3), max_ctx=256, k_cap=64, l_upper=i32(30), cond_cap=4, recent=16)
+    pr = P(wl, want_mask=False)
+    for t in range(70):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)
+        pr.ob.step(q, kn, vn, wl.p)
+        pr.check_out(f"step {t}")
+        assert pr.check_selection_band() == 0
+        pr.check_bookkeeping()
+        pr.check_votes()
+
+
+def test_cuda_graph_replay(P):
+    """The fused step captured once and replayed: shapes static, counts on the device (L53, L63)."""
+    wl = WL["c2s"]
+    pr = P(wl, want_mask=False)
+    q, kn, vn, (qd, knd, vnd) = pr.inputs(0)
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)   # warm-up outside capture (step 0)
+    torch.cuda.current_stream().wait_stream(s)
+    pr.ob.step(q, kn, vn, wl.p)
+    pr.check_out("warm-up step")
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)
+    # capture does not execute: the first replay is step 1
+    for t in range(1, 5):
+        q, kn, vn, (q2, k2, v2) = pr.inputs(t)
+        qd.copy_(q2); knd.copy_(k2); vnd.copy_(v2)
+        g.replay()
+        pr.ob.step(q, kn, vn, wl.p)
+        pr.check_out(f"replay {t}")
+        assert pr.check_selection_band() == 0
+        pr.check_bookkeeping()
+
+
+def test_error_paths(P):
+    """Host-detectable errors come back as status codes; a full context sets err_flag on the device."""
+    from paper_2606_28831_b200 import hardkv
+    with pytest.raises(hardkv.HardKVError):
+        hardkv.HardKV(batch=1, num_q_heads=6, num_kv_heads=2, head_dim=128, max_ctx=64, sink=4, recent=8, k_cap=16,
+                      cond_cap=0, kv_dtype=hardkv.BF16)          # G = 3 is not built
+    with pytest.raises(hardkv.HardKVError):
+        hardkv.HardKV(batch=1, num_q_heads=4, num_kv_heads=1, head_dim=128, max_ctx=70, sink=4, recent=8, k_cap=16,
+                      cond_cap=0, kv_dtype=hardkv.BF16)          # max_ctx not a multiple of the page
+    wl = make_workload(1, Hq=4, Hkv=1, n0=i32(64), max_ctx=64, k_cap=16, l_upper=i32(100), cond_cap=0, recent=16)
+    pr = P(wl, want_mask=False)
+    q, kn, vn, (qd, knd, vnd) = pr.inputs(0)
+    pr.eng.append_kv(pr.st, knd, vnd)                             # ctx_len == max_ctx: no room
+    torch.cuda.synchronize()
+    assert int(pr.st.err_flag.item()) == 1 and int(pr.st.ctx_len.item()) == 64
+    with pytest.raises(hardkv.HardKVError):
+        pr.eng.score(pr.st, None)
