@@ -34,7 +34,7 @@ class Pair:
     def inputs(self, t: int):
         wl = self.wl
         q = wl.step_q(t)
-        k_new, v_new = wl.step_kv(t, self.prefill if wl.mix_new_keys else None)
+        k_new, v_new = wl.step_kv(t, {u: kv[0] for u, kv in self.prefill.items()} if wl.mix_new_keys else None)
         return q, k_new, v_new, (harness.to_dev(q, wl, DEV), harness.to_dev(k_new, wl, DEV),
                                  harness.to_dev(v_new, wl, DEV))
 
