@@ -1,0 +1,350 @@
+#!/usr/bin/env python
+"""bench.py -- HARD-KV decode-step hot path on B200 (BASELINE.json metric).
+
+One "step" = one fused pass of the whole hot path (append + retire, score, calibrate + Top-p,
+rewrite + tiered attention: SURVEY.md section 8(a)) over one batch of synthetic input, one layer.
+Workload at N=1: BASELINE.json configs[2] (batch 16, contexts 4096..32768, the config the >= 70 %
+target is quoted on).  K pool of one layer ~ 580 MB >> 126 MB L2, so no L2 flush is needed.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config I]
+
+N > 1 (torchrun): every rank runs its own batch of the same shape (units shard with no data-path
+collective; weak scaling); value = bytes of all ranks / max-over-ranks time.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "decode_step_kv_bandwidth"      # B_min / time of the fused select+rewrite+attend layer-step
+UNIT = "GB/s"
+NOMINAL_HBM_GBS = 8000.0                 # the contract's "8 TB/s"
+FALLBACK_HBM_GBS = 6650.0                # B200_PROFILING.md fallback
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks sampling (nvidia-smi in the background during the timed region)
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, uuid: str | None):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        cmd = ["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "50"]
+        if uuid:
+            cmd += ["-i", uuid]
+        try:
+            self.p = subprocess.Popen(cmd, stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self) -> dict:
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.12)
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush()
+        rows = [r.strip().split(",") for r in open(self.f.name).read().strip().splitlines() if r.strip()]
+        os.unlink(self.f.name)
+        sm, smax, reasons, pw = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in rows:
+            try:
+                sm.append(float(r[0])); smax.append(float(r[1])); pw.append(float(r[2]))
+                for nme, v in zip(names, r[3:7]):
+                    if v.strip().lower().startswith("active"):
+                        reasons.add(nme)
+            except Exception:
+                continue
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "reasons": sorted(reasons),
+                "samples": len(sm), "power_w_max": float(max(pw))}
+
+
+# ------------------------------------------------------------------------------------------------
+# the CPU oracle leg (cpu_baseline at N=1, and --impl reference)
+# ------------------------------------------------------------------------------------------------
+def oracle_leg(cfg_index: int, steps: int, warmup: int, budget_s: float, sample_B: int):
+    """Time oracle/ (as it stands) on the first `sample_B` sequences of the workload: all of their
+    KV heads, whole decode steps.  Returns (GB/s of B_min, us/step, cores, sample text, steps timed)."""
+    from oracle import oracle as ora
+    from oracle.batch import OracleBatch
+    from paper_2606_28831_b200 import accounting
+    from paper_2606_28831_b200.synth import make_workload
+    ora.build()
+    wl = make_workload(cfg_index, B=sample_B) if cfg_index in (2, 3, 4) else make_workload(cfg_index)
+    prefill = {(b, h): wl.prefill_unit(b, h) for b in range(wl.B) for h in range(wl.Hkv)}
+    ob = OracleBatch(wl, prefill)
+    pk = {u: kv[0] for u, kv in prefill.items()} if wl.mix_new_keys else None
+    t_acc, bytes_acc, done = 0.0, 0, 0
+    for t in range(warmup + steps):
+        q = wl.step_q(t)
+        kn, vn = wl.step_kv(t, pk)
+        t0 = time.perf_counter()
+        ob.step(q, kn, vn, wl.p)
+        dt = time.perf_counter() - t0
+        if t >= warmup:
+            t_acc += dt
+            done += 1
+            bytes_acc += accounting.algorithmic_bytes(wl, ob.ctx_len(), ob.c_lo(), ob.sel_count(),
+                                                        ob.cond_count())["total"]
+            if t_acc > budget_s:
+                break
+    gbs = bytes_acc / t_acc / 1e9
+    sample = (f"{wl.name}: first {wl.B} of the sequences (n0={wl.n0.tolist()}), all {wl.Hkv} KV heads, "
+              f"{done} whole decode steps after {warmup} warm-up, OpenMP over (b,h)")
+    return gbs, t_acc / done * 1e6, int(ob.threads), sample, done, wl
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    gbs, us, cores, sample, done, wl = oracle_leg(args.config, args.steps, args.warmup, budget_s=150.0,
+                                                  sample_B=args.ref_batch)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": args.gpus, "steps": done,
+        "warmup": args.warmup, "ms_per_step": us / 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}] ({wl.name})", "sample": sample},
+        "cpu_baseline": {"value": gbs, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gbs, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "us_per_layer_step": us, "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ------------------------------------------------------------------------------------------------
+def run_cuda(args):
+    import torch
+    import torch.distributed as dist
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback; use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = f"cuda:{local}"
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device(dev))
+
+    import __graft_entry__
+    __graft_entry__.build_cuda()
+    from paper_2606_28831_b200 import accounting, harness
+    from paper_2606_28831_b200.synth import make_workload
+
+    K, W = args.steps, args.warmup
+    wl = make_workload(args.config)
+    wl.seed += 1000 * rank                       # every rank: its own batch of the same shape
+    if K + W > wl.max_ctx - int(wl.n0.max()):
+        raise SystemExit(f"steps + warmup must be <= {wl.max_ctx - int(wl.n0.max())} for {wl.name}")
+    t0 = time.time()
+    eng = harness.make_engine(wl, dev)
+    (st,), prefill = harness.make_state(wl, dev)
+    pk = {u: kv[0] for u, kv in prefill.items()} if wl.mix_new_keys else None
+    tdt = harness.torch_dtype(wl)
+    qs, ks, vs = [], [], []
+    for t in range(W + K):
+        qs.append(wl.step_q(t))
+        kn, vn = wl.step_kv(t, pk)
+        ks.append(kn); vs.append(vn)
+    q_h = torch.from_numpy(np.stack(qs)).to(tdt).pin_memory()      # [W+K][B][Hq][d] pinned host
+    k_h = torch.from_numpy(np.stack(ks)).to(tdt).pin_memory()
+    v_h = torch.from_numpy(np.stack(vs)).to(tdt).pin_memory()
+    q_d, k_d, v_d = q_h.to(dev), k_h.to(dev), v_h.to(dev)          # resident in HBM before the timed region
+    out = torch.zeros(wl.B, wl.Hq, wl.d, dtype=torch.float32, device=dev)
+    out_h = torch.zeros(wl.B, wl.Hq, wl.d, dtype=torch.float32).pin_memory()
+    if rank == 0:
+        log(f"[bench] {wl.name}: setup {time.time() - t0:.1f}s, units={wl.B * wl.Hkv}, "
+            f"n0 mean={wl.n0.mean():.0f}, steps={K}, warmup={W}")
+    snap0 = harness.snapshot(st)
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def warm():
+        harness.restore(st, snap0)
+        for t in range(W):
+            eng.decode_step(st, q_d[t], k_d[t], v_d[t], wl.p, out)
+
+    # ---- (1) device-resident timed region: K fused steps --------------------------------------
+    warm()
+    uuid = str(torch.cuda.get_device_properties(local).uuid)
+    uuid = uuid if uuid.startswith("GPU-") else "GPU-" + uuid
+    barrier()
+    sampler = ClockSampler(uuid)
+    time.sleep(0.15)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n_before = eng.launch_count()
+    barrier()
+    e0.record(stream)
+    for t in range(W, W + K):
+        eng.decode_step(st, q_d[t], k_d[t], v_d[t], wl.p, out)
+    e1.record(stream)
+    barrier()
+    launches = eng.launch_count() - n_before
+    ms_total = e0.elapsed_time(e1)
+    clocks = sampler.stop()
+    assert int(st.err_flag.item()) == 0, "device err_flag set"
+    assert bool(torch.isfinite(out).all()), "non-finite attention output"
+
+    # ---- (2) same steps, stage by stage with events (kernel shares + per-step byte counts) ------
+    warm()
+    STAGES = ["append_retire", "score", "calibrate_topp", "rewrite_attend"]
+    ev = [[torch.cuda.Event(enable_timing=True) for _ in range(len(STAGES) + 1)] for _ in range(K)]
+    cnt_sel = torch.zeros(K, wl.B * wl.Hkv, dtype=torch.int32, device=dev)
+    cnt_cond = torch.zeros(K, wl.B * wl.Hkv, dtype=torch.int32, device=dev)
+    cnt_n = torch.zeros(K, wl.B, dtype=torch.int32, device=dev)
+    cnt_lo = torch.zeros(K, wl.B, dtype=torch.int32, device=dev)
+    torch.cuda.synchronize()
+    for i, t in enumerate(range(W, W + K)):
+        ev[i][0].record(stream)
+        eng.append_kv(st, k_d[t], v_d[t]); ev[i][1].record(stream)
+        eng.score(st, q_d[t]); ev[i][2].record(stream)
+        eng.calibrate_topp(st, wl.p); ev[i][3].record(stream)
+        eng.rewrite_attend(st, q_d[t], out); ev[i][4].record(stream)
+        cnt_sel[i].copy_(st.sel_count); cnt_cond[i].copy_(st.cond_count)
+        cnt_n[i].copy_(st.ctx_len); cnt_lo[i].copy_(st.c_lo)
+    torch.cuda.synchronize()
+    stage_us = {s: float(np.mean([ev[i][j].elapsed_time(ev[i][j + 1]) for i in range(K)]) * 1e3)
+                for j, s in enumerate(STAGES)}
+    csel, ccond, cn, clo = (x.cpu().numpy() for x in (cnt_sel, cnt_cond, cnt_n, cnt_lo))
+    per_step = [accounting.algorithmic_bytes(wl, cn[i], clo[i], csel[i], ccond[i]) for i in range(K)]
+    bytes_total = sum(p["total"] for p in per_step)
+    bytes_stage = {"score": float(np.mean([p["score"] for p in per_step])),
+                   "rewrite_attend": float(np.mean([p["attend"] + p["rewrite_write"] for p in per_step]))}
+
+    # ---- (3) end to end through the host-buffer entry point -------------------------------------
+    warm()
+    torch.cuda.synchronize()
+    barrier()
+    t_e2e0 = time.perf_counter()
+    for t in range(W, W + K):
+        eng.decode_step_host(st, q_h[t], k_h[t], v_h[t], wl.p, out_h)
+        stream.synchronize()                      # the caller reads out_h before the next token
+    t_e2e = time.perf_counter() - t_e2e0
+    h2d = (q_h[0].numel() + k_h[0].numel() + v_h[0].numel()) * q_h.element_size()
+    d2h = out_h.numel() * 4
+
+    # ---- reduce over ranks ------------------------------------------------------------------------
+    red = torch.tensor([ms_total, t_e2e * 1e3], dtype=torch.float64, device=dev)
+    tot = torch.tensor([float(bytes_total)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(red, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    ms_total, ms_e2e = float(red[0]), float(red[1])
+    bytes_all = float(tot[0])
+
+    if rank == 0:
+        peak, peak_src = measured_peak()
+        gbs = bytes_all / (ms_total * 1e-3) / 1e9
+        e2e_gbs = bytes_all / (ms_e2e * 1e-3) / 1e9
+        us_step = ms_total / K * 1e3
+        dom = max(("score", "rewrite_attend", "calibrate_topp"), key=lambda s: stage_us[s])
+        roof = {"kernel": dom, "bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src, "traffic": None}
+        if dom in bytes_stage:
+            roof["achieved"] = bytes_stage[dom] / (stage_us[dom] * 1e-6) / 1e9
+            roof["algorithmic_bytes_per_launch"] = bytes_stage[dom]
+        else:  # the select kernel moves no algorithmic KV bytes: report its logits+probs traffic
+            lb = float(np.mean([p["select_bytes"] for p in per_step]))
+            roof["achieved"] = lb / (stage_us[dom] * 1e-6) / 1e9
+            roof["algorithmic_bytes_per_launch"] = lb
+        roof["frac"] = roof["achieved"] / peak
+        roof["avg_launch_us"] = stage_us[dom]
+        line = {
+            "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
+            "config": {"workload": f"BASELINE.json configs[{args.config}] ({wl.name})", "batch": wl.B,
+                       "q_heads": wl.Hq, "kv_heads": wl.Hkv, "head_dim": wl.d, "ctx": [int(wl.n0.min()), int(wl.n0.max())],
+                       "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": 1,
+                       "l2": "inputs larger than L2 (K pool %.0f MB per layer-step), no flush" % (
+                           per_step[0]["score"] / 1e6),
+                       "parallelism": f"units sharded, {world} rank(s), no collective"},
+            "us_per_layer_step": us_step,
+            "tokens_per_s_layer": wl.B * world / (us_step * 1e-6),
+            "frac_of_8TBs": gbs / world / NOMINAL_HBM_GBS,
+            "frac_of_measured_copy": gbs / world / peak,
+            "algorithmic_bytes_per_step": bytes_all / K / world,
+            "mean_k": float(np.mean([p["mean_k"] for p in per_step])), "max_k": int(max(p["max_k"] for p in per_step)),
+            "sparsity_utilisation": float(np.mean([p["mean_k"] / max(p["max_k"], 1) for p in per_step])),
+            "stages_us": stage_us, "stages_sum_us": float(sum(stage_us.values())),
+            "roofline": roof,
+            "e2e": {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "us_per_layer_step": ms_e2e / K * 1e3, "sync": "stream sync after every step"},
+            "gpu_launches": int(launches),
+            "clocks": clocks,
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            del st, eng
+            torch.cuda.empty_cache()
+            g, us, cores, sample, done, _ = oracle_leg(args.config, steps=4, warmup=1, budget_s=20.0,
+                                                       sample_B=args.ref_batch)
+            line["cpu_baseline"] = {"value": g, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                                    "us_per_layer_step_of_sample": us}
+        else:
+            line["cpu_baseline"] = None
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=64)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: the target config)")
+    ap.add_argument("--ref-batch", type=int, default=4, help="sequences in the oracle's bounded sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -113,12 +113,29 @@ hardkv_status hardkv_rewrite(hardkv_ctx *, const hardkv_state *, hardkv_stream);
 /* Split-K decode attention over dense + selected + condensed tiers merged by Eq. 6 (L748-762). */
 hardkv_status hardkv_decode_attn(hardkv_ctx *, const hardkv_state *, const void *q, float *out,
                                  float *lse /* nullable */, hardkv_stream);
+/* Steps 3 + 4 fused: the selected rows are gathered from the base pool through sel_idx, written
+ * through to the selected tier (L172) and attended while they are in flight, so each selected
+ * row is read once; same results as hardkv_rewrite followed by hardkv_decode_attn. */
+hardkv_status hardkv_rewrite_attend(hardkv_ctx *, const hardkv_state *, const void *q, float *out,
+                                    float *lse /* nullable */, hardkv_stream);
 /* The whole step on one stream: append, retire, score, calibrate + Top-p, rewrite fused
  * with attention (selected rows are read once).  do_select = 0 skips score/select/rewrite
  * and attends over the previous selected tier (the steps between two compressions, L274). */
 hardkv_status hardkv_decode_step(hardkv_ctx *, const hardkv_state *, const void *q, const void *k_new,
                                  const void *v_new, float p, int32_t do_select, float *out,
                                  float *lse /* nullable */, hardkv_stream);
+
+/* hardkv_decode_step with HOST buffers for the per-step tensors (end-to-end entry): q_host
+ * [B][Hq][d], k_new_host / v_new_host [B][Hkv][d] in kv_dtype and out_host [B][Hq][d] f32 are
+ * HOST pointers (pinned memory for truly asynchronous copies; pageable works, slower).  The
+ * call enqueues H2D copies into staging buffers inside the workspace, the step, and the D2H
+ * copy of `out`, all on `stream`; it does not synchronise -- out_host is valid after the caller
+ * synchronises the stream.  The host input buffers must stay untouched until then. */
+hardkv_status hardkv_decode_step_host(hardkv_ctx *, const hardkv_state *, const void *q_host,
+                                      const void *k_new_host, const void *v_new_host, float p,
+                                      int32_t do_select, float *out_host, hardkv_stream);
+/* Number of kernels this ctx has launched since hardkv_create (host counter; memcpys excluded). */
+int64_t hardkv_launch_count(const hardkv_ctx *ctx);
 
 #ifdef __cplusplus
 }

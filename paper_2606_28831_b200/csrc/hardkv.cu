@@ -15,13 +15,18 @@ struct hardkv_ctx {
   Params base;      // config-derived fields + workspace pointers; `st` is filled per call
   int variant;
   size_t ws_bytes;
+  int64_t launches;              // kernels launched through this ctx (hardkv_launch_count)
+  char *stage_q, *stage_k, *stage_v;  // device staging of hardkv_decode_step_host (inside the workspace)
+  float *stage_out;
 };
 
 namespace {
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout { size_t part, arrive, total; };
+struct WsLayout { size_t part, arrive, stage_q, stage_k, stage_v, stage_out, total; };
+
+size_t esize_of(const hardkv_config &c) { return c.kv_dtype == HARDKV_F32 ? 4 : 2; }
 
 int att_chunks_of(const hardkv_config &c) {
   return (c.sink + c.recent + c.k_cap + c.cond_cap + ATT_CHUNK - 1) / ATT_CHUNK;
@@ -34,6 +39,11 @@ WsLayout ws_layout(const hardkv_config &c) {
   size_t off = 0;
   w.arrive = off; off += align256(units * sizeof(int32_t));
   w.part = off;   off += align256(units * att_chunks_of(c) * G * (c.head_dim + 2) * sizeof(float));
+  const size_t qb = (size_t)c.batch * c.num_q_heads * c.head_dim, kb = units * c.head_dim;
+  w.stage_q = off;   off += align256(qb * esize_of(c));
+  w.stage_k = off;   off += align256(kb * esize_of(c));
+  w.stage_v = off;   off += align256(kb * esize_of(c));
+  w.stage_out = off; off += align256(qb * sizeof(float));
   w.total = off;
   return w;
 }
@@ -89,27 +99,32 @@ Params params_of(const hardkv_ctx *ctx, const hardkv_state *s) {
     }                                                                                              \
   } while (0)
 
-void launch_append(const hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, cudaStream_t st) {
+void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, cudaStream_t st) {
+  ctx->launches += 1;
   HK_DISPATCH_TD(ctx->cfg, (append_retire_kernel<T, D><<<P.B, 256, 0, st>>>(P, k_new, v_new)));
 }
 
-void launch_score(const hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
+void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
+  ctx->launches += 1;
   dim3 grid((P.ppu + SCORE_PAGES_PER_CTA - 1) / SCORE_PAGES_PER_CTA, P.B * P.Hkv);
   HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (score_generic_kernel<T, D, G><<<grid, 256, 0, st>>>(P, q))));
 }
 
-void launch_select(const hardkv_ctx *, const Params &P, float p, bool calibrate, cudaStream_t st) {
+void launch_select(hardkv_ctx *ctx, const Params &P, float p, bool calibrate, cudaStream_t st) {
+  ctx->launches += 1;
   if (calibrate) select_kernel<1><<<P.B * P.Hkv, SEL_NT, SEL_SMEM, st>>>(P, p);
   else select_kernel<0><<<P.B * P.Hkv, SEL_NT, SEL_SMEM, st>>>(P, p);
 }
 
-void launch_rewrite(const hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
+void launch_rewrite(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
+  ctx->launches += 1;
   dim3 grid((P.k_cap + RW_ROWS_PER_CTA - 1) / RW_ROWS_PER_CTA, P.B * P.Hkv);
   HK_DISPATCH_TD(ctx->cfg, (rewrite_kernel<T, D><<<grid, 256, 0, st>>>(P)));
 }
 
-void launch_attend(const hardkv_ctx *ctx, const Params &P, const void *q, float *out, float *lse, bool fused,
+void launch_attend(hardkv_ctx *ctx, const Params &P, const void *q, float *out, float *lse, bool fused,
                    cudaStream_t st) {
+  ctx->launches += 1;
   dim3 grid(P.att_chunks, P.B * P.Hkv);
   if (fused)
     HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, true><<<grid, 256, 0, st>>>(P, q, out, lse))));
@@ -163,6 +178,8 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   char *base = reinterpret_cast<char *>(workspace);
   P.att_arrive = reinterpret_cast<int32_t *>(base + w.arrive);
   P.part = reinterpret_cast<float *>(base + w.part);
+  ctx->stage_q = base + w.stage_q; ctx->stage_k = base + w.stage_k; ctx->stage_v = base + w.stage_v;
+  ctx->stage_out = reinterpret_cast<float *>(base + w.stage_out);
   // opt in to the large dynamic shared memory of the select kernel (host-side attribute, no stream work)
   if (cudaFuncSetAttribute(select_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SEL_SMEM) != cudaSuccess ||
       cudaFuncSetAttribute(select_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SEL_SMEM) != cudaSuccess) {
@@ -226,6 +243,15 @@ hardkv_status hardkv_decode_attn(hardkv_ctx *ctx, const hardkv_state *s, const v
   return launch_status();
 }
 
+hardkv_status hardkv_rewrite_attend(hardkv_ctx *ctx, const hardkv_state *s, const void *q, float *out, float *lse,
+                                    hardkv_stream st) {
+  if (!state_ok(ctx, s) || !q || !out) return HARDKV_ERR_INVALID_ARG;
+  launch_attend(ctx, params_of(ctx, s), q, out, lse, true, st);
+  return launch_status();
+}
+
+int64_t hardkv_launch_count(const hardkv_ctx *ctx) { return ctx ? ctx->launches : -1; }
+
 hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const void *q, const void *k_new,
                                  const void *v_new, float p, int32_t do_select, float *out, float *lse,
                                  hardkv_stream st) {
@@ -239,6 +265,25 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   }
   launch_attend(ctx, P, q, out, lse, do_select != 0, st);
   return launch_status();
+}
+
+hardkv_status hardkv_decode_step_host(hardkv_ctx *ctx, const hardkv_state *s, const void *q_host,
+                                      const void *k_new_host, const void *v_new_host, float p, int32_t do_select,
+                                      float *out_host, hardkv_stream st) {
+  if (!ctx || !q_host || !k_new_host || !v_new_host || !out_host) return HARDKV_ERR_INVALID_ARG;
+  const hardkv_config &c = ctx->cfg;
+  const size_t qe = (size_t)c.batch * c.num_q_heads * c.head_dim, ke = (size_t)c.batch * c.num_kv_heads * c.head_dim;
+  const size_t es = esize_of(c);
+  if (cudaMemcpyAsync(ctx->stage_q, q_host, qe * es, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+      cudaMemcpyAsync(ctx->stage_k, k_new_host, ke * es, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+      cudaMemcpyAsync(ctx->stage_v, v_new_host, ke * es, cudaMemcpyHostToDevice, st) != cudaSuccess)
+    return HARDKV_ERR_CUDA;
+  hardkv_status r = hardkv_decode_step(ctx, s, ctx->stage_q, ctx->stage_k, ctx->stage_v, p, do_select,
+                                       ctx->stage_out, nullptr, st);
+  if (r != HARDKV_OK) return r;
+  if (cudaMemcpyAsync(out_host, ctx->stage_out, qe * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess)
+    return HARDKV_ERR_CUDA;
+  return HARDKV_OK;
 }
 
 }  // extern "C"

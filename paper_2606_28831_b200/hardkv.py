@@ -55,7 +55,8 @@ class StateStruct(C.Structure):
 F32, BF16 = 0, 1
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
            "hardkv_set_variant", "hardkv_append_kv", "hardkv_score", "hardkv_calibrate_topp",
-           "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_decode_step"]
+           "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend",
+           "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count"]
 
 
 def _load():
@@ -77,9 +78,13 @@ def _load():
     lib.hardkv_topp_select.argtypes = [vp, sp, C.c_float, vp]
     lib.hardkv_rewrite.argtypes = [vp, sp, vp]
     lib.hardkv_decode_attn.argtypes = [vp, sp, vp, vp, vp, vp]
+    lib.hardkv_rewrite_attend.argtypes = [vp, sp, vp, vp, vp, vp]
     lib.hardkv_decode_step.argtypes = [vp, sp, vp, vp, vp, C.c_float, C.c_int32, vp, vp, vp]
+    lib.hardkv_decode_step_host.argtypes = [vp, sp, vp, vp, vp, C.c_float, C.c_int32, vp, vp]
+    lib.hardkv_launch_count.argtypes = [vp]
+    lib.hardkv_launch_count.restype = C.c_int64
     for n in EXPORTS:
-        if n not in ("hardkv_destroy", "hardkv_status_string"):
+        if n not in ("hardkv_destroy", "hardkv_status_string", "hardkv_launch_count"):
             getattr(lib, n).restype = C.c_int
     return lib
 
@@ -163,6 +168,21 @@ class HardKV:
 
     def decode_attn(self, st: DeviceState, q, out, lse=None):
         _check(lib.hardkv_decode_attn(self._ctx, C.byref(st.struct()), _ptr(q), _ptr(out), _ptr(lse), _stream()))
+
+    def rewrite_attend(self, st: DeviceState, q, out, lse=None):
+        _check(lib.hardkv_rewrite_attend(self._ctx, C.byref(st.struct()), _ptr(q), _ptr(out), _ptr(lse), _stream()))
+
+    def launch_count(self) -> int:
+        return int(lib.hardkv_launch_count(self._ctx))
+
+    def decode_step_host(self, st: DeviceState, q_host, k_new_host, v_new_host, p: float, out_host,
+                         do_select: bool = True):
+        """q_host / k_new_host / v_new_host / out_host: HOST (ideally pinned) torch tensors; see hardkv.h."""
+        for t in (q_host, k_new_host, v_new_host, out_host):
+            assert not t.is_cuda and t.is_contiguous()
+        _check(lib.hardkv_decode_step_host(self._ctx, C.byref(st.struct()), _ptr(q_host), _ptr(k_new_host),
+                                           _ptr(v_new_host), np.float32(p), int(do_select), _ptr(out_host),
+                                           _stream()))
 
     def decode_step(self, st: DeviceState, q, k_new, v_new, p: float, out, lse=None, do_select: bool = True):
         _check(lib.hardkv_decode_step(self._ctx, C.byref(st.struct()), _ptr(q), _ptr(k_new), _ptr(v_new),

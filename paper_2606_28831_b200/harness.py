@@ -104,3 +104,17 @@ def gather_rows(pool: torch.Tensor, table_unit: torch.Tensor, n: int) -> np.ndar
     """Logical rows 0..n-1 of one unit from a paged pool -> float32 host array [n][d]."""
     d = pool.shape[-1]
     return pool[table_unit.long()].reshape(-1, d)[:n].float().cpu().numpy()
+
+
+_MUTABLE = ["votes", "cond_k", "cond_v", "cond_pos", "cond_votes", "cond_count", "ctx_len", "c_lo", "sel_idx",
+            "sel_count", "sel_table", "acc", "ring", "ring_slot"]
+
+
+def snapshot(st: hardkv.DeviceState) -> dict:
+    """Clone the tensors a decode step mutates (appended KV rows are rewritten identically on a rerun)."""
+    return {n: getattr(st, n).clone() for n in _MUTABLE if getattr(st, n) is not None}
+
+
+def restore(st: hardkv.DeviceState, snap: dict) -> None:
+    for n, t in snap.items():
+        getattr(st, n).copy_(t)
