@@ -19,8 +19,8 @@ struct Params {
   // workspace
   float *part;          // [units][att_chunks][G][d + 2] split-K partial states (m, l, acc[d])
   int32_t *att_arrive;  // [units] arrival counters of the split-K merge (zero between launches)
-  float *stat_part;     // [units][G][score_chunks][2] per-chunk softmax statistics (m, s)
-  int score_chunks;
+  int sel_cluster;       // CTAs per (b, h) cluster of the select kernel
+  int sel_slice_cap;     // capacity (tokens) of one CTA's probability slice in shared memory
 };
 
 // ---- 16-byte vector access -------------------------------------------------------------------
@@ -71,6 +71,16 @@ __device__ __forceinline__ void pool_bounds(const Params &P, int b, int &n, int 
 __device__ __forceinline__ unsigned long long shfl_xor_u64(unsigned long long v, int off) {
   unsigned lo = __shfl_xor_sync(0xffffffffu, (unsigned)v, off);
   unsigned hi = __shfl_xor_sync(0xffffffffu, (unsigned)(v >> 32), off);
+  return ((unsigned long long)hi << 32) | lo;
+}
+__device__ __forceinline__ unsigned long long shfl_up_u64(unsigned long long v, int off) {
+  unsigned lo = __shfl_up_sync(0xffffffffu, (unsigned)v, off);
+  unsigned hi = __shfl_up_sync(0xffffffffu, (unsigned)(v >> 32), off);
+  return ((unsigned long long)hi << 32) | lo;
+}
+__device__ __forceinline__ unsigned long long shfl_u64(unsigned long long v, int src) {
+  unsigned lo = __shfl_sync(0xffffffffu, (unsigned)v, src);
+  unsigned hi = __shfl_sync(0xffffffffu, (unsigned)(v >> 32), src);
   return ((unsigned long long)hi << 32) | lo;
 }
 __device__ __forceinline__ unsigned long long warp_sum_u64(unsigned long long v) {

@@ -48,6 +48,20 @@ WsLayout ws_layout(const hardkv_config &c) {
   return w;
 }
 
+size_t select_smem_bytes(const Params &P) { return (size_t)P.sel_slice_cap * 4 + sizeof(SelShared); }
+
+// Cluster size of the select kernel: enough CTAs per (b, h) to keep a slice near 8.5k tokens and
+// to spread few units over the chip (one wave of 512-thread CTAs is about 4 x 148).
+void select_geometry(const hardkv_config &c, int *cluster, int *slice_cap) {
+  const int units = c.batch * c.num_kv_heads;
+  const int max_pool = c.max_ctx - c.recent > 0 ? c.max_ctx - c.recent : 1;
+  int cmin = 1, cpar = 1;
+  while (cmin < SEL_MAXC && (max_pool + cmin - 1) / cmin > 8704) cmin <<= 1;
+  while (cpar * 2 <= SEL_MAXC && cpar * 2 * units <= 592) cpar <<= 1;
+  *cluster = cmin > cpar ? cmin : cpar;
+  *slice_cap = sel_slice_len(max_pool, *cluster);
+}
+
 hardkv_status check_config(const hardkv_config *c) {
   if (!c) return HARDKV_ERR_INVALID_ARG;
   if (c->batch <= 0 || c->num_q_heads <= 0 || c->num_kv_heads <= 0 || c->head_dim <= 0) return HARDKV_ERR_INVALID_ARG;
@@ -60,6 +74,9 @@ hardkv_status check_config(const hardkv_config *c) {
   const bool tok = (c->kv_dtype == HARDKV_F32 && c->head_dim == 64) ||
                    (c->kv_dtype == HARDKV_BF16 && (c->head_dim == 64 || c->head_dim == 128));
   if (!gok || !tok) return HARDKV_ERR_UNSUPPORTED;
+  int cl, cap;
+  select_geometry(*c, &cl, &cap);
+  if ((size_t)cap * 4 + sizeof(SelShared) > 227u * 1024u) return HARDKV_ERR_UNSUPPORTED;  // pool slice must fit one SM
   return HARDKV_OK;
 }
 
@@ -112,8 +129,18 @@ void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t 
 
 void launch_select(hardkv_ctx *ctx, const Params &P, float p, bool calibrate, cudaStream_t st) {
   ctx->launches += 1;
-  if (calibrate) select_kernel<1><<<P.B * P.Hkv, SEL_NT, SEL_SMEM, st>>>(P, p);
-  else select_kernel<0><<<P.B * P.Hkv, SEL_NT, SEL_SMEM, st>>>(P, p);
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3(P.B * P.Hkv * P.sel_cluster);
+  lc.blockDim = dim3(SEL_NT);
+  lc.dynamicSmemBytes = select_smem_bytes(P);
+  lc.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = P.sel_cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  lc.attrs = at;
+  lc.numAttrs = 1;
+  if (calibrate) cudaLaunchKernelEx(&lc, select_kernel<1>, P, p);
+  else cudaLaunchKernelEx(&lc, select_kernel<0>, P, p);
 }
 
 void launch_rewrite(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
@@ -180,9 +207,13 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.part = reinterpret_cast<float *>(base + w.part);
   ctx->stage_q = base + w.stage_q; ctx->stage_k = base + w.stage_k; ctx->stage_v = base + w.stage_v;
   ctx->stage_out = reinterpret_cast<float *>(base + w.stage_out);
-  // opt in to the large dynamic shared memory of the select kernel (host-side attribute, no stream work)
-  if (cudaFuncSetAttribute(select_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SEL_SMEM) != cudaSuccess ||
-      cudaFuncSetAttribute(select_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SEL_SMEM) != cudaSuccess) {
+  select_geometry(*cfg, &P.sel_cluster, &P.sel_slice_cap);
+  // opt in to the large dynamic shared memory of the select kernel (host-side attribute, no stream work);
+  // the attribute is per function, so it is raised to the largest request seen in this process
+  static size_t sel_smem_max = 0;
+  if (select_smem_bytes(P) > sel_smem_max) sel_smem_max = select_smem_bytes(P);
+  if (cudaFuncSetAttribute(select_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess ||
+      cudaFuncSetAttribute(select_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess) {
     cudaGetLastError();
     delete ctx;
     return HARDKV_ERR_CUDA;

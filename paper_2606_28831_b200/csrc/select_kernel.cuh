@@ -1,46 +1,84 @@
 // select_kernel.cuh -- Logits Calibration (apply-T) + Top-p nucleus + stream compaction.
-// One CTA per (sequence, KV head).  PAPER.md L106-128 (calibration), L108 (Top-p), L86 (votes),
-// L207-209 / L439 (head-wise block table, packed mask); readings C2-C6, C9.
+// PAPER.md L106-128 (calibration), L108 (Top-p), L86 (votes), L207-209 / L439 (head-wise block
+// table, packed mask); readings C2-C6, C9.
+//
+// One thread-block CLUSTER per (sequence, KV head); the C CTAs of a cluster split the pool into
+// contiguous, 32-aligned position slices and keep their slice of the probability row (fp32 bit
+// patterns) in shared memory for the whole kernel.  Cross-CTA exchange goes through distributed
+// shared memory (DSMEM) and cluster barriers; nothing but the final results touches HBM.
 //
 // The nucleus is found without a sort: a most-significant-digit radix descent on the fp32 bit
-// pattern of P (all P >= 0, so unsigned order == float order), 5 bits per level.  Each level
-// builds, per digit, (count, integer mass) with w_i = rn(P_i * 2^32) in u64: exact and order
-// independent, so it reproduces a sorted-prefix definition bit for bit (reading C5).
-// Histograms are PRIVATE per thread (hist[digit][tid], one packed u64 = count << 40 | mass):
-// plain LDS/STS, no atomics -- shared-memory atomics retire about one lane per clock and would
-// bound the whole step on long rows.
+// pattern of P (all P >= 0, so unsigned order == float order) with digits of 11, 10 and 10 bits.
+// Each level builds a histogram of (count, integer mass) per digit with w_i = rn(P_i * 2^32)
+// summed exactly (u32 shared atomics on count, w >> 12 and w & 4095): exact and order
+// independent, so it reproduces a sorted-prefix definition bit for bit (reading C5).  The bins
+// are merged across the cluster by their owner CTA, and every CTA then walks the merged bins from
+// the top to the bin in which the mass reaches Theta = ceil(p * Wtot) (or the count reaches
+// k_cap, reading C6).
 #pragma once
+#include <cooperative_groups.h>
+
 #include "common.cuh"
 
 namespace hardkv {
+namespace cg = cooperative_groups;
 
 constexpr int SEL_NT = 512;
-constexpr int SEL_BINS = 32;
-constexpr int SEL_DIGIT = 5;
 constexpr int SEL_NW = SEL_NT / 32;
-constexpr size_t SEL_SMEM = (size_t)SEL_BINS * SEL_NT * 8;
+constexpr int SEL_MAXC = 8;        // portable cluster size limit
+constexpr int SEL_NB = 2048;       // bins of the widest level
+constexpr int SEL_MSPLIT = 12;     // mass kept as (w >> 12, w & 4095) in two u32 counters
+constexpr uint32_t SEL_INVALID = 0xffffffffu;  // slice entry outside the pool (never a probability)
+
+struct SelShared {
+  uint32_t h_cnt[SEL_NB], h_hi[SEL_NB], h_lo[SEL_NB];  // local histogram of the current level
+  uint32_t m_cnt[SEL_NB / 2];                          // bins owned by this CTA, merged over the cluster
+  unsigned long long m_mass[SEL_NB / 2];
+  unsigned long long tot_mass[SEL_MAXC];               // per owner range: totals (written by the owner into every CTA)
+  uint32_t tot_cnt[SEL_MAXC];
+  float st_m[SEL_MAXC][8], st_s[SEL_MAXC][8];          // per CTA softmax statistics of the G query heads
+  double acc_tot[SEL_MAXC];
+  int c_gt[SEL_MAXC], c_tie[SEL_MAXC];
+  float red_f[SEL_NW][8][2];
+  double red_d[SEL_NW];
+  unsigned long long red_u[SEL_NW];
+  uint32_t red_c[SEL_NW];
+  int w_gt[SEL_NW], w_tie[SEL_NW];
+  // result of one level's walk (written by warp 0)
+  int res_bin, res_bin_cnt, res_cum_cnt;
+  unsigned long long res_cum_mass, res_theta;
+};
 
 __device__ __forceinline__ unsigned long long mass_of_bits(uint32_t bits) {
   // w = rn(P * 2^32): the product is exact in fp32 (power-of-two scale), conversion rounds to nearest even
   return __float2ull_rn(__uint_as_float(bits) * 4294967296.0f);
 }
 
-struct SelShared {
-  float red_f[SEL_NW][8][2];
-  unsigned long long red_u[SEL_NW];
-  double red_d[SEL_NW];
-  unsigned long long bin[SEL_BINS];
-  int w_gt[SEL_NW], w_tie[SEL_NW];
-  uint32_t mask_words[1];  // placeholder (mask is staged in the histogram area)
-};
+__device__ __forceinline__ void hist_add(SelShared &sh, int bin, uint32_t bits) {
+  const unsigned long long w = mass_of_bits(bits);
+  atomicAdd(&sh.h_cnt[bin], 1u);
+  atomicAdd(&sh.h_hi[bin], (uint32_t)(w >> SEL_MSPLIT));
+  atomicAdd(&sh.h_lo[bin], (uint32_t)(w & ((1u << SEL_MSPLIT) - 1u)));
+}
+
+// Per-CTA slice geometry: the cluster covers absolute positions [base, base + C*per), base = lo & ~31.
+__host__ __device__ __forceinline__ int sel_slice_len(int span, int C) {
+  const int per = (span + C - 1) / C;
+  return (per + SEL_NT - 1) / SEL_NT * SEL_NT;
+}
 
 // CALIBRATE: 1 = logits -> probs (2a) then select; 0 = select on state->probs as given.
 template <int CALIBRATE>
 __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
-  extern __shared__ unsigned long long s_hist[];  // [SEL_BINS][SEL_NT]
-  __shared__ SelShared sh;
-  const int unit = blockIdx.x, b = unit / P.Hkv, h = unit % P.Hkv;
+  extern __shared__ __align__(16) unsigned char sel_smem[];
+  cg::cluster_group cluster = cg::this_cluster();
+  const int C = P.sel_cluster;
+  const int rank = (int)cluster.block_rank();
+  const int unit = blockIdx.x / C, b = unit / P.Hkv, h = unit % P.Hkv;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  uint32_t *pbits = reinterpret_cast<uint32_t *>(sel_smem);                       // [P.sel_slice_cap]
+  SelShared &sh = *reinterpret_cast<SelShared *>(sel_smem + (size_t)P.sel_slice_cap * 4);
+
   int n, lo, hi;
   pool_bounds(P, b, n, lo, hi);
   const int N = hi - lo;
@@ -48,19 +86,51 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
   float *probs = P.st.probs + (size_t)unit * P.max_ctx;
   int32_t *sel_idx = P.st.sel_idx + (size_t)unit * P.k_cap;
   int32_t *sel_table = P.st.sel_table + (size_t)unit * P.spu;
+  const bool want_mask = P.st.sel_mask != nullptr;
+  uint8_t *mask = want_mask ? P.st.sel_mask + (size_t)unit * (P.max_ctx / 8) : nullptr;
+  const int mask_bytes = P.max_ctx / 8;
+
+  if (N <= 0) {  // empty pool: nothing selected (uniform over the cluster: no barrier is pending)
+    for (int j = rank * SEL_NT + tid; j < P.k_cap; j += C * SEL_NT) sel_idx[j] = -1;
+    for (int j = rank * SEL_NT + tid; j < P.spu; j += C * SEL_NT) sel_table[j] = -1;
+    if (want_mask)
+      for (int y = rank * SEL_NT + tid; y < mask_bytes; y += C * SEL_NT) mask[y] = 0;
+    if (rank == 0 && tid == 0) P.st.sel_count[unit] = 0;
+    return;
+  }
+
+  const int base = lo & ~31;
+  const int per = sel_slice_len(hi - base, C);   // <= P.sel_slice_cap by construction of the cap
+  const int s0 = base + rank * per;              // this CTA's slice: absolute positions [s0, s0 + per)
+  const int wseg = per / SEL_NW;                 // positions per warp (multiple of 32)
+
+  // split-phase cluster barrier: every CTA of the cluster must be running before its shared memory
+  // is written by a peer; the wait sits in front of the first DSMEM access.
+  if (C > 1) cluster.barrier_arrive();
+  for (int d = tid; d < SEL_NB; d += SEL_NT) { sh.h_cnt[d] = 0; sh.h_hi[d] = 0; sh.h_lo[d] = 0; }
 
   // ---------------- 2a: calibration ------------------------------------------------------------
-  if (CALIBRATE && N > 0) {
+  if (CALIBRATE) {
     const float invT = 1.0f / P.st.temperature[unit];
     const float *lg = P.st.logits + ((size_t)(b * P.Hq + h * G)) * P.max_ctx;
     // per query head: max and sum of exp over the pool (softmax over the pool only, reading C3)
-    float mg[8], sg[8];
-    for (int g = 0; g < G; ++g) {
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      if (g >= G) break;
+      const float *row = lg + (size_t)g * P.max_ctx;
       float m = -INFINITY, s = 0.f;
-      for (int i = lo + tid; i < hi; i += SEL_NT) {
-        const float x = __ldcg(lg + (size_t)g * P.max_ctx + i) * invT;
-        if (x > m) { s *= expf(m - x); m = x; }
-        s += expf(x - m);
+      for (int i0 = tid; i0 < per; i0 += 4 * SEL_NT) {
+        float x[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int pos = s0 + i0 + u * SEL_NT;
+          x[u] = (i0 + u * SEL_NT < per && pos >= lo && pos < hi) ? __ldcg(row + pos) * invT : -INFINITY;
+        }
+        const float mn = fmaxf(fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3])), m);
+        if (mn != -INFINITY) {
+          s = s * expf(m - mn) + expf(x[0] - mn) + expf(x[1] - mn) + expf(x[2] - mn) + expf(x[3] - mn);
+          m = mn;
+        }
       }
 #pragma unroll
       for (int o = 16; o; o >>= 1) {
@@ -72,26 +142,54 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
       if (lane == 0) { sh.red_f[warp][g][0] = m; sh.red_f[warp][g][1] = s; }
     }
     __syncthreads();
-    for (int g = 0; g < G; ++g) {
-      float m = -INFINITY;
-      for (int w = 0; w < SEL_NW; ++w) m = fmaxf(m, sh.red_f[w][g][0]);
-      float s = 0.f;
-      for (int w = 0; w < SEL_NW; ++w) {
-        const float mw = sh.red_f[w][g][0];
-        if (mw != -INFINITY) s += sh.red_f[w][g][1] * expf(mw - m);
+    if (C > 1) cluster.barrier_wait();
+    if (tid < C * 8) {  // thread (c, g): publish this CTA's (m_g, s_g) into CTA c
+      const int c = tid >> 3, g = tid & 7;
+      float m = -INFINITY, s = 0.f;
+      if (g < G) {
+        for (int w = 0; w < SEL_NW; ++w) m = fmaxf(m, sh.red_f[w][g][0]);
+        for (int w = 0; w < SEL_NW; ++w) {
+          const float mw = sh.red_f[w][g][0];
+          if (mw != -INFINITY) s += sh.red_f[w][g][1] * expf(mw - m);
+        }
+      }
+      SelShared *dst = cluster.map_shared_rank(&sh, c);
+      dst->st_m[rank][g] = m;
+      dst->st_s[rank][g] = s;
+    }
+    cluster.sync();
+    float mg[8], rs[8];
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      float m = -INFINITY, s = 0.f;
+      if (g < G) {
+        for (int c = 0; c < C; ++c) m = fmaxf(m, sh.st_m[c][g]);
+        for (int c = 0; c < C; ++c) {
+          const float mc = sh.st_m[c][g];
+          if (mc != -INFINITY) s += sh.st_s[c][g] * expf(mc - m);
+        }
       }
       mg[g] = m;
-      sg[g] = 1.0f / s;
+      rs[g] = 1.0f / s;
     }
     const float invG = 1.0f / (float)G;
     const bool accum = P.st.score_mode[h] == HARDKV_SCORE_ACCUM;
     if (!accum) {
       // S_hat = softmax(z / T) per query head (Solution 1, L120), group mean (reading C2)
-      for (int i = lo + tid; i < hi; i += SEL_NT) {
-        float pr = 0.f;
-        for (int g = 0; g < G; ++g)
-          pr += expf(__ldcg(lg + (size_t)g * P.max_ctx + i) * invT - mg[g]) * sg[g];
-        probs[i] = pr * invG;
+      for (int i = tid; i < per; i += SEL_NT) {
+        const int pos = s0 + i;
+        uint32_t bits = SEL_INVALID;
+        if (pos >= lo && pos < hi) {
+          float pr = 0.f;
+#pragma unroll
+          for (int g = 0; g < 8; ++g)
+            if (g < G) pr += expf(__ldcg(lg + (size_t)g * P.max_ctx + pos) * invT - mg[g]) * rs[g];
+          pr *= invG;
+          probs[pos] = pr;
+          bits = __float_as_uint(pr);
+          hist_add(sh, bits >> 20, bits);
+        }
+        pbits[i] = bits;
       }
     } else {
       // ACCUM (reading C4): sliding sum of the last accum_window per-step rows, renormalised.
@@ -99,95 +197,229 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
       float *acc = P.st.acc + (size_t)unit * P.max_ctx;
       float *ring = P.st.ring + ((size_t)unit * P.accum_window + slot) * P.max_ctx;
       double tot = 0.0;
-      for (int i = lo + tid; i < hi; i += SEL_NT) {
-        float pr = 0.f;
-        for (int g = 0; g < G; ++g)
-          pr += expf(__ldcg(lg + (size_t)g * P.max_ctx + i) * invT - mg[g]) * sg[g];
-        pr *= invG;
-        float a = (acc[i] - ring[i]) + pr;
-        a = fmaxf(a, 0.f);
-        acc[i] = a;
-        ring[i] = pr;
-        tot += (double)a;
+      for (int i = tid; i < per; i += SEL_NT) {
+        const int pos = s0 + i;
+        uint32_t bits = SEL_INVALID;
+        if (pos >= lo && pos < hi) {
+          float pr = 0.f;
+#pragma unroll
+          for (int g = 0; g < 8; ++g)
+            if (g < G) pr += expf(__ldcg(lg + (size_t)g * P.max_ctx + pos) * invT - mg[g]) * rs[g];
+          pr *= invG;
+          float a = (acc[pos] - ring[pos]) + pr;
+          a = fmaxf(a, 0.f);
+          acc[pos] = a;
+          ring[pos] = pr;
+          tot += (double)a;
+          bits = __float_as_uint(a);  // acc for now; normalised below
+        }
+        pbits[i] = bits;
       }
 #pragma unroll
       for (int o = 16; o; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
       if (lane == 0) sh.red_d[warp] = tot;
       __syncthreads();
+      if (tid < C) {
+        double t = 0.0;
+        for (int w = 0; w < SEL_NW; ++w) t += sh.red_d[w];
+        cluster.map_shared_rank(&sh, tid)->acc_tot[rank] = t;
+      }
+      cluster.sync();
       tot = 0.0;
-      for (int w = 0; w < SEL_NW; ++w) tot += sh.red_d[w];
-      for (int i = lo + tid; i < hi; i += SEL_NT)
-        probs[i] = tot > 0.0 ? (float)((double)acc[i] / tot) : 0.f;
-      if (tid == 0) P.st.ring_slot[unit] = (slot + 1) % P.accum_window;
+      for (int c = 0; c < C; ++c) tot += sh.acc_tot[c];
+      for (int i = tid; i < per; i += SEL_NT) {
+        const uint32_t ab = pbits[i];
+        if (ab == SEL_INVALID) continue;
+        const float pr = tot > 0.0 ? (float)((double)__uint_as_float(ab) / tot) : 0.f;
+        probs[s0 + i] = pr;
+        const uint32_t bits = __float_as_uint(pr);
+        pbits[i] = bits;
+        hist_add(sh, bits >> 20, bits);
+      }
+      if (rank == 0 && tid == 0) P.st.ring_slot[unit] = (slot + 1) % P.accum_window;
     }
-    __syncthreads();  // probs written by this CTA are read back below
+  } else {
+    __syncthreads();  // histogram zeroed
+    if (C > 1) cluster.barrier_wait();
+    for (int i = tid; i < per; i += SEL_NT) {
+      const int pos = s0 + i;
+      uint32_t bits = SEL_INVALID;
+      if (pos >= lo && pos < hi) {
+        bits = __float_as_uint(probs[pos]) & 0x7fffffffu;
+        hist_add(sh, bits >> 20, bits);
+      }
+      pbits[i] = bits;
+    }
   }
 
   // ---------------- 2b: Top-p threshold --------------------------------------------------------
-  const uint32_t *row = reinterpret_cast<const uint32_t *>(probs) + lo;  // bit patterns of the pool
+  const bool all = (p >= 1.0f) || (N <= P.st.l_lower[b]);  // no sparsity yet (L197, reading C8)
+  const int kt = P.k_cap;                                   // reading C6: k = min(k_topp, k_cap), same order
   uint32_t tau = 0;          // bit pattern of the smallest selected P
   int r_ties = 0x7fffffff;   // how many tokens with P == tau are taken (ascending position)
   int k = 0;
-  if (N > 0) {
-    const bool all = (p >= 1.0f) || (N <= P.st.l_lower[b]);  // no sparsity yet (L197, reading C8)
-    unsigned long long theta = ~0ull;
-    if (!all) {
-      unsigned long long wsum = 0;
-      for (int i = tid; i < N; i += SEL_NT) wsum += mass_of_bits(row[i]);
-      wsum = warp_sum_u64(wsum);
-      if (lane == 0) sh.red_u[warp] = wsum;
+  {
+    uint32_t prefix = 0;
+    unsigned long long theta = ~0ull, cum_mass = 0;
+    int cum_cnt = 0, bin_cnt = 0;
+    bool everything = false;
+#pragma unroll 1
+    for (int level = 0; level < 3; ++level) {
+      const int db = level == 0 ? 11 : 10;          // digit bits
+      const int shift = level == 0 ? 20 : (level == 1 ? 10 : 0);
+      const int nb = 1 << db;
+      if (level > 0) {
+        // histogram of the next digit over the tokens whose high bits equal the prefix
+        for (int d = tid; d < nb; d += SEL_NT) { sh.h_cnt[d] = 0; sh.h_hi[d] = 0; sh.h_lo[d] = 0; }
+        __syncthreads();
+        const int hs = shift + db;
+        for (int i = tid; i < per; i += SEL_NT) {
+          const uint32_t bits = pbits[i];
+          if ((bits >> hs) == prefix) hist_add(sh, (bits >> shift) & (nb - 1), bits);
+        }
+      }
       __syncthreads();
-      unsigned long long wtot = 0;
-      for (int w = 0; w < SEL_NW; ++w) wtot += sh.red_u[w];
-      // Theta = ceil(p * Wtot) in double: one correctly rounded multiply, identical on host and device
-      theta = (unsigned long long)ceil(__dmul_rn((double)p, (double)wtot));
-      if (theta < 1) theta = 1;
-      if (theta > wtot) theta = ~0ull;  // unreachable mass (Wtot == 0): the nucleus is the whole pool
-    }
-    const int kt = P.k_cap;  // reading C6: k = min(k_topp, k_cap), same order
-    if (theta == ~0ull && N <= kt) {
-      k = N;  // everything: tau = 0, all ties taken
-    } else {
-      uint32_t prefix = 0;
-      int shift = 31;  // unresolved low bits (bit 31 is the sign: always 0)
-      unsigned long long cum_mass = 0;
-      int cum_cnt = 0, bin_cnt = 0;
-      while (shift > 0) {
-        const int db = shift < SEL_DIGIT ? shift : SEL_DIGIT;
-        const int nb = 1 << db;
-        const int hs = shift;  // bits above the digit: row >> hs == prefix
-        shift -= db;
-        for (int d = 0; d < nb; ++d) s_hist[d * SEL_NT + tid] = 0ull;
-        for (int i = tid; i < N; i += SEL_NT) {
-          const uint32_t bits = row[i];
-          if ((bits >> hs) == prefix) {
-            const int d = (bits >> shift) & (nb - 1);
-            s_hist[d * SEL_NT + tid] += (1ull << 40) + mass_of_bits(bits);
+      const int S = nb / C;  // bins per owner CTA (>= 128)
+      if (C > 1) {
+        cluster.sync();      // A: every local histogram of this level is complete
+        unsigned long long tm = 0;
+        uint32_t tc = 0;
+        for (int j = tid; j < S; j += SEL_NT) {
+          const int bin = rank * S + j;
+          uint32_t c_ = 0;
+          unsigned long long hi_ = 0, lo_ = 0;
+          for (int c = 0; c < C; ++c) {
+            const SelShared *src = cluster.map_shared_rank(&sh, c);
+            c_ += src->h_cnt[bin];
+            hi_ += src->h_hi[bin];
+            lo_ += src->h_lo[bin];
+          }
+          const unsigned long long ms = (hi_ << SEL_MSPLIT) + lo_;
+          sh.m_cnt[j] = c_;
+          sh.m_mass[j] = ms;
+          tc += c_;
+          tm += ms;
+        }
+        tm = warp_sum_u64(tm);
+        tc = __reduce_add_sync(0xffffffffu, tc);
+        if (lane == 0) { sh.red_u[warp] = tm; sh.red_c[warp] = tc; }
+        __syncthreads();
+        if (tid < C) {
+          unsigned long long m_ = 0;
+          uint32_t c_ = 0;
+          for (int w = 0; w < SEL_NW; ++w) { m_ += sh.red_u[w]; c_ += sh.red_c[w]; }
+          SelShared *dst = cluster.map_shared_rank(&sh, tid);
+          dst->tot_mass[rank] = m_;
+          dst->tot_cnt[rank] = c_;
+        }
+        cluster.sync();      // B: merged ranges and range totals are visible
+      }
+      if (warp == 0) {
+        // ---- walk the merged bins from the top (every CTA computes the same result) ----
+        int q = 0;  // owner range that holds the crossing
+        if (C > 1) {
+          if (level == 0) {
+            unsigned long long wtot = 0;
+            for (int c = 0; c < C; ++c) wtot += sh.tot_mass[c];
+            if (!all) {
+              // Theta = ceil(p * Wtot) in double: one correctly rounded multiply, identical on host and device
+              theta = (unsigned long long)ceil(__dmul_rn((double)p, (double)wtot));
+              if (theta < 1) theta = 1;
+              if (theta > wtot) theta = ~0ull;  // unreachable mass (Wtot == 0): the nucleus is the whole pool
+            }
+            everything = (theta == ~0ull && N <= kt);
+          }
+          if (!everything) {
+            for (q = C - 1; q > 0; --q) {
+              const unsigned long long rm = sh.tot_mass[q];
+              const int rc = (int)sh.tot_cnt[q];
+              if ((theta != ~0ull && cum_mass + rm >= theta) || cum_cnt + rc >= kt) break;
+              cum_mass += rm;
+              cum_cnt += rc;
+            }
           }
         }
-        __syncthreads();
-        for (int d = warp; d < nb; d += SEL_NW) {
-          unsigned long long t = 0;
-          for (int c = lane; c < SEL_NT; c += 32) t += s_hist[d * SEL_NT + c];
-          t = warp_sum_u64(t);
-          if (lane == 0) sh.bin[d] = t;
+        const SelShared *own = C > 1 ? cluster.map_shared_rank(&sh, q) : &sh;
+        // lane l takes bins [S - (l+1)*cb, S - l*cb) of the range, top first
+        const int cb = S / 32;
+        unsigned long long lm = 0;
+        int lc = 0;
+        if (C == 1 || !everything) {
+          for (int j = 0; j < cb; ++j) {
+            const int bin = S - 1 - (lane * cb + j);
+            if (C > 1) { lc += (int)own->m_cnt[bin]; lm += own->m_mass[bin]; }
+            else { lc += (int)sh.h_cnt[bin]; lm += ((unsigned long long)sh.h_hi[bin] << SEL_MSPLIT) + sh.h_lo[bin]; }
+          }
         }
-        __syncthreads();
-        int chosen = -1;
-        for (int d = nb - 1; d >= 0; --d) {
-          const unsigned long long t = sh.bin[d];
-          const int c = (int)(t >> 40);
-          const unsigned long long ms = t & ((1ull << 40) - 1);
-          if ((theta != ~0ull && cum_mass + ms >= theta) || cum_cnt + c >= kt) { chosen = d; bin_cnt = c; break; }
-          cum_mass += ms;
-          cum_cnt += c;
+        if (C == 1 && level == 0) {
+          const unsigned long long wtot = warp_sum_u64(lm);
+          if (!all) {
+            theta = (unsigned long long)ceil(__dmul_rn((double)p, (double)wtot));
+            if (theta < 1) theta = 1;
+            if (theta > wtot) theta = ~0ull;
+          }
+          everything = (theta == ~0ull && N <= kt);
         }
-        // chosen >= 0 always: theta <= Wtot guarantees the mass condition fires at the latest in
-        // the lowest digit, and theta == inf implies N > kt so the count condition fires.
-        if (chosen < 0) { chosen = 0; bin_cnt = (int)(sh.bin[0] >> 40); }
-        prefix = (prefix << db) | (uint32_t)chosen;
-        __syncthreads();  // sh.bin / s_hist are rewritten by the next level
+        if (!everything) {
+          // inclusive scan over lanes (lane 0 holds the top bins)
+          unsigned long long im = lm;
+          int ic = lc;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long om = shfl_up_u64(im, o);
+            const int oc = __shfl_up_sync(0xffffffffu, ic, o);
+            if (lane >= o) { im += om; ic += oc; }
+          }
+          const bool cross = (theta != ~0ull && cum_mass + im >= theta) || cum_cnt + ic >= kt;
+          const unsigned cm_ = __ballot_sync(0xffffffffu, cross);
+          // crossing lane: first lane whose inclusive prefix fires (lane 31 if none: cannot happen, see below)
+          const int cl = cm_ ? __ffs(cm_) - 1 : 31;
+          int r_bin = 0, r_bc = 0, r_cc = 0;
+          unsigned long long r_cm = 0;
+          if (lane == cl) {
+            unsigned long long m_ = cum_mass + (im - lm);
+            int c_ = cum_cnt + (ic - lc);
+            int chosen = 0, ccnt = 0;
+            // the crossing fires inside this chunk: theta <= Wtot guarantees the mass condition at the
+            // latest in the lowest non-empty bin, and theta == inf implies N > kt so the count condition
+            // fires; the chunk's last bin is taken unconditionally to keep the walk total.
+            for (int j = 0; j < cb; ++j) {
+              const int bin = S - 1 - (lane * cb + j);
+              unsigned long long ms;
+              int c2;
+              if (C > 1) { c2 = (int)own->m_cnt[bin]; ms = own->m_mass[bin]; }
+              else { c2 = (int)sh.h_cnt[bin]; ms = ((unsigned long long)sh.h_hi[bin] << SEL_MSPLIT) + sh.h_lo[bin]; }
+              chosen = bin; ccnt = c2;
+              if ((theta != ~0ull && m_ + ms >= theta) || c_ + c2 >= kt || j == cb - 1) break;
+              m_ += ms;
+              c_ += c2;
+            }
+            r_bin = q * S + chosen; r_bc = ccnt; r_cc = c_; r_cm = m_;
+          }
+          r_bin = __shfl_sync(0xffffffffu, r_bin, cl);
+          r_bc = __shfl_sync(0xffffffffu, r_bc, cl);
+          r_cc = __shfl_sync(0xffffffffu, r_cc, cl);
+          r_cm = shfl_u64(r_cm, cl);
+          if (lane == 0) {
+            sh.res_bin = r_bin; sh.res_bin_cnt = r_bc; sh.res_cum_cnt = r_cc; sh.res_cum_mass = r_cm;
+          }
+        } else if (lane == 0) {
+          sh.res_bin = -1;
+        }
+        if (lane == 0) sh.res_theta = theta;
       }
+      __syncthreads();
+      theta = sh.res_theta;
+      if (sh.res_bin < 0) { everything = true; break; }
+      prefix = (prefix << db) | (uint32_t)sh.res_bin;
+      bin_cnt = sh.res_bin_cnt;
+      cum_cnt = sh.res_cum_cnt;
+      cum_mass = sh.res_cum_mass;
+      // the next level rewrites sh.h_* (after its own __syncthreads) and sh.res_* (after two more barriers)
+    }
+    if (everything) {
+      k = N;  // tau = 0, all ties taken
+    } else {
       tau = prefix;
       const unsigned long long wt = mass_of_bits(tau);
       long long r = bin_cnt;
@@ -203,23 +435,12 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
   }
 
   // ---------------- 2c: stream compaction in ascending position order -----------------------------
-  uint32_t *s_mask = reinterpret_cast<uint32_t *>(s_hist);  // packed mask staged in shared memory
-  const bool want_mask = P.st.sel_mask != nullptr;
-  const int mask_words = (P.max_ctx + 31) / 32;
-  if (want_mask) {
-    for (int i = tid; i < mask_words; i += SEL_NT) s_mask[i] = 0u;
-  }
-  const int seg = (((N + SEL_NW - 1) / SEL_NW) + 31) & ~31;
-  const int w0 = warp * seg, w1 = min(N, w0 + seg);
+  const int w0 = warp * wseg;  // this warp's contiguous segment of the slice
   {
     int gt = 0, tie = 0;
-    for (int base = w0; base < w1; base += 32) {
-      const int i = base + lane;
-      if (i < w1) {
-        const uint32_t bits = row[i];
-        gt += bits > tau;
-        tie += bits == tau;
-      }
+    for (int i = w0 + lane; i < w0 + wseg; i += 32) {
+      const uint32_t bits = pbits[i];
+      if (bits != SEL_INVALID) { gt += bits > tau; tie += bits == tau; }
     }
     gt = __reduce_add_sync(0xffffffffu, gt);
     tie = __reduce_add_sync(0xffffffffu, tie);
@@ -227,6 +448,23 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
   }
   __syncthreads();
   int tie_before = 0, sel_before = 0;
+  if (C > 1) {
+    if (tid < C) {
+      int g_ = 0, t_ = 0;
+      for (int w = 0; w < SEL_NW; ++w) { g_ += sh.w_gt[w]; t_ += sh.w_tie[w]; }
+      SelShared *dst = cluster.map_shared_rank(&sh, tid);
+      dst->c_gt[rank] = g_;
+      dst->c_tie[rank] = t_;
+    }
+    cluster.sync();
+    for (int c = 0; c < rank; ++c) {
+      const int tw = sh.c_tie[c];
+      int take = r_ties - tie_before;
+      take = take < 0 ? 0 : (take > tw ? tw : take);
+      sel_before += sh.c_gt[c] + take;
+      tie_before += tw;
+    }
+  }
   for (int w = 0; w < warp; ++w) {
     const int tw = sh.w_tie[w];
     int take = r_ties - tie_before;
@@ -236,36 +474,41 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
   }
   int32_t *votes = P.st.votes + (size_t)unit * P.max_ctx;
   const unsigned lt = (1u << lane) - 1u;
-  for (int base = w0; base < w1; base += 32) {
-    const int i = base + lane;
-    const bool valid = i < w1;
-    const uint32_t bits = valid ? row[i] : 0u;
+  for (int i0 = w0; i0 < w0 + wseg; i0 += 32) {
+    const int pos0 = s0 + i0;               // multiple of 32: one aligned word of the packed mask
+    if (pos0 >= hi) break;                  // warp-uniform
+    const uint32_t bits = pbits[i0 + lane];
+    const bool valid = bits != SEL_INVALID;
     const bool g = valid && bits > tau;
     const bool t = valid && bits == tau;
     const unsigned tb = __ballot_sync(0xffffffffu, t);
     const bool s = g || (t && (tie_before + __popc(tb & lt)) < r_ties);
     const unsigned sb = __ballot_sync(0xffffffffu, s);
     if (s) {
-      const int pos = lo + i;
+      const int pos = pos0 + lane;
       sel_idx[sel_before + __popc(sb & lt)] = pos;
       votes[pos] += 1;  // cumulative selection mask = votes (L86)
-      if (want_mask) atomicOr(&s_mask[pos >> 5], 1u << (pos & 31));
+    }
+    if (want_mask && lane < 4) {  // bit i%8 of byte i/8 (L439): byte y of the word holds bits 8y..8y+7
+      const int y = (pos0 >> 3) + lane;
+      if (y < mask_bytes) mask[y] = (uint8_t)(sb >> (8 * lane));
     }
     tie_before += __popc(tb);
     sel_before += __popc(sb);
   }
-  // pads and the head-wise block table (reading C9; L207-209)
-  for (int j = k + tid; j < P.k_cap; j += SEL_NT) sel_idx[j] = -1;
+  // pads, the head-wise block table (reading C9; L207-209) and the mask bytes outside the slices
+  const int gt_ = rank * SEL_NT + tid, gs_ = C * SEL_NT;
+  for (int j = k + gt_; j < P.k_cap; j += gs_) sel_idx[j] = -1;
   const int used = (k + PAGE - 1) / PAGE;
   const int32_t *sp = P.st.sel_pages + (size_t)unit * P.spu;
-  for (int j = tid; j < P.spu; j += SEL_NT) sel_table[j] = j < used ? sp[j] : -1;
-  if (tid == 0) P.st.sel_count[unit] = k;
+  for (int j = gt_; j < P.spu; j += gs_) sel_table[j] = j < used ? sp[j] : -1;
+  if (rank == 0 && tid == 0) P.st.sel_count[unit] = k;
   if (want_mask) {
-    __syncthreads();
-    uint8_t *mk = P.st.sel_mask + (size_t)unit * (P.max_ctx / 8);
-    const uint8_t *sb = reinterpret_cast<const uint8_t *>(s_mask);  // little endian: byte y holds bits 8y..8y+7
-    for (int y = tid; y < P.max_ctx / 8; y += SEL_NT) mk[y] = sb[y];
+    const int y0 = base >> 3, y1 = min(mask_bytes, ((hi + 31) & ~31) >> 3);
+    for (int y = gt_; y < y0; y += gs_) mask[y] = 0;
+    for (int y = y1 + gt_; y < mask_bytes; y += gs_) mask[y] = 0;
   }
+  if (C > 1) cluster.sync();  // no CTA may exit while a peer can still read its shared memory
 }
 
 }  // namespace hardkv
