@@ -19,6 +19,8 @@ struct Params {
   // workspace
   float *part;          // [units][att_chunks][G][d + 2] split-K partial states (m, l, acc[d])
   int32_t *att_arrive;  // [units] arrival counters of the split-K merge (zero between launches)
+  float2 *score_stats;   // [units][score_chunks][8] per (chunk, query head): (max, sum of 2^(x - max)) of x = z*log2(e)/T
+  int score_chunks;
   int sel_cluster;       // CTAs per (b, h) cluster of the select kernel
   int sel_slice_cap;     // capacity (tokens) of one CTA's probability slice in shared memory
 };
@@ -67,6 +69,23 @@ __device__ __forceinline__ void pool_bounds(const Params &P, int b, int &n, int 
   hi = n - P.recent;
   if (hi < lo) hi = lo;
 }
+
+__device__ __forceinline__ float fast_exp2(float x) {   // MUFU.EX2; 2^-inf = +0
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+__device__ __forceinline__ float warp_max_f32(float v) {
+#pragma unroll
+  for (int o = 16; o; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  return v;
+}
+__device__ __forceinline__ float warp_sum_f32(float v) {
+#pragma unroll
+  for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+constexpr int SCORE_PAGES_PER_CTA = 32;  // score kernel: 8 warps x 4 pages = 512 tokens = 128 KiB of K per CTA
 
 __device__ __forceinline__ unsigned long long shfl_xor_u64(unsigned long long v, int off) {
   unsigned lo = __shfl_xor_sync(0xffffffffu, (unsigned)v, off);

@@ -5,6 +5,7 @@
 #include <string.h>
 
 #include "common.cuh"
+#include "fast_kernels.cuh"
 #include "select_kernel.cuh"
 #include "stage_kernels.cuh"
 
@@ -24,12 +25,16 @@ namespace {
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout { size_t part, arrive, stage_q, stage_k, stage_v, stage_out, total; };
+struct WsLayout { size_t part, arrive, stats, stage_q, stage_k, stage_v, stage_out, total; };
 
 size_t esize_of(const hardkv_config &c) { return c.kv_dtype == HARDKV_F32 ? 4 : 2; }
 
 int att_chunks_of(const hardkv_config &c) {
   return (c.sink + c.recent + c.k_cap + c.cond_cap + ATT_CHUNK - 1) / ATT_CHUNK;
+}
+
+int score_chunks_of(const hardkv_config &c) {
+  return (c.max_ctx / PAGE + SCORE_PAGES_PER_CTA - 1) / SCORE_PAGES_PER_CTA;
 }
 
 WsLayout ws_layout(const hardkv_config &c) {
@@ -39,6 +44,7 @@ WsLayout ws_layout(const hardkv_config &c) {
   size_t off = 0;
   w.arrive = off; off += align256(units * sizeof(int32_t));
   w.part = off;   off += align256(units * att_chunks_of(c) * G * (c.head_dim + 2) * sizeof(float));
+  w.stats = off;  off += align256(units * score_chunks_of(c) * 8 * sizeof(float2));
   const size_t qb = (size_t)c.batch * c.num_q_heads * c.head_dim, kb = units * c.head_dim;
   w.stage_q = off;   off += align256(qb * esize_of(c));
   w.stage_k = off;   off += align256(kb * esize_of(c));
@@ -116,6 +122,9 @@ Params params_of(const hardkv_ctx *ctx, const hardkv_state *s) {
     }                                                                                              \
   } while (0)
 
+// bf16 tensor-core paths (variant 1); fp32 K/V and variant 0 run the generic FMA kernels
+bool fast_path(const hardkv_ctx *ctx) { return ctx->variant == 1 && ctx->cfg.kv_dtype == HARDKV_BF16; }
+
 void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, cudaStream_t st) {
   ctx->launches += 1;
   HK_DISPATCH_TD(ctx->cfg, (append_retire_kernel<T, D><<<P.B, 256, 0, st>>>(P, k_new, v_new)));
@@ -123,11 +132,18 @@ void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const vo
 
 void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
   ctx->launches += 1;
-  dim3 grid((P.ppu + SCORE_PAGES_PER_CTA - 1) / SCORE_PAGES_PER_CTA, P.B * P.Hkv);
+  dim3 grid(P.score_chunks, P.B * P.Hkv);
+  if (fast_path(ctx)) {
+    if (P.d == 128) score_mma_kernel<128><<<grid, 256, 0, st>>>(P, q);
+    else score_mma_kernel<64><<<grid, 256, 0, st>>>(P, q);
+    return;
+  }
   HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (score_generic_kernel<T, D, G><<<grid, 256, 0, st>>>(P, q))));
 }
 
-void launch_select(hardkv_ctx *ctx, const Params &P, float p, bool calibrate, cudaStream_t st) {
+// calibrate: 0 = select on probs as given, 1 = logits -> probs with in-kernel statistics,
+// 2 = logits -> probs with the chunk statistics the bf16 score kernel left in the workspace
+void launch_select(hardkv_ctx *ctx, const Params &P, float p, int calibrate, cudaStream_t st) {
   ctx->launches += 1;
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3(P.B * P.Hkv * P.sel_cluster);
@@ -139,7 +155,8 @@ void launch_select(hardkv_ctx *ctx, const Params &P, float p, bool calibrate, cu
   at[0].val.clusterDim.x = P.sel_cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   lc.attrs = at;
   lc.numAttrs = 1;
-  if (calibrate) cudaLaunchKernelEx(&lc, select_kernel<1>, P, p);
+  if (calibrate == 2) cudaLaunchKernelEx(&lc, select_kernel<2>, P, p);
+  else if (calibrate == 1) cudaLaunchKernelEx(&lc, select_kernel<1>, P, p);
   else cudaLaunchKernelEx(&lc, select_kernel<0>, P, p);
 }
 
@@ -205,6 +222,8 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   char *base = reinterpret_cast<char *>(workspace);
   P.att_arrive = reinterpret_cast<int32_t *>(base + w.arrive);
   P.part = reinterpret_cast<float *>(base + w.part);
+  P.score_stats = reinterpret_cast<float2 *>(base + w.stats);
+  P.score_chunks = score_chunks_of(*cfg);
   ctx->stage_q = base + w.stage_q; ctx->stage_k = base + w.stage_k; ctx->stage_v = base + w.stage_v;
   ctx->stage_out = reinterpret_cast<float *>(base + w.stage_out);
   select_geometry(*cfg, &P.sel_cluster, &P.sel_slice_cap);
@@ -213,7 +232,8 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   static size_t sel_smem_max = 0;
   if (select_smem_bytes(P) > sel_smem_max) sel_smem_max = select_smem_bytes(P);
   if (cudaFuncSetAttribute(select_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess ||
-      cudaFuncSetAttribute(select_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess) {
+      cudaFuncSetAttribute(select_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess ||
+      cudaFuncSetAttribute(select_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess) {
     cudaGetLastError();
     delete ctx;
     return HARDKV_ERR_CUDA;
@@ -251,13 +271,13 @@ static bool accum_ok(const hardkv_ctx *ctx, const hardkv_state *s) {
 
 hardkv_status hardkv_calibrate_topp(hardkv_ctx *ctx, const hardkv_state *s, float p, hardkv_stream st) {
   if (!state_ok(ctx, s) || !(p > 0.f) || !accum_ok(ctx, s)) return HARDKV_ERR_INVALID_ARG;
-  launch_select(ctx, params_of(ctx, s), p, true, st);
+  launch_select(ctx, params_of(ctx, s), p, 1, st);
   return launch_status();
 }
 
 hardkv_status hardkv_topp_select(hardkv_ctx *ctx, const hardkv_state *s, float p, hardkv_stream st) {
   if (!state_ok(ctx, s) || !(p > 0.f)) return HARDKV_ERR_INVALID_ARG;
-  launch_select(ctx, params_of(ctx, s), p, false, st);
+  launch_select(ctx, params_of(ctx, s), p, 0, st);
   return launch_status();
 }
 
@@ -292,7 +312,7 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   launch_append(ctx, P, k_new, v_new, st);
   if (do_select) {
     launch_score(ctx, P, q, st);
-    launch_select(ctx, P, p, true, st);
+    launch_select(ctx, P, p, fast_path(ctx) ? 2 : 1, st);
   }
   launch_attend(ctx, P, q, out, lse, do_select != 0, st);
   return launch_status();

@@ -111,68 +111,87 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
 
   // ---------------- 2a: calibration ------------------------------------------------------------
   if (CALIBRATE) {
-    const float invT = 1.0f / P.st.temperature[unit];
+    // softmax in the base-2 domain: exp(z/T - m) = 2^(z*c2 - m2), c2 = log2(e)/T (one FFMA + one MUFU.EX2)
+    const float c2 = 1.4426950408889634f / P.st.temperature[unit];
     const float *lg = P.st.logits + ((size_t)(b * P.Hq + h * G)) * P.max_ctx;
-    // per query head: max and sum of exp over the pool (softmax over the pool only, reading C3)
-#pragma unroll
-    for (int g = 0; g < 8; ++g) {
-      if (g >= G) break;
-      const float *row = lg + (size_t)g * P.max_ctx;
-      float m = -INFINITY, s = 0.f;
-      for (int i0 = tid; i0 < per; i0 += 4 * SEL_NT) {
-        float x[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int pos = s0 + i0 + u * SEL_NT;
-          x[u] = (i0 + u * SEL_NT < per && pos >= lo && pos < hi) ? __ldcg(row + pos) * invT : -INFINITY;
-        }
-        const float mn = fmaxf(fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3])), m);
-        if (mn != -INFINITY) {
-          s = s * expf(m - mn) + expf(x[0] - mn) + expf(x[1] - mn) + expf(x[2] - mn) + expf(x[3] - mn);
-          m = mn;
-        }
-      }
-#pragma unroll
-      for (int o = 16; o; o >>= 1) {
-        const float om = __shfl_xor_sync(0xffffffffu, m, o), os = __shfl_xor_sync(0xffffffffu, s, o);
-        const float mn = fmaxf(m, om);
-        s = (m == -INFINITY ? 0.f : s * expf(m - mn)) + (om == -INFINITY ? 0.f : os * expf(om - mn));
-        m = mn;
-      }
-      if (lane == 0) { sh.red_f[warp][g][0] = m; sh.red_f[warp][g][1] = s; }
-    }
-    __syncthreads();
-    if (C > 1) cluster.barrier_wait();
-    if (tid < C * 8) {  // thread (c, g): publish this CTA's (m_g, s_g) into CTA c
-      const int c = tid >> 3, g = tid & 7;
-      float m = -INFINITY, s = 0.f;
-      if (g < G) {
-        for (int w = 0; w < SEL_NW; ++w) m = fmaxf(m, sh.red_f[w][g][0]);
-        for (int w = 0; w < SEL_NW; ++w) {
-          const float mw = sh.red_f[w][g][0];
-          if (mw != -INFINITY) s += sh.red_f[w][g][1] * expf(mw - m);
-        }
-      }
-      SelShared *dst = cluster.map_shared_rank(&sh, c);
-      dst->st_m[rank][g] = m;
-      dst->st_s[rank][g] = s;
-    }
-    cluster.sync();
     float mg[8], rs[8];
+    if (CALIBRATE == 2) {
+      // statistics were produced by the score kernel: one (m2, s) pair per query head and 512-token chunk
+      if (C > 1) cluster.barrier_wait();
+      const int ch0 = (lo >> 4) / SCORE_PAGES_PER_CTA, ch1 = ((hi - 1) >> 4) / SCORE_PAGES_PER_CTA;
+      const float2 *sp = P.score_stats + ((size_t)unit * P.score_chunks) * 8;
 #pragma unroll
-    for (int g = 0; g < 8; ++g) {
-      float m = -INFINITY, s = 0.f;
-      if (g < G) {
-        for (int c = 0; c < C; ++c) m = fmaxf(m, sh.st_m[c][g]);
-        for (int c = 0; c < C; ++c) {
-          const float mc = sh.st_m[c][g];
-          if (mc != -INFINITY) s += sh.st_s[c][g] * expf(mc - m);
+      for (int g = 0; g < 8; ++g) {
+        float m = -INFINITY, sacc = 0.f;
+        if (g < G) {
+          for (int c = ch0 + lane; c <= ch1; c += 32) m = fmaxf(m, __ldcg(&sp[(size_t)c * 8 + g]).x);
+          m = warp_max_f32(m);
+          for (int c = ch0 + lane; c <= ch1; c += 32) {
+            const float2 v = __ldcg(&sp[(size_t)c * 8 + g]);
+            sacc += v.y * fast_exp2(v.x - m);
+          }
+          sacc = warp_sum_f32(sacc);
         }
+        mg[g] = m;
+        rs[g] = 1.0f / (sacc * (float)G);
       }
-      mg[g] = m;
-      rs[g] = 1.0f / s;
+      __syncthreads();  // histogram zeroed
+    } else {
+      // per query head: max and sum of exp over the pool (softmax over the pool only, reading C3)
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+        if (g >= G) break;
+        const float *row = lg + (size_t)g * P.max_ctx;
+        float m = -INFINITY, sacc = 0.f;
+        for (int i0 = tid; i0 < per; i0 += 4 * SEL_NT) {
+          float x[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int pos = s0 + i0 + u * SEL_NT;
+            x[u] = (i0 + u * SEL_NT < per && pos >= lo && pos < hi) ? __ldcg(row + pos) * c2 : -INFINITY;
+          }
+          const float mn = fmaxf(fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3])), m);
+          if (mn != -INFINITY) {
+            sacc = sacc * fast_exp2(m - mn) + fast_exp2(x[0] - mn) + fast_exp2(x[1] - mn) + fast_exp2(x[2] - mn) +
+                   fast_exp2(x[3] - mn);
+            m = mn;
+          }
+        }
+        const float mw = warp_max_f32(m);
+        sacc = warp_sum_f32(mw == -INFINITY ? 0.f : sacc * fast_exp2(m - mw));
+        if (lane == 0) { sh.red_f[warp][g][0] = mw; sh.red_f[warp][g][1] = sacc; }
+      }
+      __syncthreads();
+      if (C > 1) cluster.barrier_wait();
+      if (tid < C * 8) {  // thread (c, g): publish this CTA's (m_g, s_g) into CTA c
+        const int c = tid >> 3, g = tid & 7;
+        float m = -INFINITY, sacc = 0.f;
+        if (g < G) {
+          for (int w = 0; w < SEL_NW; ++w) m = fmaxf(m, sh.red_f[w][g][0]);
+          for (int w = 0; w < SEL_NW; ++w) {
+            const float mw = sh.red_f[w][g][0];
+            if (mw != -INFINITY) sacc += sh.red_f[w][g][1] * fast_exp2(mw - m);
+          }
+        }
+        SelShared *dst = cluster.map_shared_rank(&sh, c);
+        dst->st_m[rank][g] = m;
+        dst->st_s[rank][g] = sacc;
+      }
+      cluster.sync();
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+        float m = -INFINITY, sacc = 0.f;
+        if (g < G) {
+          for (int c = 0; c < C; ++c) m = fmaxf(m, sh.st_m[c][g]);
+          for (int c = 0; c < C; ++c) {
+            const float mc = sh.st_m[c][g];
+            if (mc != -INFINITY) sacc += sh.st_s[c][g] * fast_exp2(mc - m);
+          }
+        }
+        mg[g] = m;
+        rs[g] = 1.0f / (sacc * (float)G);   // the group mean (reading C2) is folded into the normaliser
+      }
     }
-    const float invG = 1.0f / (float)G;
     const bool accum = P.st.score_mode[h] == HARDKV_SCORE_ACCUM;
     if (!accum) {
       // S_hat = softmax(z / T) per query head (Solution 1, L120), group mean (reading C2)
@@ -183,8 +202,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
           float pr = 0.f;
 #pragma unroll
           for (int g = 0; g < 8; ++g)
-            if (g < G) pr += expf(__ldcg(lg + (size_t)g * P.max_ctx + pos) * invT - mg[g]) * rs[g];
-          pr *= invG;
+            if (g < G) pr = fmaf(fast_exp2(fmaf(__ldcg(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
           probs[pos] = pr;
           bits = __float_as_uint(pr);
           hist_add(sh, bits >> 20, bits);
@@ -204,8 +222,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
           float pr = 0.f;
 #pragma unroll
           for (int g = 0; g < 8; ++g)
-            if (g < G) pr += expf(__ldcg(lg + (size_t)g * P.max_ctx + pos) * invT - mg[g]) * rs[g];
-          pr *= invG;
+            if (g < G) pr = fmaf(fast_exp2(fmaf(__ldcg(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
           float a = (acc[pos] - ring[pos]) + pr;
           a = fmaxf(a, 0.f);
           acc[pos] = a;

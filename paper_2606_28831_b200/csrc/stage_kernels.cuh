@@ -98,7 +98,6 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
 // A warp streams one 16-row page per iteration: each load instruction covers 512 contiguous
 // bytes (32 lanes x 16 B); the LPR lanes that share a row reduce with xor-shuffles.
 // =============================================================================================
-constexpr int SCORE_PAGES_PER_CTA = 32;  // 8 warps x 4 pages = 512 tokens = 128 KiB of K
 
 template <typename T, int D, int G>
 __global__ void __launch_bounds__(256) score_generic_kernel(Params P, const void *q_) {
