@@ -8,6 +8,7 @@
 #include "fast_kernels.cuh"
 #include "select_kernel.cuh"
 #include "stage_kernels.cuh"
+#include "attend_mma.cuh"
 
 using namespace hardkv;
 
@@ -169,6 +170,17 @@ void launch_rewrite(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
 void launch_attend(hardkv_ctx *ctx, const Params &P, const void *q, float *out, float *lse, bool fused,
                    cudaStream_t st) {
   ctx->launches += 1;
+  if (fast_path(ctx)) {
+    dim3 gm((P.att_chunks * ATT_CHUNK + ATT_MMA_CHUNK - 1) / ATT_MMA_CHUNK, P.B * P.Hkv);
+    if (P.d == 128) {
+      if (fused) attend_mma_kernel<128, true><<<gm, 256, 0, st>>>(P, q, out, lse);
+      else attend_mma_kernel<128, false><<<gm, 256, 0, st>>>(P, q, out, lse);
+    } else {
+      if (fused) attend_mma_kernel<64, true><<<gm, 256, 0, st>>>(P, q, out, lse);
+      else attend_mma_kernel<64, false><<<gm, 256, 0, st>>>(P, q, out, lse);
+    }
+    return;
+  }
   dim3 grid(P.att_chunks, P.B * P.Hkv);
   if (fused)
     HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, true><<<grid, 256, 0, st>>>(P, q, out, lse))));
