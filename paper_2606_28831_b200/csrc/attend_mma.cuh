@@ -37,7 +37,6 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   constexpr int NKC = D / 32;   // 64-byte chunks of a key row
   constexpr int NVC = D / 64;   // 128-byte chunks of a value row
   constexpr int ROWB = D * 2;
-  constexpr int TILES = ATT_MMA_CHUNK / 16;
   const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
   const int n = P.st.ctx_len[b];
   const int s_end = min(P.sink, n);
@@ -77,45 +76,46 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   for (int i = 0; i < NVC * 4; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
 
   const int v0 = c * ATT_MMA_CHUNK, v1 = min(total, v0 + ATT_MMA_CHUNK);
-#pragma unroll 1
-  for (int ti = warp; ti < TILES; ti += 8) {
-    const int vbase = v0 + ti * 16;
-    if (vbase >= v1) break;
-    // ---- lanes 0..15 resolve the source (tier << 30 | row) and rewrite destination of one row each ----
-    uint32_t src = ROW_INVALID, dst = ROW_INVALID;
-    if (lane < 16) {
-      const int v = vbase + lane;
-      if (v < n_dense) {                      // Tier 1: sinks + recent window, read in place
-        const int pos = v < s_end ? v : r_lo + (v - s_end);
+  // ---- every lane resolves the source (tier << 30 | row) and rewrite destination of one of the warp's 32 rows ----
+  uint32_t src = ROW_INVALID, dst = ROW_INVALID;
+  {
+    const int v = v0 + warp * 32 + lane;
+    if (v < n_dense) {                      // Tier 1: sinks + recent window, read in place
+      const int pos = v < s_end ? v : r_lo + (v - s_end);
+      src = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
+    } else if (v < n_dense + k) {           // Tier 2: selected rows
+      const int j = v - n_dense;
+      const uint32_t srow = (uint32_t)(__ldg(stab + (j >> 4)) * PAGE + (j & 15));
+      if (FUSED) {
+        const int pos = __ldg(idx + j);
         src = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
-      } else if (v < n_dense + k) {           // Tier 2: selected rows
-        const int j = v - n_dense;
-        const uint32_t srow = (uint32_t)(__ldg(stab + (j >> 4)) * PAGE + (j & 15));
-        if (FUSED) {
-          const int pos = __ldg(idx + j);
-          src = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
-          dst = srow;
-        } else {
-          src = (1u << 30) | srow;
-        }
-      } else if (v < total) {                 // Tier 3: condensed residents
-        src = (2u << 30) | (uint32_t)(unit * P.cond_cap + (v - n_dense - k));
+        dst = srow;
+      } else {
+        src = (1u << 30) | srow;
       }
+    } else if (v < total) {                 // Tier 3: condensed residents
+      src = (2u << 30) | (uint32_t)(unit * P.cond_cap + (v - n_dense - k));
     }
+  }
+#pragma unroll 1
+  for (int it = 0; it < 2; ++it) {
+    const int vbase = v0 + warp * 32 + it * 16;
+    if (vbase >= v1) break;
+    const int lb = it * 16;
     uint32_t ks[2], vs[4], kd[2], vd[4];
-    ks[0] = __shfl_sync(0xffffffffu, src, gid);
-    ks[1] = __shfl_sync(0xffffffffu, src, gid + 8);
-    vs[0] = __shfl_sync(0xffffffffu, src, 2 * tig);
-    vs[1] = __shfl_sync(0xffffffffu, src, 2 * tig + 1);
-    vs[2] = __shfl_sync(0xffffffffu, src, 2 * tig + 8);
-    vs[3] = __shfl_sync(0xffffffffu, src, 2 * tig + 9);
+    ks[0] = __shfl_sync(0xffffffffu, src, lb + gid);
+    ks[1] = __shfl_sync(0xffffffffu, src, lb + gid + 8);
+    vs[0] = __shfl_sync(0xffffffffu, src, lb + 2 * tig);
+    vs[1] = __shfl_sync(0xffffffffu, src, lb + 2 * tig + 1);
+    vs[2] = __shfl_sync(0xffffffffu, src, lb + 2 * tig + 8);
+    vs[3] = __shfl_sync(0xffffffffu, src, lb + 2 * tig + 9);
     if (FUSED) {
-      kd[0] = __shfl_sync(0xffffffffu, dst, gid);
-      kd[1] = __shfl_sync(0xffffffffu, dst, gid + 8);
-      vd[0] = __shfl_sync(0xffffffffu, dst, 2 * tig);
-      vd[1] = __shfl_sync(0xffffffffu, dst, 2 * tig + 1);
-      vd[2] = __shfl_sync(0xffffffffu, dst, 2 * tig + 8);
-      vd[3] = __shfl_sync(0xffffffffu, dst, 2 * tig + 9);
+      kd[0] = __shfl_sync(0xffffffffu, dst, lb + gid);
+      kd[1] = __shfl_sync(0xffffffffu, dst, lb + gid + 8);
+      vd[0] = __shfl_sync(0xffffffffu, dst, lb + 2 * tig);
+      vd[1] = __shfl_sync(0xffffffffu, dst, lb + 2 * tig + 1);
+      vd[2] = __shfl_sync(0xffffffffu, dst, lb + 2 * tig + 8);
+      vd[3] = __shfl_sync(0xffffffffu, dst, lb + 2 * tig + 9);
     }
     // ---- loads: 16 x 16 B per lane = the 16 key rows and 16 value rows of the tile ----
     uint4 kr[2][NKC], vr[4][NVC];
@@ -257,7 +257,8 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
     part[g * (D + 2) + 2 + e] = A;
     if (e == 0) { part[g * (D + 2)] = M; part[g * (D + 2) + 1] = L; }
   }
-  // ---- last CTA of the unit merges all partials ----
+  // ---- the last CTA of the unit to arrive merges all chunk partials (Eq. 6): its 8 warps take
+  //      chunks w, w + 8, ... in parallel (lanes over d), then combine through shared memory ----
   __threadfence();
   __syncthreads();
   if (tid == 0) {
@@ -267,18 +268,57 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  const float *pu = P.part + (size_t)unit * P.att_chunks * G * (D + 2);
+  {
+    float mm[8], ll[8], aa[8][D / 32];
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      mm[g] = -INFINITY; ll[g] = 0.f;
+#pragma unroll
+      for (int i = 0; i < D / 32; ++i) aa[g][i] = 0.f;
+    }
+    const float *pu = P.part + (size_t)unit * P.att_chunks * G * (D + 2);
+    for (int ch = warp; ch < nchunks; ch += 8) {
+      const float *pc = pu + (size_t)ch * G * (D + 2);
+#pragma unroll
+      for (int g = 0; g < 8; ++g) {
+        if (g < G) {
+          const float *pp = pc + g * (D + 2);
+          const float mw = __ldcg(pp), lw = __ldcg(pp + 1);
+          float v[D / 32];
+#pragma unroll
+          for (int i = 0; i < D / 32; ++i) v[i] = __ldcg(pp + 2 + lane + 32 * i);
+          const float mn = fmaxf(mm[g], mw);
+          const float ca = (mm[g] == -INFINITY) ? 0.f : fast_exp2(mm[g] - mn);
+          const float cb = (mw == -INFINITY) ? 0.f : fast_exp2(mw - mn);
+          ll[g] = ll[g] * ca + lw * cb;
+#pragma unroll
+          for (int i = 0; i < D / 32; ++i) aa[g][i] = aa[g][i] * ca + v[i] * cb;
+          mm[g] = mn;
+        }
+      }
+    }
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {
+      if (g < G) {
+        if (lane == 0) { s_st[warp][g][0] = mm[g]; s_st[warp][g][1] = ll[g]; }
+#pragma unroll
+        for (int i = 0; i < D / 32; ++i) s_st[warp][g][2 + lane + 32 * i] = aa[g][i];
+      }
+    }
+  }
+  __syncthreads();
   for (int it = tid; it < G * D; it += 256) {
     const int g = it / D, e = it % D;
     float M = -INFINITY;
-    for (int ch = 0; ch < nchunks; ++ch) M = fmaxf(M, __ldcg(pu + ((size_t)ch * G + g) * (D + 2)));
+#pragma unroll
+    for (int w = 0; w < 8; ++w) M = fmaxf(M, s_st[w][g][0]);
     float L = 0.f, A = 0.f;
-    for (int ch = 0; ch < nchunks; ++ch) {
-      const float *pp = pu + ((size_t)ch * G + g) * (D + 2);
-      const float mw = __ldcg(pp);
+#pragma unroll
+    for (int w = 0; w < 8; ++w) {
+      const float mw = s_st[w][g][0];
       const float cw = (mw == -INFINITY) ? 0.f : fast_exp2(mw - M);
-      L += __ldcg(pp + 1) * cw;
-      A += __ldcg(pp + 2 + e) * cw;
+      L += s_st[w][g][1] * cw;
+      A += s_st[w][g][2 + e] * cw;
     }
     out[((size_t)(b * P.Hq + h * G + g)) * D + e] = A / L;
     if (e == 0 && lse) lse[b * P.Hq + h * G + g] = (M + log2f(L)) * 0.6931471805599453f;
