@@ -2,6 +2,7 @@
 // (kv_dtype, head_dim, G), stream-ordered launches only.  No allocation, no synchronisation.
 #include <math.h>
 #include <new>
+#include <stdlib.h>
 #include <string.h>
 
 #include "common.cuh"
@@ -57,16 +58,31 @@ WsLayout ws_layout(const hardkv_config &c) {
 
 size_t select_smem_bytes(const Params &P) { return (size_t)P.sel_slice_cap * 4 + sizeof(SelShared); }
 
-// Cluster size of the select kernel: enough CTAs per (b, h) to keep a slice near 8.5k tokens and
-// to spread few units over the chip (one wave of 512-thread CTAs is about 4 x 148).
+// Cluster size of the select kernel.  The kernel is latency bound (barriers, DSMEM merges, a few
+// dependent memory round trips), so the cost of a geometry is modelled as
+//   waves x (fixed + tokens per thread [+ cluster overhead]),
+// with waves from the CTAs that fit on 148 SMs given the shared memory of one slice.  The cheapest
+// of C = 1, 2, 4, 8 wins; a slice must fit one SM.
 void select_geometry(const hardkv_config &c, int *cluster, int *slice_cap) {
   const int units = c.batch * c.num_kv_heads;
   const int max_pool = c.max_ctx - c.recent > 0 ? c.max_ctx - c.recent : 1;
-  int cmin = 1, cpar = 1;
-  while (cmin < SEL_MAXC && (max_pool + cmin - 1) / cmin > 8704) cmin <<= 1;
-  while (cpar * 2 <= SEL_MAXC && cpar * 2 * units <= 592) cpar <<= 1;
-  *cluster = cmin > cpar ? cmin : cpar;
-  *slice_cap = sel_slice_len(max_pool, *cluster);
+  const char *force = getenv("HARDKV_SELECT_CLUSTER");   // A/B measurements only
+  const int forced = force ? atoi(force) : 0;
+  double best = 1e30;
+  *cluster = 0;
+  for (int C = 1; C <= SEL_MAXC; C <<= 1) {
+    const int cap = sel_slice_len(max_pool + 31, C);
+    const size_t smem = (size_t)cap * 4 + sizeof(SelShared);
+    if (smem > 227u * 1024u) continue;
+    int cps = (int)((228u * 1024u) / (smem + 1024u));
+    if (cps > 2048 / SEL_NT) cps = 2048 / SEL_NT;
+    const int slots = 148 * cps;
+    const int waves = (units * C + slots - 1) / slots;
+    double cost = waves * (20.0 + (double)cap / SEL_NT + (C > 1 ? 3.0 : 0.0));
+    if (forced == C) cost = -1.0;
+    if (cost < best) { best = cost; *cluster = C; *slice_cap = cap; }
+  }
+  if (*cluster == 0) { *cluster = SEL_MAXC; *slice_cap = sel_slice_len(max_pool + 31, SEL_MAXC); }
 }
 
 hardkv_status check_config(const hardkv_config *c) {

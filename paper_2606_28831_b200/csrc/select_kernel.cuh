@@ -120,22 +120,24 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
       if (C > 1) cluster.barrier_wait();
       const int ch0 = (lo >> 4) / SCORE_PAGES_PER_CTA, ch1 = ((hi - 1) >> 4) / SCORE_PAGES_PER_CTA;
       const float2 *sp = P.score_stats + ((size_t)unit * P.score_chunks) * 8;
+      if (warp < G) {   // warp g reduces the chunk statistics of query head g (lanes over chunks)
+        const int g = warp;
+        float m = -INFINITY, sacc = 0.f;
+        for (int c = ch0 + lane; c <= ch1; c += 32) m = fmaxf(m, __ldg(&sp[(size_t)c * 8 + g]).x);
+        m = warp_max_f32(m);
+        for (int c = ch0 + lane; c <= ch1; c += 32) {
+          const float2 v = __ldg(&sp[(size_t)c * 8 + g]);
+          sacc += v.y * fast_exp2(v.x - m);
+        }
+        sacc = warp_sum_f32(sacc);
+        if (lane == 0) { sh.st_m[0][g] = m; sh.st_s[0][g] = 1.0f / (sacc * (float)G); }
+      }
+      __syncthreads();  // statistics published, histogram zeroed
 #pragma unroll
       for (int g = 0; g < 8; ++g) {
-        float m = -INFINITY, sacc = 0.f;
-        if (g < G) {
-          for (int c = ch0 + lane; c <= ch1; c += 32) m = fmaxf(m, __ldcg(&sp[(size_t)c * 8 + g]).x);
-          m = warp_max_f32(m);
-          for (int c = ch0 + lane; c <= ch1; c += 32) {
-            const float2 v = __ldcg(&sp[(size_t)c * 8 + g]);
-            sacc += v.y * fast_exp2(v.x - m);
-          }
-          sacc = warp_sum_f32(sacc);
-        }
-        mg[g] = m;
-        rs[g] = 1.0f / (sacc * (float)G);
+        mg[g] = g < G ? sh.st_m[0][g] : -INFINITY;
+        rs[g] = g < G ? sh.st_s[0][g] : 0.f;
       }
-      __syncthreads();  // histogram zeroed
     } else {
       // per query head: max and sum of exp over the pool (softmax over the pool only, reading C3)
 #pragma unroll
@@ -148,7 +150,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int pos = s0 + i0 + u * SEL_NT;
-            x[u] = (i0 + u * SEL_NT < per && pos >= lo && pos < hi) ? __ldcg(row + pos) * c2 : -INFINITY;
+            x[u] = (i0 + u * SEL_NT < per && pos >= lo && pos < hi) ? __ldg(row + pos) * c2 : -INFINITY;
           }
           const float mn = fmaxf(fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3])), m);
           if (mn != -INFINITY) {
@@ -195,19 +197,33 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
     const bool accum = P.st.score_mode[h] == HARDKV_SCORE_ACCUM;
     if (!accum) {
       // S_hat = softmax(z / T) per query head (Solution 1, L120), group mean (reading C2)
-      for (int i = tid; i < per; i += SEL_NT) {
-        const int pos = s0 + i;
-        uint32_t bits = SEL_INVALID;
-        if (pos >= lo && pos < hi) {
-          float pr = 0.f;
+      constexpr int UB = 4;
+      for (int i0 = tid; i0 < per; i0 += UB * SEL_NT) {
+        float x[UB][8];
+        bool ok[UB];
 #pragma unroll
-          for (int g = 0; g < 8; ++g)
-            if (g < G) pr = fmaf(fast_exp2(fmaf(__ldcg(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
-          probs[pos] = pr;
-          bits = __float_as_uint(pr);
-          hist_add(sh, bits >> 20, bits);
+        for (int u = 0; u < UB; ++u) {
+          const int i = i0 + u * SEL_NT, pos = s0 + i;
+          ok[u] = i < per && pos >= lo && pos < hi;
+#pragma unroll
+          for (int g = 0; g < 8; ++g) x[u][g] = (ok[u] && g < G) ? __ldg(lg + (size_t)g * P.max_ctx + pos) : 0.f;
         }
-        pbits[i] = bits;
+#pragma unroll
+        for (int u = 0; u < UB; ++u) {
+          const int i = i0 + u * SEL_NT;
+          if (i >= per) break;
+          uint32_t bits = SEL_INVALID;
+          if (ok[u]) {
+            float pr = 0.f;
+#pragma unroll
+            for (int g = 0; g < 8; ++g)
+              if (g < G) pr = fmaf(fast_exp2(fmaf(x[u][g], c2, -mg[g])), rs[g], pr);
+            probs[s0 + i] = pr;
+            bits = __float_as_uint(pr);
+            hist_add(sh, bits >> 20, bits);
+          }
+          pbits[i] = bits;
+        }
       }
     } else {
       // ACCUM (reading C4): sliding sum of the last accum_window per-step rows, renormalised.
@@ -222,7 +238,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
           float pr = 0.f;
 #pragma unroll
           for (int g = 0; g < 8; ++g)
-            if (g < G) pr = fmaf(fast_exp2(fmaf(__ldcg(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
+            if (g < G) pr = fmaf(fast_exp2(fmaf(__ldg(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
           float a = (acc[pos] - ring[pos]) + pr;
           a = fmaxf(a, 0.f);
           acc[pos] = a;
@@ -389,34 +405,56 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
           }
           const bool cross = (theta != ~0ull && cum_mass + im >= theta) || cum_cnt + ic >= kt;
           const unsigned cm_ = __ballot_sync(0xffffffffu, cross);
-          // crossing lane: first lane whose inclusive prefix fires (lane 31 if none: cannot happen, see below)
+          // crossing lane: first lane whose inclusive prefix fires.  theta <= Wtot guarantees the mass
+          // condition at the latest in the lowest non-empty bin, and theta == inf implies N > kt so the
+          // count condition fires; lane 31 (whose last bin is taken unconditionally) keeps the walk total.
           const int cl = cm_ ? __ffs(cm_) - 1 : 31;
+          const unsigned long long base_m = cum_mass + shfl_u64(im - lm, cl);
+          const int base_c = cum_cnt + __shfl_sync(0xffffffffu, ic - lc, cl);
+          // second level: the 32 lanes share the cb bins of lane cl (cb <= 64: at most 2 bins per lane)
+          const int per_l = (cb + 31) / 32;
+          unsigned long long bm[2] = {0, 0};
+          int bc[2] = {0, 0};
+#pragma unroll
+          for (int u = 0; u < 2; ++u) {
+            const int j = lane * per_l + u;
+            if (u < per_l && j < cb) {
+              const int bin = S - 1 - (cl * cb + j);
+              if (C > 1) { bc[u] = (int)own->m_cnt[bin]; bm[u] = own->m_mass[bin]; }
+              else { bc[u] = (int)sh.h_cnt[bin]; bm[u] = ((unsigned long long)sh.h_hi[bin] << SEL_MSPLIT) + sh.h_lo[bin]; }
+            }
+          }
+          unsigned long long im2 = bm[0] + bm[1];
+          int ic2 = bc[0] + bc[1];
+          const unsigned long long lm2 = im2;
+          const int lc2 = ic2;
+#pragma unroll
+          for (int o = 1; o < 32; o <<= 1) {
+            const unsigned long long om = shfl_up_u64(im2, o);
+            const int oc = __shfl_up_sync(0xffffffffu, ic2, o);
+            if (lane >= o) { im2 += om; ic2 += oc; }
+          }
+          const bool cross2 = (theta != ~0ull && base_m + im2 >= theta) || base_c + ic2 >= kt;
+          const unsigned cm2 = __ballot_sync(0xffffffffu, cross2);
+          const int last_l = (cb - 1) / per_l;                 // lane that holds the chunk's last bin
+          const int cl2 = cm2 ? __ffs(cm2) - 1 : last_l;
           int r_bin = 0, r_bc = 0, r_cc = 0;
           unsigned long long r_cm = 0;
-          if (lane == cl) {
-            unsigned long long m_ = cum_mass + (im - lm);
-            int c_ = cum_cnt + (ic - lc);
-            int chosen = 0, ccnt = 0;
-            // the crossing fires inside this chunk: theta <= Wtot guarantees the mass condition at the
-            // latest in the lowest non-empty bin, and theta == inf implies N > kt so the count condition
-            // fires; the chunk's last bin is taken unconditionally to keep the walk total.
-            for (int j = 0; j < cb; ++j) {
-              const int bin = S - 1 - (lane * cb + j);
-              unsigned long long ms;
-              int c2;
-              if (C > 1) { c2 = (int)own->m_cnt[bin]; ms = own->m_mass[bin]; }
-              else { c2 = (int)sh.h_cnt[bin]; ms = ((unsigned long long)sh.h_hi[bin] << SEL_MSPLIT) + sh.h_lo[bin]; }
-              chosen = bin; ccnt = c2;
-              if ((theta != ~0ull && m_ + ms >= theta) || c_ + c2 >= kt || j == cb - 1) break;
-              m_ += ms;
-              c_ += c2;
+          if (lane == cl2) {
+            unsigned long long m_ = base_m + (im2 - lm2);
+            int c_ = base_c + (ic2 - lc2);
+            int u = 0;
+            if (per_l == 2 && lane * per_l + 1 < cb &&
+                !((theta != ~0ull && m_ + bm[0] >= theta) || c_ + bc[0] >= kt)) {
+              m_ += bm[0]; c_ += bc[0]; u = 1;
             }
-            r_bin = q * S + chosen; r_bc = ccnt; r_cc = c_; r_cm = m_;
+            r_bin = q * S + (S - 1 - (cl * cb + lane * per_l + u));
+            r_bc = bc[u]; r_cc = c_; r_cm = m_;
           }
-          r_bin = __shfl_sync(0xffffffffu, r_bin, cl);
-          r_bc = __shfl_sync(0xffffffffu, r_bc, cl);
-          r_cc = __shfl_sync(0xffffffffu, r_cc, cl);
-          r_cm = shfl_u64(r_cm, cl);
+          r_bin = __shfl_sync(0xffffffffu, r_bin, cl2);
+          r_bc = __shfl_sync(0xffffffffu, r_bc, cl2);
+          r_cc = __shfl_sync(0xffffffffu, r_cc, cl2);
+          r_cm = shfl_u64(r_cm, cl2);
           if (lane == 0) {
             sh.res_bin = r_bin; sh.res_bin_cnt = r_bc; sh.res_cum_cnt = r_cc; sh.res_cum_mass = r_cm;
           }
@@ -504,7 +542,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
     if (s) {
       const int pos = pos0 + lane;
       sel_idx[sel_before + __popc(sb & lt)] = pos;
-      votes[pos] += 1;  // cumulative selection mask = votes (L86)
+      atomicAdd(votes + pos, 1);  // cumulative selection mask = votes (L86); result unused -> RED, no round trip
     }
     if (want_mask && lane < 4) {  // bit i%8 of byte i/8 (L439): byte y of the word holds bits 8y..8y+7
       const int y = (pos0 >> 3) + lane;
