@@ -172,9 +172,15 @@ void launch_select(hardkv_ctx *ctx, const Params &P, float p, int calibrate, cud
   at[0].val.clusterDim.x = P.sel_cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
   lc.attrs = at;
   lc.numAttrs = 1;
-  if (calibrate == 2) cudaLaunchKernelEx(&lc, select_kernel<2>, P, p);
-  else if (calibrate == 1) cudaLaunchKernelEx(&lc, select_kernel<1>, P, p);
-  else cudaLaunchKernelEx(&lc, select_kernel<0>, P, p);
+  if (P.G <= 4) {
+    if (calibrate == 2) cudaLaunchKernelEx(&lc, select_kernel<2, 4>, P, p);
+    else if (calibrate == 1) cudaLaunchKernelEx(&lc, select_kernel<1, 4>, P, p);
+    else cudaLaunchKernelEx(&lc, select_kernel<0, 4>, P, p);
+  } else {
+    if (calibrate == 2) cudaLaunchKernelEx(&lc, select_kernel<2, 8>, P, p);
+    else if (calibrate == 1) cudaLaunchKernelEx(&lc, select_kernel<1, 8>, P, p);
+    else cudaLaunchKernelEx(&lc, select_kernel<0, 8>, P, p);
+  }
 }
 
 void launch_rewrite(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
@@ -259,9 +265,11 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   // the attribute is per function, so it is raised to the largest request seen in this process
   static size_t sel_smem_max = 0;
   if (select_smem_bytes(P) > sel_smem_max) sel_smem_max = select_smem_bytes(P);
-  if (cudaFuncSetAttribute(select_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess ||
-      cudaFuncSetAttribute(select_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess ||
-      cudaFuncSetAttribute(select_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sel_smem_max) != cudaSuccess) {
+  const int smx = (int)sel_smem_max;
+  const cudaFuncAttribute fa = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  if (cudaFuncSetAttribute(select_kernel<0, 4>, fa, smx) != cudaSuccess || cudaFuncSetAttribute(select_kernel<1, 4>, fa, smx) != cudaSuccess ||
+      cudaFuncSetAttribute(select_kernel<2, 4>, fa, smx) != cudaSuccess || cudaFuncSetAttribute(select_kernel<0, 8>, fa, smx) != cudaSuccess ||
+      cudaFuncSetAttribute(select_kernel<1, 8>, fa, smx) != cudaSuccess || cudaFuncSetAttribute(select_kernel<2, 8>, fa, smx) != cudaSuccess) {
     cudaGetLastError();
     delete ctx;
     return HARDKV_ERR_CUDA;

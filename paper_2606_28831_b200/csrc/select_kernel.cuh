@@ -68,8 +68,9 @@ __host__ __device__ __forceinline__ int sel_slice_len(int span, int C) {
 }
 
 // CALIBRATE: 1 = logits -> probs (2a) then select; 0 = select on state->probs as given.
-template <int CALIBRATE>
-__global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
+// GMAX: compile-time bound of the GQA group (4 or 8) -- sizes the register arrays of the calibration.
+template <int CALIBRATE, int GMAX>
+__global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
   extern __shared__ __align__(16) unsigned char sel_smem[];
   cg::cluster_group cluster = cg::this_cluster();
   const int C = P.sel_cluster;
@@ -114,7 +115,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
     // softmax in the base-2 domain: exp(z/T - m) = 2^(z*c2 - m2), c2 = log2(e)/T (one FFMA + one MUFU.EX2)
     const float c2 = 1.4426950408889634f / P.st.temperature[unit];
     const float *lg = P.st.logits + ((size_t)(b * P.Hq + h * G)) * P.max_ctx;
-    float mg[8], rs[8];
+    float mg[GMAX], rs[GMAX];
     if (CALIBRATE == 2) {
       // statistics were produced by the score kernel: one (m2, s) pair per query head and 512-token chunk
       if (C > 1) cluster.barrier_wait();
@@ -134,14 +135,14 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
       }
       __syncthreads();  // statistics published, histogram zeroed
 #pragma unroll
-      for (int g = 0; g < 8; ++g) {
+      for (int g = 0; g < GMAX; ++g) {
         mg[g] = g < G ? sh.st_m[0][g] : -INFINITY;
         rs[g] = g < G ? sh.st_s[0][g] : 0.f;
       }
     } else {
       // per query head: max and sum of exp over the pool (softmax over the pool only, reading C3)
 #pragma unroll
-      for (int g = 0; g < 8; ++g) {
+      for (int g = 0; g < GMAX; ++g) {
         if (g >= G) break;
         const float *row = lg + (size_t)g * P.max_ctx;
         float m = -INFINITY, sacc = 0.f;
@@ -181,7 +182,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
       }
       cluster.sync();
 #pragma unroll
-      for (int g = 0; g < 8; ++g) {
+      for (int g = 0; g < GMAX; ++g) {
         float m = -INFINITY, sacc = 0.f;
         if (g < G) {
           for (int c = 0; c < C; ++c) m = fmaxf(m, sh.st_m[c][g]);
@@ -197,16 +198,16 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
     const bool accum = P.st.score_mode[h] == HARDKV_SCORE_ACCUM;
     if (!accum) {
       // S_hat = softmax(z / T) per query head (Solution 1, L120), group mean (reading C2)
-      constexpr int UB = 4;
+      constexpr int UB = 16 / GMAX;
       for (int i0 = tid; i0 < per; i0 += UB * SEL_NT) {
-        float x[UB][8];
+        float x[UB][GMAX];
         bool ok[UB];
 #pragma unroll
         for (int u = 0; u < UB; ++u) {
           const int i = i0 + u * SEL_NT, pos = s0 + i;
           ok[u] = i < per && pos >= lo && pos < hi;
 #pragma unroll
-          for (int g = 0; g < 8; ++g) x[u][g] = (ok[u] && g < G) ? __ldg(lg + (size_t)g * P.max_ctx + pos) : 0.f;
+          for (int g = 0; g < GMAX; ++g) x[u][g] = (ok[u] && g < G) ? __ldg(lg + (size_t)g * P.max_ctx + pos) : 0.f;
         }
 #pragma unroll
         for (int u = 0; u < UB; ++u) {
@@ -216,7 +217,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
           if (ok[u]) {
             float pr = 0.f;
 #pragma unroll
-            for (int g = 0; g < 8; ++g)
+            for (int g = 0; g < GMAX; ++g)
               if (g < G) pr = fmaf(fast_exp2(fmaf(x[u][g], c2, -mg[g])), rs[g], pr);
             probs[s0 + i] = pr;
             bits = __float_as_uint(pr);
@@ -237,7 +238,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
         if (pos >= lo && pos < hi) {
           float pr = 0.f;
 #pragma unroll
-          for (int g = 0; g < 8; ++g)
+          for (int g = 0; g < GMAX; ++g)
             if (g < G) pr = fmaf(fast_exp2(fmaf(__ldg(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
           float a = (acc[pos] - ring[pos]) + pr;
           a = fmaxf(a, 0.f);
@@ -348,7 +349,8 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
         cluster.sync();      // B: merged ranges and range totals are visible
       }
       if (warp == 0) {
-        // ---- walk the merged bins from the top (every CTA computes the same result) ----
+        // ---- walk the merged bins from the top: every CTA finds the owner range q of the crossing from the
+        //      range totals; the owner walks its own (local) merged bins and publishes the result to all CTAs ----
         int q = 0;  // owner range that holds the crossing
         if (C > 1) {
           if (level == 0) {
@@ -372,12 +374,13 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
             }
           }
         }
-        const SelShared *own = C > 1 ? cluster.map_shared_rank(&sh, q) : &sh;
+        const SelShared *own = &sh;
+        const bool walker = C == 1 || rank == q;
         // lane l takes bins [S - (l+1)*cb, S - l*cb) of the range, top first
         const int cb = S / 32;
         unsigned long long lm = 0;
         int lc = 0;
-        if (C == 1 || !everything) {
+        if (C == 1 || (!everything && walker)) {
           for (int j = 0; j < cb; ++j) {
             const int bin = S - 1 - (lane * cb + j);
             if (C > 1) { lc += (int)own->m_cnt[bin]; lm += own->m_mass[bin]; }
@@ -393,7 +396,7 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
           }
           everything = (theta == ~0ull && N <= kt);
         }
-        if (!everything) {
+        if (!everything && walker) {
           // inclusive scan over lanes (lane 0 holds the top bins)
           unsigned long long im = lm;
           int ic = lc;
@@ -455,15 +458,17 @@ __global__ void __launch_bounds__(SEL_NT) select_kernel(Params P, float p) {
           r_bc = __shfl_sync(0xffffffffu, r_bc, cl2);
           r_cc = __shfl_sync(0xffffffffu, r_cc, cl2);
           r_cm = shfl_u64(r_cm, cl2);
-          if (lane == 0) {
-            sh.res_bin = r_bin; sh.res_bin_cnt = r_bc; sh.res_cum_cnt = r_cc; sh.res_cum_mass = r_cm;
+          if (lane < C) {
+            SelShared *dst = C > 1 ? cluster.map_shared_rank(&sh, lane) : &sh;
+            dst->res_bin = r_bin; dst->res_bin_cnt = r_bc; dst->res_cum_cnt = r_cc; dst->res_cum_mass = r_cm;
           }
-        } else if (lane == 0) {
+        } else if (everything && lane == 0) {
           sh.res_bin = -1;
         }
         if (lane == 0) sh.res_theta = theta;
       }
-      __syncthreads();
+      if (C > 1) cluster.sync();   // C: the owner's result has landed in every CTA
+      else __syncthreads();
       theta = sh.res_theta;
       if (sh.res_bin < 0) { everything = true; break; }
       prefix = (prefix << db) | (uint32_t)sh.res_bin;
