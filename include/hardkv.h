@@ -92,7 +92,8 @@ hardkv_status hardkv_workspace_bytes(const hardkv_config *cfg, size_t *bytes);
 hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t bytes, hardkv_ctx **out);
 void          hardkv_destroy(hardkv_ctx *ctx);
 const char   *hardkv_status_string(hardkv_status s);
-/* Kernel variant switch for A/B measurements: 0 = generic FMA kernels, 1 = tuned paths (default). */
+/* Kernel variant switch for A/B measurements: 0 = generic FMA kernels, 1 = tuned paths (default),
+ * 2 = tuned paths with the TMA-staged (cp.async.bulk + mbarrier ring) persistent score kernel. */
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant);
 
 /* Step 1 + Step 4 of L78.  Writes (k_new, v_new) [B][Hkv][d] at position ctx_len[b];

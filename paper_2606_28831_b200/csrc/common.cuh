@@ -85,7 +85,7 @@ __device__ __forceinline__ float warp_sum_f32(float v) {
   for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
 }
-constexpr int SCORE_PAGES_PER_CTA = 32;  // score kernel: 8 warps x 4 pages = 512 tokens = 128 KiB of K per CTA
+constexpr int SCORE_PAGES_PER_CTA = 64;  // score kernel: 8 warps x 8 pages = 1024 tokens = 256 KiB of K per CTA
 
 __device__ __forceinline__ unsigned long long shfl_xor_u64(unsigned long long v, int off) {
   unsigned lo = __shfl_xor_sync(0xffffffffu, (unsigned)v, off);

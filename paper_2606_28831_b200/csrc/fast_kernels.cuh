@@ -60,37 +60,52 @@ __global__ void __launch_bounds__(256) score_mma_kernel(Params P, const void *q_
   const float c2 = P.sm_scale * 1.4426950408889634f / P.st.temperature[unit];  // logit -> base-2 exponent of z/T
   float m0 = -INFINITY, s0 = 0.f, m1 = -INFINITY, s1 = 0.f;  // running (max, sum 2^(x - max)) of heads h0, h1
 
-  for (int pi = warp; pi < SCORE_PAGES_PER_CTA; pi += 8) {
-    const int pg = pg0 + pi;
-    if (pg < first_page || pg > last_page) continue;
-    const char *src = reinterpret_cast<const char *>(P.st.k_pool) + (size_t)__ldg(tab + pg) * (PAGE * ROWB);
-    uint4 ka[NCH], kb[NCH];
+  // a warp owns SCORE_PAGES_PER_CTA / 8 consecutive logical pages; their physical ids come in with one load
+  constexpr int PPW = SCORE_PAGES_PER_CTA / 8;
+  const int wp0 = pg0 + warp * PPW;
+  int my_page = -1;
+  if (lane < PPW && wp0 + lane >= first_page && wp0 + lane <= last_page) my_page = __ldg(tab + wp0 + lane);
+#pragma unroll 1
+  for (int j0 = 0; j0 < PPW; j0 += 2) {
+    // two pages (8 KiB) in flight per warp: all 16 loads are issued before the first MMA
+    int phys[2];
+    uint4 ka[2][NCH], kb[2][NCH];
 #pragma unroll
-    for (int c = 0; c < NCH; ++c) {
-      ka[c] = ldg_nc(src + gid * ROWB + c * 64 + tig * 16);
-      kb[c] = ldg_nc(src + (gid + 8) * ROWB + c * 64 + tig * 16);
-    }
-    float acc[4] = {0.f, 0.f, 0.f, 0.f};
+    for (int u = 0; u < 2; ++u) {
+      phys[u] = __shfl_sync(0xffffffffu, my_page, j0 + u);
+      const char *src = reinterpret_cast<const char *>(P.st.k_pool) + (size_t)(phys[u] < 0 ? 0 : phys[u]) * (PAGE * ROWB);
 #pragma unroll
-    for (int c = 0; c < NCH; ++c) {
-      mma_bf16_16816(acc, ka[c].x, kb[c].x, ka[c].y, kb[c].y, qv[c].x, qv[c].y);
-      mma_bf16_16816(acc, ka[c].z, kb[c].z, ka[c].w, kb[c].w, qv[c].z, qv[c].w);
+      for (int c = 0; c < NCH; ++c) {
+        ka[u][c] = phys[u] >= 0 ? ldg_nc(src + gid * ROWB + c * 64 + tig * 16) : make_uint4(0, 0, 0, 0);
+        kb[u][c] = phys[u] >= 0 ? ldg_nc(src + (gid + 8) * ROWB + c * 64 + tig * 16) : make_uint4(0, 0, 0, 0);
+      }
     }
-    const int pa = pg * PAGE + gid, pb = pa + 8;
-    const bool va = pa >= lo && pa < hi, vb = pb >= lo && pb < hi;
-    if (h0 < G) {
-      if (va) lg[(size_t)h0 * P.max_ctx + pa] = acc[0] * P.sm_scale;
-      if (vb) lg[(size_t)h0 * P.max_ctx + pb] = acc[2] * P.sm_scale;
-      const float xa = va ? acc[0] * c2 : -INFINITY, xb = vb ? acc[2] * c2 : -INFINITY;
-      const float mn = fmaxf(m0, fmaxf(xa, xb));
-      if (mn != -INFINITY) { s0 = s0 * fast_exp2(m0 - mn) + fast_exp2(xa - mn) + fast_exp2(xb - mn); m0 = mn; }
-    }
-    if (h1 < G) {
-      if (va) lg[(size_t)h1 * P.max_ctx + pa] = acc[1] * P.sm_scale;
-      if (vb) lg[(size_t)h1 * P.max_ctx + pb] = acc[3] * P.sm_scale;
-      const float xa = va ? acc[1] * c2 : -INFINITY, xb = vb ? acc[3] * c2 : -INFINITY;
-      const float mn = fmaxf(m1, fmaxf(xa, xb));
-      if (mn != -INFINITY) { s1 = s1 * fast_exp2(m1 - mn) + fast_exp2(xa - mn) + fast_exp2(xb - mn); m1 = mn; }
+#pragma unroll
+    for (int u = 0; u < 2; ++u) {
+      if (phys[u] < 0) continue;   // warp-uniform
+      const int pg = wp0 + j0 + u;
+      float acc[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+      for (int c = 0; c < NCH; ++c) {
+        mma_bf16_16816(acc, ka[u][c].x, kb[u][c].x, ka[u][c].y, kb[u][c].y, qv[c].x, qv[c].y);
+        mma_bf16_16816(acc, ka[u][c].z, kb[u][c].z, ka[u][c].w, kb[u][c].w, qv[c].z, qv[c].w);
+      }
+      const int pa = pg * PAGE + gid, pb = pa + 8;
+      const bool va = pa >= lo && pa < hi, vb = pb >= lo && pb < hi;
+      if (h0 < G) {
+        if (va) lg[(size_t)h0 * P.max_ctx + pa] = acc[0] * P.sm_scale;
+        if (vb) lg[(size_t)h0 * P.max_ctx + pb] = acc[2] * P.sm_scale;
+        const float xa = va ? acc[0] * c2 : -INFINITY, xb = vb ? acc[2] * c2 : -INFINITY;
+        const float mn = fmaxf(m0, fmaxf(xa, xb));
+        if (mn != -INFINITY) { s0 = s0 * fast_exp2(m0 - mn) + fast_exp2(xa - mn) + fast_exp2(xb - mn); m0 = mn; }
+      }
+      if (h1 < G) {
+        if (va) lg[(size_t)h1 * P.max_ctx + pa] = acc[1] * P.sm_scale;
+        if (vb) lg[(size_t)h1 * P.max_ctx + pb] = acc[3] * P.sm_scale;
+        const float xa = va ? acc[1] * c2 : -INFINITY, xb = vb ? acc[3] * c2 : -INFINITY;
+        const float mn = fmaxf(m1, fmaxf(xa, xb));
+        if (mn != -INFINITY) { s1 = s1 * fast_exp2(m1 - mn) + fast_exp2(xa - mn) + fast_exp2(xb - mn); m1 = mn; }
+      }
     }
   }
 

@@ -7,6 +7,7 @@
 
 #include "common.cuh"
 #include "fast_kernels.cuh"
+#include "score_tma.cuh"
 #include "select_kernel.cuh"
 #include "stage_kernels.cuh"
 #include "attend_mma.cuh"
@@ -17,6 +18,7 @@ struct hardkv_ctx {
   hardkv_config cfg;
   Params base;      // config-derived fields + workspace pointers; `st` is filled per call
   int variant;
+  int num_sms;
   size_t ws_bytes;
   int64_t launches;              // kernels launched through this ctx (hardkv_launch_count)
   char *stage_q, *stage_k, *stage_v;  // device staging of hardkv_decode_step_host (inside the workspace)
@@ -140,7 +142,7 @@ Params params_of(const hardkv_ctx *ctx, const hardkv_state *s) {
   } while (0)
 
 // bf16 tensor-core paths (variant 1); fp32 K/V and variant 0 run the generic FMA kernels
-bool fast_path(const hardkv_ctx *ctx) { return ctx->variant == 1 && ctx->cfg.kv_dtype == HARDKV_BF16; }
+bool fast_path(const hardkv_ctx *ctx) { return ctx->variant >= 1 && ctx->cfg.kv_dtype == HARDKV_BF16; }
 
 void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, cudaStream_t st) {
   ctx->launches += 1;
@@ -150,6 +152,12 @@ void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const vo
 void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
   ctx->launches += 1;
   dim3 grid(P.score_chunks, P.B * P.Hkv);
+  if (fast_path(ctx) && ctx->variant == 2) {   // TMA-staged persistent variant (A/B: see DESIGN.md)
+    const size_t smem = score_tma_smem(P.d, P.B * P.Hkv, P.B);
+    if (P.d == 128) score_tma_kernel<128><<<ctx->num_sms, SCORE_TMA_THREADS, smem, st>>>(P, q);
+    else score_tma_kernel<64><<<ctx->num_sms, SCORE_TMA_THREADS, smem, st>>>(P, q);
+    return;
+  }
   if (fast_path(ctx)) {
     if (P.d == 128) score_mma_kernel<128><<<grid, 256, 0, st>>>(P, q);
     else score_mma_kernel<64><<<grid, 256, 0, st>>>(P, q);
@@ -265,6 +273,17 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   // the attribute is per function, so it is raised to the largest request seen in this process
   static size_t sel_smem_max = 0;
   if (select_smem_bytes(P) > sel_smem_max) sel_smem_max = select_smem_bytes(P);
+  int dev = 0, nsm = 148;
+  cudaGetDevice(&dev);
+  if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
+  ctx->num_sms = nsm;
+  if (cfg->kv_dtype == HARDKV_BF16) {
+    const int ssm = (int)score_tma_smem(cfg->head_dim, cfg->batch * cfg->num_kv_heads, cfg->batch);
+    static int score_smem_max = 0;
+    if (ssm > score_smem_max) score_smem_max = ssm;
+    cudaFuncSetAttribute(score_tma_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
+    cudaFuncSetAttribute(score_tma_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
+  }
   const int smx = (int)sel_smem_max;
   const cudaFuncAttribute fa = cudaFuncAttributeMaxDynamicSharedMemorySize;
   if (cudaFuncSetAttribute(select_kernel<0, 4>, fa, smx) != cudaSuccess || cudaFuncSetAttribute(select_kernel<1, 4>, fa, smx) != cudaSuccess ||
@@ -281,7 +300,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
 void hardkv_destroy(hardkv_ctx *ctx) { delete ctx; }
 
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant) {
-  if (!ctx || variant < 0 || variant > 1) return HARDKV_ERR_INVALID_ARG;
+  if (!ctx || variant < 0 || variant > 2) return HARDKV_ERR_INVALID_ARG;
   ctx->variant = variant;
   return HARDKV_OK;
 }

@@ -116,6 +116,23 @@ def test_fused_decode_step(name, teacher, P):
             pr.force_discrete_state()
 
 
+@pytest.mark.parametrize("variant", [0, 2])
+@pytest.mark.parametrize("name", ["c1s", "c2s", "c3s", "c4s", "g1d64"])
+def test_kernel_variants(name, variant, P):
+    """Variant 0 (generic fp32-FMA kernels) and variant 2 (TMA-staged persistent score) against the oracle."""
+    wl = WL[name]
+    pr = P(wl, want_mask=False)
+    pr.eng.set_variant(variant)
+    for t in range(min(wl.steps, 8)):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)
+        pr.ob.step(q, kn, vn, wl.p)
+        pr.check_out(f"{name} v{variant} step {t}")
+        pr.check_selection_band()
+        pr.force_discrete_state()
+    pr.check_logits()
+
+
 def test_select_interval_reuses_selected_tier(P):
     """do_select = 0 between compressions (L274): append + attend over the previous selected tier."""
     wl = WL["c1s"]
