@@ -166,12 +166,10 @@ def run_cuda(args):
 
     import __graft_entry__
     __graft_entry__.build_cuda()
-    from paper_2606_28831_b200 import accounting, harness
-    from paper_2606_28831_b200.synth import make_workload
+    from paper_2606_28831_b200 import accounting, harness, sharding
 
     K, W = args.steps, args.warmup
-    wl = make_workload(args.config)
-    wl.seed += 1000 * rank                       # every rank: its own batch of the same shape
+    wl = sharding.rank_workload(args.config, rank)   # every rank: its own batch of the same shape
     if K + W > wl.max_ctx - int(wl.n0.max()):
         raise SystemExit(f"steps + warmup must be <= {wl.max_ctx - int(wl.n0.max())} for {wl.name}")
     t0 = time.time()
@@ -266,17 +264,11 @@ def run_cuda(args):
     d2h = out_h.numel() * 4
 
     # ---- reduce over ranks ------------------------------------------------------------------------
-    red = torch.tensor([ms_total, t_e2e * 1e3], dtype=torch.float64, device=dev)
-    tot = torch.tensor([float(bytes_total)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(red, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
-    ms_total, ms_e2e = float(red[0]), float(red[1])
-    bytes_all = float(tot[0])
+    ms_total, ms_e2e, bytes_all = sharding.reduce_run(ms_total, t_e2e * 1e3, bytes_total, dev)
 
     if rank == 0:
         peak, peak_src = measured_peak()
-        gbs = bytes_all / (ms_total * 1e-3) / 1e9
+        gbs = sharding.job_throughput_gbs(ms_total, bytes_all)
         e2e_gbs = bytes_all / (ms_e2e * 1e-3) / 1e9
         us_step = ms_total / K * 1e3
         dom = max(("score", "rewrite_attend", "calibrate_topp"), key=lambda s: stage_us[s])

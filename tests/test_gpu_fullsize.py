@@ -1,0 +1,94 @@
+"""-m gpu parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times (the fused
+hardkv_decode_step over the whole batch), judged on SAMPLED units the oracle computes one by one: selection
+(only tokens within 1e-6 of the threshold may differ), counts, condensed-tier bookkeeping, rewritten rows and
+attention outputs (max-abs 2e-2, mean-abs 2e-3) of the sampled (sequence, KV head) pairs.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle.oracle import OracleConfig, Unit, decode_step_batch
+from paper_2606_28831_b200 import harness
+from paper_2606_28831_b200.synth import PAGE, make_workload
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+OUT_MAX_ABS, OUT_MEAN_ABS, TAU_BAND = 2e-2, 2e-3, 1e-6
+
+
+def run_sampled(wl, sample, steps, p=None):
+    p = wl.p if p is None else p
+    eng = harness.make_engine(wl, DEV)
+    (st,), prefill = harness.make_state(wl, DEV)
+    cfg = OracleConfig(G=wl.G, d=wl.d, max_ctx=wl.max_ctx, sink=wl.sink, recent=wl.recent, k_cap=wl.k_cap,
+                       cond_cap=wl.cond_cap, accum_window=wl.accum_window, sm_scale=float(wl.sm_scale))
+    units = [Unit(cfg, *prefill[(b, h)], l_upper=int(wl.l_upper[b]), l_lower=int(wl.l_lower[b]),
+                  T=float(wl.temperature[b, h]), score_mode=int(wl.score_mode[h])) for b, h in sample]
+    pk = {u: kv[0] for u, kv in prefill.items()} if wl.mix_new_keys else None
+    out = torch.zeros(wl.B, wl.Hq, wl.d, dtype=torch.float32, device=DEV)
+    _, sel_pages = wl.page_tables()
+    flips = 0
+    for t in range(steps):
+        q = wl.step_q(t)
+        kn, vn = wl.step_kv(t, pk)
+        eng.decode_step(st, harness.to_dev(q, wl, DEV), harness.to_dev(kn, wl, DEV), harness.to_dev(vn, wl, DEV), p, out)
+        qs = np.stack([q[b, h * wl.G:(h + 1) * wl.G] for b, h in sample])
+        decode_step_batch(units, qs, np.stack([kn[b, h] for b, h in sample]), np.stack([vn[b, h] for b, h in sample]), p)
+        torch.cuda.synchronize()
+        assert int(st.err_flag.item()) == 0
+        o = out.cpu().numpy()
+        cnt, idx = st.sel_count.cpu().numpy(), st.sel_idx.cpu().numpy()
+        ccnt = st.cond_count.cpu().numpy()
+        errs = []
+        for (b, h), u in zip(sample, units):
+            i = b * wl.Hkv + h
+            assert int(st.ctx_len[b]) == u.n and int(st.c_lo[b]) == u.c_lo
+            a, r = set(idx[i, :cnt[i]].tolist()), set(u.sel_idx[:u.sel_count].tolist())
+            diff = sorted(a ^ r)
+            if diff:
+                tau = np.array([u.tau_bits], np.uint32).view(np.float32)[0]
+                assert np.all(np.abs(u.probs[diff].astype(np.float64) - float(tau)) <= TAU_BAND), (b, h, diff[:8])
+                flips += len(diff)
+            else:
+                assert cnt[i] == u.sel_count
+                kend = (u.sel_count + PAGE - 1) // PAGE * PAGE
+                if kend:
+                    pages = torch.from_numpy(sel_pages[b, h, :kend // PAGE].astype(np.int64)).to(DEV)
+                    rows = st.sel_k_pool[pages].reshape(kend, wl.d).float().cpu().numpy()
+                    np.testing.assert_array_equal(rows, u.sel_k[:kend])       # rewritten rows + zero tail: bit exact
+            assert ccnt[i] == u.cond_count
+            np.testing.assert_array_equal(st.cond_pos[i, :u.cond_count].cpu().numpy(), u.cond_pos[:u.cond_count])
+            errs.append(np.abs(o[b, h * wl.G:(h + 1) * wl.G] - u.out))
+        e = np.stack(errs)
+        assert np.isfinite(o).all() and e.max() <= OUT_MAX_ABS and e.mean() <= OUT_MEAN_ABS, (t, e.max(), e.mean())
+        # teacher forcing of the sampled units' discrete state keeps later steps comparable after a flip
+        for (b, h), u in zip(sample, units):
+            i = b * wl.Hkv + h
+            st.votes[i].copy_(torch.from_numpy(u.votes))
+    return flips
+
+
+def test_config2_full_size_sampled():
+    wl = make_workload(2)
+    order = np.argsort(wl.n0)
+    sample = [(int(order[0]), 0), (int(order[-1]), 7), (int(order[len(order) // 2]), 3), (int(order[-2]), 1),
+              (int(order[1]), 5), (int(order[-1]), 2)]
+    run_sampled(wl, sample, steps=3)
+
+
+def test_config1_full_size_sampled():
+    wl = make_workload(1)
+    run_sampled(wl, [(0, h) for h in (0, 3, 7)], steps=3)
+
+
+def test_config3_full_size_checkpoint():
+    """Config 3 at the n = 8400 checkpoint of its growth (pool above l_upper: retirement every step), batch 32."""
+    wl = make_workload(3, n0=np.full(32, 8400, np.int32))
+    run_sampled(wl, [(0, 0), (13, 2), (31, 3)], steps=3)
+
+
+@pytest.mark.parametrize("p", [0.8, 0.99])
+def test_config4_full_size_sampled(p):
+    """Config 4 (G = 5, 64k context, RAW and ACCUM heads) at two ends of its p sweep."""
+    wl = make_workload(4)
+    run_sampled(wl, [(0, 1), (3, 6), (7, 4)], steps=3, p=p)

@@ -355,3 +355,33 @@ def test_empty_pool_and_short_context():
             Vt = torch.tensor(u.V[:n], dtype=torch.float64)[None].expand(2, -1, -1)
             ref = torch.nn.functional.scaled_dot_product_attention(torch.tensor(q, dtype=torch.float64)[:, None], Kt, Vt)
             np.testing.assert_allclose(u.out, ref[:, 0].numpy(), atol=1e-5, rtol=0)
+
+
+# ---- golden fixtures: closed-form nucleus sizes (tests/golden/closed_forms.txt, with derivations) ----
+def _golden_rows():
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "closed_forms.txt")
+    rows = []
+    for line in open(path):
+        line = line.strip()
+        if line and not line.startswith("#"):
+            case, N, p, param, k = line.split()
+            rows.append((case, int(N), float(p), float(param), int(k)))
+    return rows
+
+
+@pytest.mark.parametrize("case,N,p,param,expect", _golden_rows())
+def test_golden_closed_forms(case, N, p, param, expect):
+    mc = (4 + N + 16 + 15) // 16 * 16
+    cfg, u, rng = _unit(G=1, d=64, n0=4 + N + 16, max_ctx=mc, W=16, k_cap=mc)
+    if case == "equal":
+        z = np.zeros((1, N))
+    elif case == "geometric":
+        z = -param * np.arange(N)[None, :]
+    else:
+        z = rng.standard_normal((1, N)); z[0, N // 2] += param
+    _set_logits(u, z)
+    u.calibrate(); u.topp_select(p)
+    assert u.sel_count == expect
+    if case != "dominant":
+        assert list(u.sel_idx[:expect]) == list(range(4, 4 + expect))
