@@ -23,7 +23,8 @@
 
 namespace hardkv {
 
-constexpr int ATT_MMA_CHUNK = 256;            // virtual rows per CTA: 8 warps x 2 tiles of 16
+constexpr int ATT_TPW = 4;                    // tiles of 16 rows per warp
+constexpr int ATT_MMA_CHUNK = 8 * ATT_TPW * 16;   // virtual rows per CTA: 8 warps x ATT_TPW tiles
 constexpr uint32_t ROW_INVALID = 0xffffffffu;
 
 __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
@@ -76,32 +77,37 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   for (int i = 0; i < NVC * 4; ++i) acc[i][0] = acc[i][1] = acc[i][2] = acc[i][3] = 0.f;
 
   const int v0 = c * ATT_MMA_CHUNK, v1 = min(total, v0 + ATT_MMA_CHUNK);
-  // ---- every lane resolves the source (tier << 30 | row) and rewrite destination of one of the warp's 32 rows ----
-  uint32_t src = ROW_INVALID, dst = ROW_INVALID;
-  {
-    const int v = v0 + warp * 32 + lane;
+  // ---- the rows of all tiles of the warp are resolved up front: lane l holds rows l and l + 32 of the warp's
+  //      ATT_TPW * 16 rows as source (tier << 30 | row) and rewrite destination ----
+  constexpr int RPL = ATT_TPW / 2;
+  uint32_t srcs[RPL], dsts[RPL];
+#pragma unroll
+  for (int r = 0; r < RPL; ++r) {
+    srcs[r] = ROW_INVALID; dsts[r] = ROW_INVALID;
+    const int v = v0 + warp * (ATT_TPW * 16) + r * 32 + lane;
     if (v < n_dense) {                      // Tier 1: sinks + recent window, read in place
       const int pos = v < s_end ? v : r_lo + (v - s_end);
-      src = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
+      srcs[r] = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
     } else if (v < n_dense + k) {           // Tier 2: selected rows
       const int j = v - n_dense;
       const uint32_t srow = (uint32_t)(__ldg(stab + (j >> 4)) * PAGE + (j & 15));
       if (FUSED) {
         const int pos = __ldg(idx + j);
-        src = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
-        dst = srow;
+        srcs[r] = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
+        dsts[r] = srow;
       } else {
-        src = (1u << 30) | srow;
+        srcs[r] = (1u << 30) | srow;
       }
     } else if (v < total) {                 // Tier 3: condensed residents
-      src = (2u << 30) | (uint32_t)(unit * P.cond_cap + (v - n_dense - k));
+      srcs[r] = (2u << 30) | (uint32_t)(unit * P.cond_cap + (v - n_dense - k));
     }
   }
-#pragma unroll 1
-  for (int it = 0; it < 2; ++it) {
-    const int vbase = v0 + warp * 32 + it * 16;
+#pragma unroll
+  for (int it = 0; it < ATT_TPW; ++it) {
+    const int vbase = v0 + warp * (ATT_TPW * 16) + it * 16;
     if (vbase >= v1) break;
-    const int lb = it * 16;
+    const int lb = (it & 1) * 16;
+    const uint32_t src = srcs[it >> 1], dst = dsts[it >> 1];
     uint32_t ks[2], vs[4], kd[2], vd[4];
     ks[0] = __shfl_sync(0xffffffffu, src, lb + gid);
     ks[1] = __shfl_sync(0xffffffffu, src, lb + gid + 8);
