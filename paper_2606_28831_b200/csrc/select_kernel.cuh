@@ -314,30 +314,49 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
       }
       __syncthreads();
       const int S = nb / C;  // bins per owner CTA (>= 128)
-      if (C > 1) {
-        cluster.sync();      // A: every local histogram of this level is complete
+      // ---- range pass: thread t takes bpt consecutive bins of this CTA's owner range, from the top (local index
+      //      jt = t * bpt + u <-> bin S - 1 - jt); across a cluster it first merges the C local histograms of those
+      //      bins over DSMEM.  A warp therefore covers one contiguous sub-range, whose (count, mass) it reduces. ----
+      const int bpt = S > SEL_NT ? S / SEL_NT : 1;   // <= 4
+      if (C > 1) cluster.sync();      // A: every local histogram of this level is complete
+      {
         unsigned long long tm = 0;
         uint32_t tc = 0;
-        for (int j = tid; j < S; j += SEL_NT) {
-          const int bin = rank * S + j;
-          uint32_t c_ = 0;
-          unsigned long long hi_ = 0, lo_ = 0;
-          for (int c = 0; c < C; ++c) {
-            const SelShared *src = cluster.map_shared_rank(&sh, c);
-            c_ += src->h_cnt[bin];
-            hi_ += src->h_hi[bin];
-            lo_ += src->h_lo[bin];
+        if (tid * bpt < S) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            if (u < bpt) {
+              const int bl = S - 1 - (tid * bpt + u);
+              uint32_t c_;
+              unsigned long long ms;
+              if (C > 1) {
+                const int bin = rank * S + bl;
+                unsigned long long hi_ = 0, lo_ = 0;
+                c_ = 0;
+                for (int c = 0; c < C; ++c) {
+                  const SelShared *src = cluster.map_shared_rank(&sh, c);
+                  c_ += src->h_cnt[bin];
+                  hi_ += src->h_hi[bin];
+                  lo_ += src->h_lo[bin];
+                }
+                ms = (hi_ << SEL_MSPLIT) + lo_;
+                sh.m_cnt[bl] = c_;
+                sh.m_mass[bl] = ms;
+              } else {
+                c_ = sh.h_cnt[bl];
+                ms = ((unsigned long long)sh.h_hi[bl] << SEL_MSPLIT) + sh.h_lo[bl];
+              }
+              tc += c_;
+              tm += ms;
+            }
           }
-          const unsigned long long ms = (hi_ << SEL_MSPLIT) + lo_;
-          sh.m_cnt[j] = c_;
-          sh.m_mass[j] = ms;
-          tc += c_;
-          tm += ms;
         }
         tm = warp_sum_u64(tm);
         tc = __reduce_add_sync(0xffffffffu, tc);
         if (lane == 0) { sh.red_u[warp] = tm; sh.red_c[warp] = tc; }
-        __syncthreads();
+      }
+      __syncthreads();
+      if (C > 1) {
         if (tid < C) {
           unsigned long long m_ = 0;
           uint32_t c_ = 0;
@@ -349,9 +368,9 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
         cluster.sync();      // B: merged ranges and range totals are visible
       }
       if (warp == 0) {
-        // ---- walk the merged bins from the top: every CTA finds the owner range q of the crossing from the
-        //      range totals; the owner walks its own (local) merged bins and publishes the result to all CTAs ----
-        int q = 0;  // owner range that holds the crossing
+        // ---- walk from the top: every CTA finds the owner range q of the crossing from the range totals; the
+        //      owner descends warp sub-range -> lane -> bin on its own (local) data and publishes the result ----
+        int q = 0;
         if (C > 1) {
           if (level == 0) {
             unsigned long long wtot = 0;
@@ -374,19 +393,10 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
             }
           }
         }
-        const SelShared *own = &sh;
         const bool walker = C == 1 || rank == q;
-        // lane l takes bins [S - (l+1)*cb, S - l*cb) of the range, top first
-        const int cb = S / 32;
-        unsigned long long lm = 0;
-        int lc = 0;
-        if (C == 1 || (!everything && walker)) {
-          for (int j = 0; j < cb; ++j) {
-            const int bin = S - 1 - (lane * cb + j);
-            if (C > 1) { lc += (int)own->m_cnt[bin]; lm += own->m_mass[bin]; }
-            else { lc += (int)sh.h_cnt[bin]; lm += ((unsigned long long)sh.h_hi[bin] << SEL_MSPLIT) + sh.h_lo[bin]; }
-          }
-        }
+        const int nwr = (S / bpt) / 32;                     // active warp sub-ranges (<= 16)
+        unsigned long long lm = lane < nwr ? sh.red_u[lane] : 0ull;
+        int lc = lane < nwr ? (int)sh.red_c[lane] : 0;
         if (C == 1 && level == 0) {
           const unsigned long long wtot = warp_sum_u64(lm);
           if (!all) {
@@ -397,7 +407,10 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
           everything = (theta == ~0ull && N <= kt);
         }
         if (!everything && walker) {
-          // inclusive scan over lanes (lane 0 holds the top bins)
+          // crossing test of an inclusive prefix: theta <= Wtot guarantees the mass condition at the latest in the
+          // lowest non-empty bin, and theta == inf implies N > kt so the count condition fires; the last element is
+          // taken unconditionally at every level to keep the walk total.
+          // level A: the warp sub-ranges (lane w holds sub-range w, top first)
           unsigned long long im = lm;
           int ic = lc;
 #pragma unroll
@@ -406,53 +419,49 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
             const int oc = __shfl_up_sync(0xffffffffu, ic, o);
             if (lane >= o) { im += om; ic += oc; }
           }
-          const bool cross = (theta != ~0ull && cum_mass + im >= theta) || cum_cnt + ic >= kt;
-          const unsigned cm_ = __ballot_sync(0xffffffffu, cross);
-          // crossing lane: first lane whose inclusive prefix fires.  theta <= Wtot guarantees the mass
-          // condition at the latest in the lowest non-empty bin, and theta == inf implies N > kt so the
-          // count condition fires; lane 31 (whose last bin is taken unconditionally) keeps the walk total.
-          const int cl = cm_ ? __ffs(cm_) - 1 : 31;
-          const unsigned long long base_m = cum_mass + shfl_u64(im - lm, cl);
-          const int base_c = cum_cnt + __shfl_sync(0xffffffffu, ic - lc, cl);
-          // second level: the 32 lanes share the cb bins of lane cl (cb <= 64: at most 2 bins per lane)
-          const int per_l = (cb + 31) / 32;
-          unsigned long long bm[2] = {0, 0};
-          int bc[2] = {0, 0};
+          const unsigned cmA = __ballot_sync(0xffffffffu, (theta != ~0ull && cum_mass + im >= theta) || cum_cnt + ic >= kt);
+          const int wr = cmA ? min(__ffs(cmA) - 1, nwr - 1) : nwr - 1;
+          const unsigned long long baseA_m = cum_mass + shfl_u64(im - lm, wr);
+          const int baseA_c = cum_cnt + __shfl_sync(0xffffffffu, ic - lc, wr);
+          // level B: the 32 lanes of sub-range wr, bpt bins each
+          unsigned long long bm[4] = {0, 0, 0, 0};
+          int bc[4] = {0, 0, 0, 0};
 #pragma unroll
-          for (int u = 0; u < 2; ++u) {
-            const int j = lane * per_l + u;
-            if (u < per_l && j < cb) {
-              const int bin = S - 1 - (cl * cb + j);
-              if (C > 1) { bc[u] = (int)own->m_cnt[bin]; bm[u] = own->m_mass[bin]; }
-              else { bc[u] = (int)sh.h_cnt[bin]; bm[u] = ((unsigned long long)sh.h_hi[bin] << SEL_MSPLIT) + sh.h_lo[bin]; }
+          for (int u = 0; u < 4; ++u) {
+            if (u < bpt) {
+              const int bl = S - 1 - ((wr * 32 + lane) * bpt + u);
+              if (C > 1) { bc[u] = (int)sh.m_cnt[bl]; bm[u] = sh.m_mass[bl]; }
+              else { bc[u] = (int)sh.h_cnt[bl]; bm[u] = ((unsigned long long)sh.h_hi[bl] << SEL_MSPLIT) + sh.h_lo[bl]; }
             }
           }
-          unsigned long long im2 = bm[0] + bm[1];
-          int ic2 = bc[0] + bc[1];
-          const unsigned long long lm2 = im2;
-          const int lc2 = ic2;
+          const unsigned long long lm2 = bm[0] + bm[1] + bm[2] + bm[3];
+          const int lc2 = bc[0] + bc[1] + bc[2] + bc[3];
+          unsigned long long im2 = lm2;
+          int ic2 = lc2;
 #pragma unroll
           for (int o = 1; o < 32; o <<= 1) {
             const unsigned long long om = shfl_up_u64(im2, o);
             const int oc = __shfl_up_sync(0xffffffffu, ic2, o);
             if (lane >= o) { im2 += om; ic2 += oc; }
           }
-          const bool cross2 = (theta != ~0ull && base_m + im2 >= theta) || base_c + ic2 >= kt;
-          const unsigned cm2 = __ballot_sync(0xffffffffu, cross2);
-          const int last_l = (cb - 1) / per_l;                 // lane that holds the chunk's last bin
-          const int cl2 = cm2 ? __ffs(cm2) - 1 : last_l;
+          const unsigned cmB = __ballot_sync(0xffffffffu, (theta != ~0ull && baseA_m + im2 >= theta) || baseA_c + ic2 >= kt);
+          const int cl2 = cmB ? __ffs(cmB) - 1 : 31;
           int r_bin = 0, r_bc = 0, r_cc = 0;
           unsigned long long r_cm = 0;
           if (lane == cl2) {
-            unsigned long long m_ = base_m + (im2 - lm2);
-            int c_ = base_c + (ic2 - lc2);
+            // level C: the (<= 4) bins of the crossing lane
+            unsigned long long m_ = baseA_m + (im2 - lm2);
+            int c_ = baseA_c + (ic2 - lc2);
             int u = 0;
-            if (per_l == 2 && lane * per_l + 1 < cb &&
-                !((theta != ~0ull && m_ + bm[0] >= theta) || c_ + bc[0] >= kt)) {
-              m_ += bm[0]; c_ += bc[0]; u = 1;
+#pragma unroll
+            for (int v = 0; v < 3; ++v) {
+              if (u == v && v + 1 < bpt && !((theta != ~0ull && m_ + bm[v] >= theta) || c_ + bc[v] >= kt)) {
+                m_ += bm[v]; c_ += bc[v]; u = v + 1;
+              }
             }
-            r_bin = q * S + (S - 1 - (cl * cb + lane * per_l + u));
-            r_bc = bc[u]; r_cc = c_; r_cm = m_;
+            r_bin = q * S + (S - 1 - ((wr * 32 + lane) * bpt + u));
+            r_bc = u == 0 ? bc[0] : (u == 1 ? bc[1] : (u == 2 ? bc[2] : bc[3]));
+            r_cc = c_; r_cm = m_;
           }
           r_bin = __shfl_sync(0xffffffffu, r_bin, cl2);
           r_bc = __shfl_sync(0xffffffffu, r_bc, cl2);

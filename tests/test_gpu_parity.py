@@ -133,6 +133,27 @@ def test_kernel_variants(name, variant, P):
     pr.check_logits()
 
 
+@pytest.mark.parametrize("cluster", [1, 2, 4, 8])
+@pytest.mark.parametrize("name", ["c2s", "c4s", "g8"])
+def test_select_every_cluster_size(name, cluster, P, monkeypatch):
+    """The select kernel at every cluster size (1 = single CTA, no DSMEM): bit exact from identical probabilities."""
+    monkeypatch.setenv("HARDKV_SELECT_CLUSTER", str(cluster))
+    wl = WL[name]
+    pr = P(wl)
+    for t in range(3):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)
+        pr.ob.step(q, kn, vn, wl.p)
+        pr.check_out(f"{name} C{cluster} step {t}")
+        assert pr.check_selection_band() == 0
+        votes0 = pr.st.votes.clone()
+        pr.upload_oracle_probs()
+        pr.eng.topp_select(pr.st, wl.p)
+        pr.st.votes.copy_(votes0)
+        np.testing.assert_array_equal(pr.st.sel_idx.cpu().numpy(), pr.ob.sel_idx())
+        np.testing.assert_array_equal(pr.st.sel_count.cpu().numpy(), pr.ob.sel_count())
+
+
 def test_select_interval_reuses_selected_tier(P):
     """do_select = 0 between compressions (L274): append + attend over the previous selected tier."""
     wl = WL["c1s"]
