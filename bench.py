@@ -31,6 +31,8 @@ METRIC = "decode_step_kv_bandwidth"      # B_min / time of the fused select+rewr
 UNIT = "GB/s"
 NOMINAL_HBM_GBS = 8000.0                 # the contract's "8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                # B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1_02_final.md), config 2
+NCU_TRAFFIC_BYTES = {2: {"score": 582.6e6, "rewrite_attend": 281.1e6, "calibrate_topp": 41.3e6}}
 
 
 def log(*a):
@@ -169,12 +171,20 @@ def run_cuda(args):
     from paper_2606_28831_b200 import accounting, harness, sharding
 
     K, W = args.steps, args.warmup
-    wl = sharding.rank_workload(args.config, rank)   # every rank: its own batch of the same shape
-    if K + W > wl.max_ctx - int(wl.n0.max()):
-        raise SystemExit(f"steps + warmup must be <= {wl.max_ctx - int(wl.n0.max())} for {wl.name}")
+    over = {}
+    if args.n0:
+        B0 = sharding.rank_workload(args.config, 0).B
+        over["n0"] = np.full(B0, args.n0, np.int32)
+    wl = sharding.rank_workload(args.config, rank, **over)   # every rank: its own batch of the same shape
+    if args.p:
+        wl.p = args.p
+    L = args.layers or (32 if args.config == 1 else 1)
     t0 = time.time()
     eng = harness.make_engine(wl, dev)
-    (st,), prefill = harness.make_state(wl, dev)
+    if K + W > (wl.max_ctx - int(wl.n0.max())) * L:
+        raise SystemExit(f"steps + warmup must be <= {(wl.max_ctx - int(wl.n0.max())) * L} for {wl.name} with {L} layer(s)")
+    states, prefill = harness.make_state(wl, dev, layers=L)   # step t runs on layer t % L (distinct data, shared tables)
+    st = states[0]
     pk = {u: kv[0] for u, kv in prefill.items()} if wl.mix_new_keys else None
     tdt = harness.torch_dtype(wl)
     qs, ks, vs = [], [], []
@@ -191,7 +201,7 @@ def run_cuda(args):
     if rank == 0:
         log(f"[bench] {wl.name}: setup {time.time() - t0:.1f}s, units={wl.B * wl.Hkv}, "
             f"n0 mean={wl.n0.mean():.0f}, steps={K}, warmup={W}")
-    snap0 = harness.snapshot(st)
+    snaps = [harness.snapshot(x) for x in states]
     stream = torch.cuda.current_stream()
 
     def barrier():
@@ -200,9 +210,10 @@ def run_cuda(args):
         torch.cuda.synchronize()
 
     def warm():
-        harness.restore(st, snap0)
+        for x, sn in zip(states, snaps):
+            harness.restore(x, sn)
         for t in range(W):
-            eng.decode_step(st, q_d[t], k_d[t], v_d[t], wl.p, out)
+            eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
 
     # ---- (1) device-resident timed region: K fused steps --------------------------------------
     warm()
@@ -216,13 +227,13 @@ def run_cuda(args):
     barrier()
     e0.record(stream)
     for t in range(W, W + K):
-        eng.decode_step(st, q_d[t], k_d[t], v_d[t], wl.p, out)
+        eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
     e1.record(stream)
     barrier()
     launches = eng.launch_count() - n_before
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop()
-    assert int(st.err_flag.item()) == 0, "device err_flag set"
+    assert all(int(x.err_flag.item()) == 0 for x in states), "device err_flag set"
     assert bool(torch.isfinite(out).all()), "non-finite attention output"
 
     # ---- (2) same steps, stage by stage with events (kernel shares + per-step byte counts) ------
@@ -235,6 +246,7 @@ def run_cuda(args):
     cnt_lo = torch.zeros(K, wl.B, dtype=torch.int32, device=dev)
     torch.cuda.synchronize()
     for i, t in enumerate(range(W, W + K)):
+        st = states[t % L]
         ev[i][0].record(stream)
         eng.append_kv(st, k_d[t], v_d[t]); ev[i][1].record(stream)
         eng.score(st, q_d[t]); ev[i][2].record(stream)
@@ -257,7 +269,7 @@ def run_cuda(args):
     barrier()
     t_e2e0 = time.perf_counter()
     for t in range(W, W + K):
-        eng.decode_step_host(st, q_h[t], k_h[t], v_h[t], wl.p, out_h)
+        eng.decode_step_host(states[t % L], q_h[t], k_h[t], v_h[t], wl.p, out_h)
         stream.synchronize()                      # the caller reads out_h before the next token
     t_e2e = time.perf_counter() - t_e2e0
     h2d = (q_h[0].numel() + k_h[0].numel() + v_h[0].numel()) * q_h.element_size()
@@ -272,7 +284,8 @@ def run_cuda(args):
         e2e_gbs = bytes_all / (ms_e2e * 1e-3) / 1e9
         us_step = ms_total / K * 1e3
         dom = max(("score", "rewrite_attend", "calibrate_topp"), key=lambda s: stage_us[s])
-        roof = {"kernel": dom, "bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src, "traffic": None}
+        roof = {"kernel": dom, "bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
+                "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(dom) if not (args.n0 or args.p) else None}
         if dom in bytes_stage:
             roof["achieved"] = bytes_stage[dom] / (stage_us[dom] * 1e-6) / 1e9
             roof["algorithmic_bytes_per_launch"] = bytes_stage[dom]
@@ -288,9 +301,9 @@ def run_cuda(args):
             "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config}] ({wl.name})", "batch": wl.B,
                        "q_heads": wl.Hq, "kv_heads": wl.Hkv, "head_dim": wl.d, "ctx": [int(wl.n0.min()), int(wl.n0.max())],
-                       "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": 1,
-                       "l2": "inputs larger than L2 (K pool %.0f MB per layer-step), no flush" % (
-                           per_step[0]["score"] / 1e6),
+                       "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": L,
+                       "l2": "inputs larger than L2 (K scan %.0f MB per layer-step x %d layer(s) of distinct data cycled), "
+                             "no flush" % (per_step[0]["score"] / 1e6, L),
                        "parallelism": f"units sharded, {world} rank(s), no collective"},
             "us_per_layer_step": us_step,
             "tokens_per_s_layer": wl.B * world / (us_step * 1e-6),
@@ -307,7 +320,7 @@ def run_cuda(args):
             "clocks": clocks,
         }
         if world == 1 and not args.no_cpu_baseline:
-            del st, eng
+            del st, eng, states, snaps
             torch.cuda.empty_cache()
             g, us, cores, sample, done, _ = oracle_leg(args.config, steps=4, warmup=1, budget_s=20.0,
                                                        sample_B=args.ref_batch)
@@ -330,6 +343,10 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: the target config)")
     ap.add_argument("--ref-batch", type=int, default=4, help="sequences in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--layers", type=int, default=0, help="layers of distinct KV data cycled per step (0: 32 for config 1 whose "
+                    "single-layer K fits L2, else 1)")
+    ap.add_argument("--n0", type=int, default=0, help="override: uniform prefill context (config 3 checkpoints)")
+    ap.add_argument("--p", type=float, default=0.0, help="override the nucleus mass (config 4 sweep)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     if args.impl == "reference":
