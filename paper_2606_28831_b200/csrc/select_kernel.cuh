@@ -198,32 +198,61 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
     const bool accum = P.st.score_mode[h] == HARDKV_SCORE_ACCUM;
     if (!accum) {
       // S_hat = softmax(z / T) per query head (Solution 1, L120), group mean (reading C2)
-      constexpr int UB = 16 / GMAX;
-      for (int i0 = tid; i0 < per; i0 += UB * SEL_NT) {
-        float x[UB][GMAX];
-        bool ok[UB];
+      // a thread owns quads of 4 consecutive tokens: one 16-byte load per query head and quad, UQ quads in
+      // flight (32 registers of logits), 16-byte stores of the probabilities and of the slice
+      constexpr int UQ = 8 / GMAX;
+      const int nq = per >> 2;
+      for (int q0 = tid; q0 < nq; q0 += UQ * SEL_NT) {
+        float4 x[UQ][GMAX];
 #pragma unroll
-        for (int u = 0; u < UB; ++u) {
-          const int i = i0 + u * SEL_NT, pos = s0 + i;
-          ok[u] = i < per && pos >= lo && pos < hi;
+        for (int u = 0; u < UQ; ++u) {
+          const int qd = q0 + u * SEL_NT, pos = s0 + 4 * qd;
+          const bool live = qd < nq && pos < hi && pos + 3 >= lo;
+          const bool vec = pos + 3 < P.max_ctx;     // the quad lies inside the logits row
 #pragma unroll
-          for (int g = 0; g < GMAX; ++g) x[u][g] = (ok[u] && g < G) ? __ldg(lg + (size_t)g * P.max_ctx + pos) : 0.f;
+          for (int g = 0; g < GMAX; ++g) {
+            x[u][g] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (live && g < G) {
+              const float *src = lg + (size_t)g * P.max_ctx + pos;
+              if (vec) {
+                x[u][g] = __ldg(reinterpret_cast<const float4 *>(src));
+              } else {
+                if (pos < P.max_ctx) x[u][g].x = __ldg(src);
+                if (pos + 1 < P.max_ctx) x[u][g].y = __ldg(src + 1);
+                if (pos + 2 < P.max_ctx) x[u][g].z = __ldg(src + 2);
+              }
+            }
+          }
         }
 #pragma unroll
-        for (int u = 0; u < UB; ++u) {
-          const int i = i0 + u * SEL_NT;
-          if (i >= per) break;
-          uint32_t bits = SEL_INVALID;
-          if (ok[u]) {
-            float pr = 0.f;
+        for (int u = 0; u < UQ; ++u) {
+          const int qd = q0 + u * SEL_NT, pos = s0 + 4 * qd;
+          if (qd >= nq) break;
+          float pr[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-            for (int g = 0; g < GMAX; ++g)
-              if (g < G) pr = fmaf(fast_exp2(fmaf(x[u][g], c2, -mg[g])), rs[g], pr);
-            probs[s0 + i] = pr;
-            bits = __float_as_uint(pr);
-            hist_add(sh, bits >> 20, bits);
+          for (int g = 0; g < GMAX; ++g) {
+            if (g < G) {
+              pr[0] = fmaf(fast_exp2(fmaf(x[u][g].x, c2, -mg[g])), rs[g], pr[0]);
+              pr[1] = fmaf(fast_exp2(fmaf(x[u][g].y, c2, -mg[g])), rs[g], pr[1]);
+              pr[2] = fmaf(fast_exp2(fmaf(x[u][g].z, c2, -mg[g])), rs[g], pr[2]);
+              pr[3] = fmaf(fast_exp2(fmaf(x[u][g].w, c2, -mg[g])), rs[g], pr[3]);
+            }
           }
-          pbits[i] = bits;
+          uint32_t bits[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const bool okk = pos + e >= lo && pos + e < hi;
+            bits[e] = okk ? __float_as_uint(pr[e]) : SEL_INVALID;
+            if (okk) hist_add(sh, bits[e] >> 20, bits[e]);
+          }
+          if (pos >= lo && pos + 3 < hi) {
+            *reinterpret_cast<float4 *>(probs + pos) = make_float4(pr[0], pr[1], pr[2], pr[3]);
+          } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+              if (bits[e] != SEL_INVALID) probs[pos + e] = pr[e];
+          }
+          *reinterpret_cast<uint4 *>(pbits + 4 * qd) = make_uint4(bits[0], bits[1], bits[2], bits[3]);
         }
       }
     } else {
@@ -307,9 +336,12 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
         for (int d = tid; d < nb; d += SEL_NT) { sh.h_cnt[d] = 0; sh.h_hi[d] = 0; sh.h_lo[d] = 0; }
         __syncthreads();
         const int hs = shift + db;
-        for (int i = tid; i < per; i += SEL_NT) {
-          const uint32_t bits = pbits[i];
-          if ((bits >> hs) == prefix) hist_add(sh, (bits >> shift) & (nb - 1), bits);
+        for (int i = tid * 4; i < per; i += 4 * SEL_NT) {
+          const uint4 b4 = *reinterpret_cast<const uint4 *>(pbits + i);
+          if ((b4.x >> hs) == prefix) hist_add(sh, (b4.x >> shift) & (nb - 1), b4.x);
+          if ((b4.y >> hs) == prefix) hist_add(sh, (b4.y >> shift) & (nb - 1), b4.y);
+          if ((b4.z >> hs) == prefix) hist_add(sh, (b4.z >> shift) & (nb - 1), b4.z);
+          if ((b4.w >> hs) == prefix) hist_add(sh, (b4.w >> shift) & (nb - 1), b4.w);
         }
       }
       __syncthreads();
