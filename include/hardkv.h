@@ -107,7 +107,8 @@ hardkv_status hardkv_score(hardkv_ctx *, const hardkv_state *, const void *q, ha
 hardkv_status hardkv_calibrate_topp(hardkv_ctx *, const hardkv_state *, float p, hardkv_stream);
 /* Top-p nucleus (L108) on state->probs as given: integer mass w_i = rn(P_i 2^32),
  * order (P bits desc, position asc), minimal prefix with mass >= ceil(p * sum w),
- * clamped to k_cap (L233).  Writes sel_idx, sel_count, sel_table, (sel_mask), votes += 1. */
+ * clamped to k_cap (L233).  Writes sel_idx, sel_count, sel_table, (sel_mask), votes += 1.
+ * probs must be probabilities (0 <= P <= 1; larger values are treated as 1). */
 hardkv_status hardkv_topp_select(hardkv_ctx *, const hardkv_state *, float p, hardkv_stream);
 /* Rewrite Cache (L172): gather the selected rows into the contiguous selected tier. */
 hardkv_status hardkv_rewrite(hardkv_ctx *, const hardkv_state *, hardkv_stream);

@@ -60,31 +60,21 @@ WsLayout ws_layout(const hardkv_config &c) {
 
 size_t select_smem_bytes(const Params &P) { return (size_t)P.sel_slice_cap * 4 + sizeof(SelShared); }
 
-// Cluster size of the select kernel.  The kernel is latency bound (barriers, DSMEM merges, a few
-// dependent memory round trips), so the cost of a geometry is modelled as
-//   waves x (fixed + tokens per thread [+ cluster overhead]),
-// with waves from the CTAs that fit on 148 SMs given the shared memory of one slice.  The cheapest
-// of C = 1, 2, 4, 8 wins; a slice must fit one SM.
+// Cluster size of the select kernel, from measurements on B200: the kernel is latency bound and
+// every extra CTA of a cluster adds DSMEM-merge and barrier latency, so the smallest cluster that keeps a CTA's
+// slice near 16 k tokens (~32 per thread) wins (config 2: C = 2 < 1 < 4 < 8; config 3: 1 < 2 < 4; config 4: 4 < 8 < 2);
+// with only a few units the clusters are widened to spread them over the chip (config 1: 8 < 2 < 1).
 void select_geometry(const hardkv_config &c, int *cluster, int *slice_cap) {
   const int units = c.batch * c.num_kv_heads;
   const int max_pool = c.max_ctx - c.recent > 0 ? c.max_ctx - c.recent : 1;
   const char *force = getenv("HARDKV_SELECT_CLUSTER");   // A/B measurements only
-  const int forced = force ? atoi(force) : 0;
-  double best = 1e30;
-  *cluster = 0;
-  for (int C = 1; C <= SEL_MAXC; C <<= 1) {
-    const int cap = sel_slice_len(max_pool + 31, C);
-    const size_t smem = (size_t)cap * 4 + sizeof(SelShared);
-    if (smem > 227u * 1024u) continue;
-    int cps = (int)((228u * 1024u) / (smem + 1024u));
-    if (cps > 2048 / SEL_NT) cps = 2048 / SEL_NT;
-    const int slots = 148 * cps;
-    const int waves = (units * C + slots - 1) / slots;
-    double cost = waves * (20.0 + (double)cap / SEL_NT + (C > 1 ? 3.0 : 0.0));
-    if (forced == C) cost = -1.0;
-    if (cost < best) { best = cost; *cluster = C; *slice_cap = cap; }
-  }
-  if (*cluster == 0) { *cluster = SEL_MAXC; *slice_cap = sel_slice_len(max_pool + 31, SEL_MAXC); }
+  int C = 1;
+  while (C < SEL_MAXC && sel_slice_len(max_pool + 31, C) > 17408) C <<= 1;
+  while (C < SEL_MAXC && units * C * 2 <= 148) C <<= 1;
+  if (force && (atoi(force) == 1 || atoi(force) == 2 || atoi(force) == 4 || atoi(force) == 8)) C = atoi(force);
+  while (C < SEL_MAXC && (size_t)sel_slice_len(max_pool + 31, C) * 4 + sizeof(SelShared) > 227u * 1024u) C <<= 1;
+  *cluster = C;
+  *slice_cap = sel_slice_len(max_pool + 31, C);
 }
 
 hardkv_status check_config(const hardkv_config *c) {

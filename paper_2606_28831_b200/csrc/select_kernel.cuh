@@ -8,7 +8,7 @@
 // shared memory (DSMEM) and cluster barriers; nothing but the final results touches HBM.
 //
 // The nucleus is found without a sort: a most-significant-digit radix descent on the fp32 bit
-// pattern of P (all P >= 0, so unsigned order == float order) with digits of 11, 10 and 10 bits.
+// pattern of P (0 <= P <= 1: unsigned order == float order, 30 significant bits) with three digits of 10 bits.
 // Each level builds a histogram of (count, integer mass) per digit with w_i = rn(P_i * 2^32)
 // summed exactly (u32 shared atomics on count, w >> 12 and w & 4095): exact and order
 // independent, so it reproduces a sorted-prefix definition bit for bit (reading C5).  The bins
@@ -26,7 +26,8 @@ namespace cg = cooperative_groups;
 constexpr int SEL_NT = 512;
 constexpr int SEL_NW = SEL_NT / 32;
 constexpr int SEL_MAXC = 8;        // portable cluster size limit
-constexpr int SEL_NB = 2048;       // bins of the widest level
+constexpr int SEL_NB = 1024;       // bins per level: a probability is <= 1, so its fp32 pattern has 30 significant bits
+constexpr uint32_t SEL_ONE = 0x3f800000u;   // bit pattern of 1.0f: larger inputs are treated as 1
 constexpr int SEL_MSPLIT = 12;     // mass kept as (w >> 12, w & 4095) in two u32 counters
 constexpr uint32_t SEL_INVALID = 0xffffffffu;  // slice entry outside the pool (never a probability)
 
@@ -243,7 +244,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
           for (int e = 0; e < 4; ++e) {
             const bool okk = pos + e >= lo && pos + e < hi;
             bits[e] = okk ? __float_as_uint(pr[e]) : SEL_INVALID;
-            if (okk) hist_add(sh, bits[e] >> 20, bits[e]);
+            if (okk) { bits[e] = min(bits[e], SEL_ONE); hist_add(sh, bits[e] >> 20, bits[e]); }
           }
           if (pos >= lo && pos + 3 < hi) {
             *reinterpret_cast<float4 *>(probs + pos) = make_float4(pr[0], pr[1], pr[2], pr[3]);
@@ -295,7 +296,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
         if (ab == SEL_INVALID) continue;
         const float pr = tot > 0.0 ? (float)((double)__uint_as_float(ab) / tot) : 0.f;
         probs[s0 + i] = pr;
-        const uint32_t bits = __float_as_uint(pr);
+        const uint32_t bits = min(__float_as_uint(pr), SEL_ONE);
         pbits[i] = bits;
         hist_add(sh, bits >> 20, bits);
       }
@@ -308,7 +309,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
       const int pos = s0 + i;
       uint32_t bits = SEL_INVALID;
       if (pos >= lo && pos < hi) {
-        bits = __float_as_uint(probs[pos]) & 0x7fffffffu;
+        bits = min(__float_as_uint(probs[pos]) & 0x7fffffffu, SEL_ONE);
         hist_add(sh, bits >> 20, bits);
       }
       pbits[i] = bits;
@@ -325,10 +326,10 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
     uint32_t prefix = 0;
     unsigned long long theta = ~0ull, cum_mass = 0;
     int cum_cnt = 0, bin_cnt = 0;
-    bool everything = false;
+    bool everything = false, single = false;
 #pragma unroll 1
     for (int level = 0; level < 3; ++level) {
-      const int db = level == 0 ? 11 : 10;          // digit bits
+      const int db = 10;                            // digit bits: 3 x 10 = the 30 significant bits
       const int shift = level == 0 ? 20 : (level == 1 ? 10 : 0);
       const int nb = 1 << db;
       if (level > 0) {
@@ -516,10 +517,17 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
       bin_cnt = sh.res_bin_cnt;
       cum_cnt = sh.res_cum_cnt;
       cum_mass = sh.res_cum_mass;
+      // a crossing bin that holds one token ends the descent: that token is the last of the nucleus, whatever its
+      // remaining digits (every CTA reads the same bin_cnt, so the exit is uniform over the cluster)
+      if (bin_cnt == 1 && level < 2) { single = true; prefix <<= shift; break; }
       // the next level rewrites sh.h_* (after its own __syncthreads) and sh.res_* (after two more barriers)
     }
     if (everything) {
       k = N;  // tau = 0, all ties taken
+    } else if (single) {
+      tau = prefix;   // low digits zero: the token is > tau, or == tau and the one tie taken
+      r_ties = 1;
+      k = cum_cnt + 1;
     } else {
       tau = prefix;
       const unsigned long long wt = mass_of_bits(tau);
