@@ -224,12 +224,25 @@ def run_cuda(args):
     time.sleep(0.15)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n_before = eng.launch_count()
-    barrier()
-    e0.record(stream)
-    for t in range(W, W + K):
-        eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
-    e1.record(stream)
-    barrier()
+    if args.eager:
+        barrier()
+        e0.record(stream)
+        for t in range(W, W + K):
+            eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
+        e1.record(stream)
+        barrier()
+    else:
+        # the K steps captured into ONE CUDA graph (static shapes, counts on the device: L53, L63) and replayed once:
+        # the state advances on the device exactly as in the eager loop
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            for t in range(W, W + K):
+                eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
+        barrier()
+        e0.record(stream)
+        graph.replay()
+        e1.record(stream)
+        barrier()
     launches = eng.launch_count() - n_before
     ms_total = e0.elapsed_time(e1)
     clocks = sampler.stop()
@@ -302,6 +315,7 @@ def run_cuda(args):
             "config": {"workload": f"BASELINE.json configs[{args.config}] ({wl.name})", "batch": wl.B,
                        "q_heads": wl.Hq, "kv_heads": wl.Hkv, "head_dim": wl.d, "ctx": [int(wl.n0.min()), int(wl.n0.max())],
                        "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": L,
+                       "launch": "eager" if args.eager else "one CUDA graph of the K steps",
                        "l2": "inputs larger than L2 (K scan %.0f MB per layer-step x %d layer(s) of distinct data cycled), "
                              "no flush" % (per_step[0]["score"] / 1e6, L),
                        "parallelism": f"units sharded, {world} rank(s), no collective"},
@@ -343,6 +357,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: the target config)")
     ap.add_argument("--ref-batch", type=int, default=4, help="sequences in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--eager", action="store_true", help="time eager launches instead of one captured CUDA graph of the K steps")
     ap.add_argument("--layers", type=int, default=0, help="layers of distinct KV data cycled per step (0: 32 for config 1 whose "
                     "single-layer K fits L2, else 1)")
     ap.add_argument("--n0", type=int, default=0, help="override: uniform prefill context (config 3 checkpoints)")
