@@ -276,6 +276,28 @@ def run_cuda(args):
     bytes_stage = {"score": float(np.mean([p["score"] for p in per_step])),
                    "rewrite_attend": float(np.mean([p["attend"] + p["rewrite_write"] for p in per_step]))}
 
+    # ---- (2b) context lines: the unfused five-call pipeline, and the paper's amortised regime (L274) ------------
+    def timed_loop(body):
+        warm()
+        a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record(stream)
+        for t in range(W, W + K):
+            body(t)
+        b_.record(stream)
+        torch.cuda.synchronize()
+        return a.elapsed_time(b_) / K * 1e3
+
+    def five_calls(t):
+        s_ = states[t % L]
+        eng.append_kv(s_, k_d[t], v_d[t]); eng.score(s_, q_d[t]); eng.calibrate_topp(s_, wl.p)
+        eng.rewrite(s_); eng.decode_attn(s_, q_d[t], out)
+
+    SI = args.select_interval
+    unfused_us = timed_loop(five_calls)
+    amortised_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out,
+                                                        do_select=((t - W) // L) % SI == 0))
+
     # ---- (3) end to end through the host-buffer entry point -------------------------------------
     warm()
     torch.cuda.synchronize()
@@ -327,6 +349,10 @@ def run_cuda(args):
             "mean_k": float(np.mean([p["mean_k"] for p in per_step])), "max_k": int(max(p["max_k"] for p in per_step)),
             "sparsity_utilisation": float(np.mean([p["mean_k"] / max(p["max_k"], 1) for p in per_step])),
             "stages_us": stage_us, "stages_sum_us": float(sum(stage_us.values())),
+            "unfused_five_calls_us": unfused_us,
+            "amortised": {"select_interval": SI, "us_per_layer_step": amortised_us,
+                          "note": "compression every select_interval steps as in the paper (L274); the other steps "
+                                  "append and attend over the previous selected tier"},
             "roofline": roof,
             "e2e": {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "us_per_layer_step": ms_e2e / K * 1e3, "sync": "stream sync after every step"},
@@ -357,6 +383,7 @@ def main():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2: the target config)")
     ap.add_argument("--ref-batch", type=int, default=4, help="sequences in the oracle's bounded sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--select-interval", type=int, default=128, help="interval of the amortised context line (paper: 128)")
     ap.add_argument("--eager", action="store_true", help="time eager launches instead of one captured CUDA graph of the K steps")
     ap.add_argument("--layers", type=int, default=0, help="layers of distinct KV data cycled per step (0: 32 for config 1 whose "
                     "single-layer K fits L2, else 1)")
