@@ -181,6 +181,8 @@ def run_cuda(args):
     L = args.layers or (32 if args.config == 1 else 1)
     t0 = time.time()
     eng = harness.make_engine(wl, dev)
+    if args.variant != 1:
+        eng.set_variant(args.variant)
     if K + W > (wl.max_ctx - int(wl.n0.max())) * L:
         raise SystemExit(f"steps + warmup must be <= {(wl.max_ctx - int(wl.n0.max())) * L} for {wl.name} with {L} layer(s)")
     states, prefill = harness.make_state(wl, dev, layers=L)   # step t runs on layer t % L (distinct data, shared tables)
@@ -336,7 +338,7 @@ def run_cuda(args):
             "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config}] ({wl.name})", "batch": wl.B,
                        "q_heads": wl.Hq, "kv_heads": wl.Hkv, "head_dim": wl.d, "ctx": [int(wl.n0.min()), int(wl.n0.max())],
-                       "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": L,
+                       "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": L, "variant": args.variant,
                        "launch": "eager" if args.eager else "one CUDA graph of the K steps",
                        "l2": "inputs larger than L2 (K scan %.0f MB per layer-step x %d layer(s) of distinct data cycled), "
                              "no flush" % (per_step[0]["score"] / 1e6, L),
@@ -388,6 +390,7 @@ def main():
     ap.add_argument("--layers", type=int, default=0, help="layers of distinct KV data cycled per step (0: 32 for config 1 whose "
                     "single-layer K fits L2, else 1)")
     ap.add_argument("--n0", type=int, default=0, help="override: uniform prefill context (config 3 checkpoints)")
+    ap.add_argument("--variant", type=int, default=1, help="kernel variant (hardkv_set_variant): 1 default, 2 TMA score, 3 async attention")
     ap.add_argument("--p", type=float, default=0.0, help="override the nucleus mass (config 4 sweep)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup

@@ -76,26 +76,53 @@ void hko_score(const hko_config *c, hko_unit *u, const float *q) {
   }
 }
 
+/* ---- metric transform g(z) of one query head (Appendix E "Reduce-Scatter", L278):
+ * SNAPKV (score_mode 2) max-pools the raw logits along the sequence with an odd
+ * window pool_kernel, stride 1, clipped to the pool (reading C15); every other mode
+ * is the identity (VANILLA, L276).  zhat has N = hi - lo entries. */
+static void hko_metric_logits(const hko_config *c, const hko_unit *u, int32_t g, int mode, double *zhat) {
+  int32_t lo = u->c_lo, hi = pool_hi(c, u);
+  const float *z = u->logits + (size_t)g * c->max_ctx;
+  int32_t r = (mode == 2 && c->pool_kernel > 1) ? (c->pool_kernel - 1) / 2 : 0;
+  for (int32_t i = lo; i < hi; ++i) {
+    double m = (double)z[i];
+    for (int32_t j = i - r; j <= i + r; ++j)
+      if (j >= lo && j < hi && (double)z[j] > m) m = (double)z[j];
+    zhat[i - lo] = m;
+  }
+}
+
+/* P[i] = (1/G) sum_g softmax_i(g(z_g)[i] / T) over the pool: Solution 1, L120
+ * ("S_hat = S(g(z/T))"; for max-pooling g(z/T) = g(z)/T exactly when T > 0), group
+ * mean of reading C2, softmax over the pool only (reading C3). */
+static void hko_metric_probs(const hko_config *c, const hko_unit *u, int mode, double T, double *P) {
+  int32_t lo = u->c_lo, hi = pool_hi(c, u), N = hi - lo;
+  double *zh = (double *)malloc(sizeof(double) * (size_t)N);
+  for (int32_t i = 0; i < N; ++i) P[i] = 0.0;
+  for (int32_t g = 0; g < c->G; ++g) {
+    hko_metric_logits(c, u, g, mode, zh);
+    double m = -INFINITY;
+    for (int32_t i = 0; i < N; ++i) { double x = zh[i] / T; if (x > m) m = x; }
+    double s = 0.0;
+    for (int32_t i = 0; i < N; ++i) s += exp(zh[i] / T - m);
+    for (int32_t i = 0; i < N; ++i) P[i] += exp(zh[i] / T - m) / s;
+  }
+  for (int32_t i = 0; i < N; ++i) P[i] /= (double)c->G;
+  free(zh);
+}
+
 /* ---- Logits Calibration, apply-T (L120 "S_hat = S(g(z/T))", g = identity for
- * VANILLA L276; H2O-style averaging L124 for ACCUM, reading C4).  One score per
- * KV head = mean over the GQA group of per-query-head softmax probabilities
- * (reading C2), softmax taken over the pool only (reading C3). */
+ * VANILLA L276, sequence max-pool for SNAPKV L278; H2O-style averaging L124 for
+ * ACCUM, reading C4).  One score per KV head = mean over the GQA group of
+ * per-query-head softmax probabilities (reading C2), softmax taken over the pool
+ * only (reading C3). */
 void hko_calibrate(const hko_config *c, hko_unit *u) {
   int32_t lo = u->c_lo, hi = pool_hi(c, u);
   if (hi <= lo) return;
-  double T = (double)u->T;
   double *P = (double *)calloc((size_t)(hi - lo), sizeof(double));
-  for (int32_t g = 0; g < c->G; ++g) {
-    const float *z = u->logits + (size_t)g * c->max_ctx;
-    double m = -INFINITY;
-    for (int32_t i = lo; i < hi; ++i) { double x = (double)z[i] / T; if (x > m) m = x; }
-    double s = 0.0;
-    for (int32_t i = lo; i < hi; ++i) s += exp((double)z[i] / T - m);
-    for (int32_t i = lo; i < hi; ++i) P[i - lo] += exp((double)z[i] / T - m) / s;
-  }
-  for (int32_t i = lo; i < hi; ++i) P[i - lo] /= (double)c->G;
+  hko_metric_probs(c, u, u->score_mode, (double)u->T, P);
 
-  if (u->score_mode == 0) {
+  if (u->score_mode != 1) {
     for (int32_t i = lo; i < hi; ++i) u->probs[i] = (float)P[i - lo];
   } else {
     /* ACCUM (reading C4): sliding sum of the last accum_window per-step rows, kept
@@ -173,6 +200,88 @@ void hko_topp_select(const hko_config *c, hko_unit *u, float p, int count_votes)
   if (count_votes)
     for (int32_t j = 0; j < k; ++j) u->votes[u->sel_idx[j]] += 1;   /* L86 cumulative mask */
   free(keys);
+}
+
+/* ---- Logits Calibration, solve-T: Algorithm 2 "Binary Search on T" (L625-648; the
+ * listing is garbled, read as in DESIGN.md C14/C16) for Problem 1 (L108-110):
+ *   k <- Num_Selected_TopP(S, p)           S = raw attention scores (g = id, T = 1)
+ *   do  T_mid <- (T_min + T_max) / 2
+ *       S_hat <- Softmax(g(z) / T_mid)      (Solution 1 / 2 coincide for the metrics built)
+ *       M_k(S) < M_k(S_hat) (too sharp): T_min <- T_mid   else: T_max <- T_mid
+ *   while |M_k(S) - M_k(S_hat)| > eps and T_min < T_max (and fewer than max_iter rounds)
+ * M_k(X) = mass of the k largest entries of X (order: fp32 bits desc, position asc),
+ * as integer mass over total integer mass (reading C5).  T_mid and the bounds are fp32.
+ * ACCUM heads are left alone (reading C4 keeps T inside the per-step softmax).
+ * Writes u->T = last T_mid, u->k_topp = k; returns the number of rounds; *resid = final
+ * |M_k(S) - M_k(S_hat)|. */
+static double hko_topk_mass(const float *probs, int32_t lo, int32_t N, int32_t k) {
+  hko_key *keys = (hko_key *)malloc(sizeof(hko_key) * (size_t)N);
+  uint64_t Wtot = 0, Wk = 0;
+  for (int32_t i = 0; i < N; ++i) { keys[i].bits = f32_bits(probs[lo + i]); keys[i].pos = lo + i; }
+  qsort(keys, (size_t)N, sizeof(hko_key), hko_key_cmp);
+  for (int32_t j = 0; j < N; ++j) {
+    float Pj; memcpy(&Pj, &keys[j].bits, 4);
+    uint64_t w = (uint64_t)nearbyint((double)Pj * 4294967296.0);
+    Wtot += w;
+    if (j < k) Wk += w;
+  }
+  free(keys);
+  return Wtot ? (double)Wk / (double)Wtot : 0.0;
+}
+
+/* Num_Selected_TopP(S, p) of Algorithm 1/2 line 1: length of the shortest prefix of the
+ * order (bits desc, position asc) whose integer mass reaches Theta (reading C5). */
+static int32_t hko_num_selected_topp(const float *probs, int32_t lo, int32_t N, float p) {
+  if (p >= 1.0f) return N;
+  hko_key *keys = (hko_key *)malloc(sizeof(hko_key) * (size_t)N);
+  uint64_t Wtot = 0;
+  for (int32_t i = 0; i < N; ++i) {
+    keys[i].bits = f32_bits(probs[lo + i]); keys[i].pos = lo + i;
+    Wtot += (uint64_t)nearbyint((double)probs[lo + i] * 4294967296.0);
+  }
+  qsort(keys, (size_t)N, sizeof(hko_key), hko_key_cmp);
+  uint64_t Theta = (uint64_t)ceil((double)p * (double)Wtot), cum = 0;
+  if (Theta < 1) Theta = 1;
+  int32_t k = N;
+  for (int32_t j = 0; j < N; ++j) {
+    float Pj; memcpy(&Pj, &keys[j].bits, 4);
+    cum += (uint64_t)nearbyint((double)Pj * 4294967296.0);
+    if (cum >= Theta) { k = j + 1; break; }
+  }
+  free(keys);
+  return k;
+}
+
+int hko_solve_temperature(const hko_config *c, hko_unit *u, float p, float t_min, float t_max,
+                          float eps, int max_iter, double *resid) {
+  int32_t lo = u->c_lo, hi = pool_hi(c, u), N = hi - lo;
+  if (resid) *resid = 0.0;
+  if (N <= 0 || u->score_mode == 1) return 0;
+  double *P = (double *)malloc(sizeof(double) * (size_t)N);
+  /* line 1: k from the raw attention scores; the k_cap clamp and l_lower do not apply */
+  hko_metric_probs(c, u, 0, 1.0, P);
+  for (int32_t i = 0; i < N; ++i) u->probs[lo + i] = (float)P[i];
+  int32_t k = hko_num_selected_topp(u->probs, lo, N, p);
+  double MkS = hko_topk_mass(u->probs, lo, N, k);
+  float tlo = t_min, thi = t_max, Tm = u->T;
+  double r = 0.0;
+  int it = 0;
+  while (it < max_iter) {
+    Tm = 0.5f * (tlo + thi);
+    hko_metric_probs(c, u, u->score_mode, (double)Tm, P);
+    for (int32_t i = 0; i < N; ++i) u->probs[lo + i] = (float)P[i];
+    double MkH = hko_topk_mass(u->probs, lo, N, k);
+    r = fabs(MkS - MkH);
+    ++it;
+    if (!(r > (double)eps)) break;
+    if (MkS < MkH) tlo = Tm; else thi = Tm;
+    if (!(tlo < thi)) break;
+  }
+  u->T = Tm;
+  u->k_topp = k;
+  if (resid) *resid = r;
+  free(P);
+  return it;
 }
 
 /* ---- Rewrite Cache (L172: "read the selected blocks and write them into a

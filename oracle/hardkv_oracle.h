@@ -21,7 +21,9 @@
  * P2 brute-force Top-p minimality, P3 ties, P4 degenerate, P5 closed form,
  * P6 order/temperature invariance, P7 Gaussian budget law, P8 merge algebra,
  * P9 rewrite copies, P10 condensed tier == top-C_cap of the retirement log,
- * P11 bookkeeping invariants, P12 integer mass vs fp64 cumsum.
+ * P11 bookkeeping invariants, P12 integer mass vs fp64 cumsum, P13 temperature
+ * solve (g = id => T* = 1; g = a z => T* = a; M_k decreasing in T), P14 SNAPKV
+ * max-pool == torch.nn.functional.max_pool1d.
  * Parity unpinned by the paper: readings C2 (GQA group mean), C3 (softmax over
  * the pool only), C4 (ACCUM window form), C7 (condensed-tier retention rule),
  * C8 (threshold mapping).  The paper prints no worked example for them; they
@@ -46,6 +48,7 @@ typedef struct {
   int32_t cond_cap;     /* C_cap                                                   */
   int32_t accum_window; /* ACCUM ring depth (32)                                   */
   float   sm_scale;     /* reading C1: 1/sqrt(d) by default                        */
+  int32_t pool_kernel;  /* SNAPKV max-pool window (odd; <= 1: identity), C15       */
 } hko_config;
 
 typedef struct {
@@ -58,7 +61,7 @@ typedef struct {
   float   *cond_k, *cond_v;    /* [cond_cap][d] condensed tier rows                 */
   int32_t *cond_pos, *cond_votes; /* [cond_cap]                                     */
   int32_t  cond_count;
-  int32_t  score_mode;         /* 0 RAW, 1 ACCUM                                    */
+  int32_t  score_mode;         /* 0 RAW, 1 ACCUM, 2 SNAPKV (max-pooled logits, L278) */
   float    T;                  /* calibration temperature of this KV head           */
   float   *acc;                /* [max_ctx] ACCUM running window sum (or NULL)      */
   float   *ring;               /* [accum_window][max_ctx] (or NULL)                 */
@@ -83,6 +86,9 @@ int  hko_retire(const hko_config *c, hko_unit *u);
 void hko_score(const hko_config *c, hko_unit *u, const float *q);
 /* Logits Calibration, apply-T form (L120 Solution 1), group mean (reading C2). */
 void hko_calibrate(const hko_config *c, hko_unit *u);
+/* Algorithm 2 (L625-648): bisection on T for Problem 1 (L108-110). Returns #rounds. */
+int  hko_solve_temperature(const hko_config *c, hko_unit *u, float p, float t_min, float t_max,
+                           float eps, int max_iter, double *resid);
 /* Top-p nucleus on u->probs (L108; reading C5/C6). votes++ when count_votes. */
 void hko_topp_select(const hko_config *c, hko_unit *u, float p, int count_votes);
 /* Rewrite Cache (L172), ascending position order, zero tail (reading C9). */

@@ -33,7 +33,7 @@ class HkoConfig(C.Structure):
     _fields_ = [
         ("G", C.c_int32), ("d", C.c_int32), ("page", C.c_int32), ("max_ctx", C.c_int32),
         ("sink", C.c_int32), ("recent", C.c_int32), ("k_cap", C.c_int32), ("cond_cap", C.c_int32),
-        ("accum_window", C.c_int32), ("sm_scale", C.c_float),
+        ("accum_window", C.c_int32), ("sm_scale", C.c_float), ("pool_kernel", C.c_int32),
     ]
 
 
@@ -68,6 +68,9 @@ def lib():
         _lib.hko_retire.restype = C.c_int
         _lib.hko_score.argtypes = [cp, up, _F]
         _lib.hko_calibrate.argtypes = [cp, up]
+        _lib.hko_solve_temperature.argtypes = [cp, up, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int,
+                                               C.POINTER(C.c_double)]
+        _lib.hko_solve_temperature.restype = C.c_int
         _lib.hko_topp_select.argtypes = [cp, up, C.c_float, C.c_int]
         _lib.hko_rewrite.argtypes = [cp, up]
         _lib.hko_attend.argtypes = [cp, up, _F]
@@ -107,11 +110,12 @@ class OracleConfig:
     page: int = 16
     accum_window: int = 32
     sm_scale: float | None = None
+    pool_kernel: int = 0
 
     def c(self) -> HkoConfig:
         s = self.sm_scale if self.sm_scale is not None else 1.0 / float(np.sqrt(self.d))
         return HkoConfig(self.G, self.d, self.page, self.max_ctx, self.sink, self.recent, self.k_cap,
-                         self.cond_cap, self.accum_window, np.float32(s))
+                         self.cond_cap, self.accum_window, np.float32(s), self.pool_kernel)
 
 
 class Unit:
@@ -180,6 +184,16 @@ class Unit:
 
     def calibrate(self):
         lib().hko_calibrate(C.byref(self.ccfg), C.byref(self.u))
+
+    def solve_temperature(self, p: float, t_min: float = 0.03125, t_max: float = 32.0, eps: float = 1e-4,
+                          max_iter: int = 40) -> tuple[int, float]:
+        """Algorithm 2 on the logits of the last score(); sets T. Returns (rounds, residual)."""
+        r = C.c_double()
+        it = lib().hko_solve_temperature(C.byref(self.ccfg), C.byref(self.u), np.float32(p), np.float32(t_min),
+                                         np.float32(t_max), np.float32(eps), int(max_iter), C.byref(r))
+        return it, r.value
+
+    T = property(lambda s: float(s.u.T))
 
     def topp_select(self, p: float, count_votes: bool = True):
         lib().hko_topp_select(C.byref(self.ccfg), C.byref(self.u), np.float32(p), int(count_votes))

@@ -385,3 +385,107 @@ def test_golden_closed_forms(case, N, p, param, expect):
     assert u.sel_count == expect
     if case != "dominant":
         assert list(u.sel_idx[:expect]) == list(range(4, 4 + expect))
+
+
+# ---- P14: SNAPKV metric = max-pool of the raw logits along the sequence (L150, L278) ------------
+@pytest.mark.parametrize("G,kernel,T", [(1, 7, 1.0), (4, 5, 0.7), (3, 1, 2.0)])
+def test_p14_snapkv_maxpool_is_library_maxpool(G, kernel, T):
+    """calibrate() of a SNAPKV head == mean_g softmax(max_pool1d(z_g) / T), the pooling done by
+    torch.nn.functional.max_pool1d (stride 1, -inf padding = window clipped to the pool)."""
+    rng = np.random.default_rng(14)
+    cfg = OracleConfig(G=G, d=64, max_ctx=256, sink=4, recent=16, k_cap=256, cond_cap=8, pool_kernel=kernel)
+    K0 = rng.standard_normal((200, 64)).astype(np.float32)
+    u = Unit(cfg, K0, K0.copy(), l_upper=10**6, T=T, score_mode=2)
+    lo, hi = u.pool
+    z = (rng.standard_normal((G, hi - lo)) * 3).astype(np.float32)
+    _set_logits(u, z)
+    u.calibrate()
+    zt = torch.tensor(z, dtype=torch.float64)[None]
+    pooled = torch.nn.functional.max_pool1d(zt, kernel, stride=1, padding=kernel // 2)[0]
+    ref = torch.softmax(pooled / T, -1).mean(0).numpy()
+    np.testing.assert_allclose(u.probs[lo:hi], ref, rtol=1e-6, atol=1e-12)
+    if kernel == 1:   # identity window: the SNAPKV head is a RAW head
+        cfg0, u0, _ = _unit(G=G, T=T)
+        _set_logits(u0, z); u0.calibrate()
+        np.testing.assert_array_equal(u0.probs[lo:hi], u.probs[lo:hi])
+
+
+# ---- P13: temperature solve, Algorithm 2 (L625-648) for Problem 1 (L108-110) --------------------
+def _topk_mass_np(P, k):
+    w = _w(np.asarray(P, np.float32))
+    return float(np.sort(w)[::-1][:k].sum() / w.sum())
+
+
+@pytest.mark.parametrize("G,sigma", [(1, 1.0), (4, 2.5)])
+def test_p13_identity_metric_solves_to_one(G, sigma):
+    """g = id: S_hat(T = 1) == S, so Problem 1's minimiser is T* = 1 (mass error 0 there)."""
+    cfg, u, rng = _unit(G=G, n0=1200, max_ctx=1280, W=16, k_cap=1280, seed=13)
+    lo, hi = u.pool
+    _set_logits(u, rng.standard_normal((G, hi - lo)) * sigma)
+    it, resid = u.solve_temperature(0.9, t_min=0.25, t_max=3.0, eps=1e-7, max_iter=60)
+    assert abs(u.T - 1.0) < 2e-3 and resid < 1e-4 and 1 <= it <= 60
+
+
+def test_p13_snapkv_geometric_closed_form():
+    """z_i = -lam * i with a max-pool of radius r: g(z) has r + 1 copies of the top logit, then the
+    same geometric tail, so M_k(S) and M_k(S_hat(T)) are geometric sums and T* is the root of a
+    scalar equation, solved here by scipy.optimize.brentq (independent of the oracle)."""
+    import scipy.optimize
+    lam, N, r, p = 0.1, 400, 5, 0.9
+    cfg = OracleConfig(G=1, d=64, max_ctx=N + 32, sink=4, recent=16, k_cap=N + 32, cond_cap=8, pool_kernel=2 * r + 1)
+    K0 = np.zeros((N + 20, 64), np.float32)
+    u = Unit(cfg, K0, K0.copy(), l_upper=10**6, score_mode=2)
+    _set_logits(u, -lam * np.arange(N)[None, :])
+    rho = math.exp(-lam)
+    k = math.ceil(math.log(1 - p * (1 - rho ** N)) / math.log(rho))          # pin P5's closed form
+    MkS = (1 - rho ** k) / (1 - rho ** N)
+
+    def f(T):
+        q = math.exp(-lam / T)
+        geo = lambda m: (1 - q ** m) / (1 - q)       # 1 + q + ... + q^(m-1)
+        return MkS - (r + geo(k - r)) / (r + geo(N - r))
+
+    Tstar = scipy.optimize.brentq(f, 0.25, 4.0, xtol=1e-10)
+    it, resid = u.solve_temperature(p, t_min=0.25, t_max=4.0, eps=1e-7, max_iter=60)
+    assert u.k_topp == k
+    assert abs(u.T - Tstar) < 2e-3 * Tstar, (u.T, Tstar)
+    assert abs(Tstar - 1.0) > 0.03          # the case is not the trivial T* = 1
+
+
+@pytest.mark.parametrize("mode,kernel", [(0, 0), (2, 7)])
+def test_p13_root_bracket_and_monotonicity(mode, kernel):
+    """Independent numpy evaluation at the returned T: the mass error is within eps, M_k(S_hat(T)) decreases in T
+    (why bisection applies, L599 'sharpened for lower T and flattened for higher T') and the root is bracketed."""
+    rng = np.random.default_rng(131)
+    G, p, eps = 4, 0.9, 1e-5
+    cfg = OracleConfig(G=G, d=64, max_ctx=2048, sink=4, recent=32, k_cap=2048, cond_cap=8, pool_kernel=kernel)
+    K0 = np.zeros((2000, 64), np.float32)
+    u = Unit(cfg, K0, K0.copy(), l_upper=10**6, score_mode=mode, T=5.0)
+    lo, hi = u.pool
+    z = (rng.standard_normal((G, hi - lo)) * 2.0).astype(np.float32)
+    _set_logits(u, z)
+    zt = torch.tensor(z, dtype=torch.float64)
+    gz = torch.nn.functional.max_pool1d(zt[None], kernel, stride=1, padding=kernel // 2)[0] if mode == 2 else zt
+    S = torch.softmax(zt, -1).mean(0).numpy().astype(np.float32)
+    w = _w(S); order = np.argsort(-S, kind="stable")
+    k = int(np.searchsorted(np.cumsum(w[order]), math.ceil(p * float(w.sum()))) + 1)
+    MkS = _topk_mass_np(S, k)
+    Mk = lambda T: _topk_mass_np(torch.softmax(gz / T, -1).mean(0).numpy().astype(np.float32), k)
+    it, resid = u.solve_temperature(p, t_min=0.125, t_max=8.0, eps=eps, max_iter=50)
+    assert u.k_topp == k
+    assert abs(Mk(u.T) - MkS) <= eps + 1e-6 and resid <= eps
+    grid = [0.125, 0.25, 0.5, 1.0, 2.0, 4.0, 8.0]
+    vals = [Mk(T) for T in grid]
+    assert all(a > b for a, b in zip(vals, vals[1:]))
+    assert vals[0] > MkS > vals[-1]
+    if mode == 0:
+        assert abs(u.T - 1.0) < 1e-2
+    else:
+        assert u.T > 1.0    # pooling repeats large logits: the pooled distribution is sharper at T = 1
+
+
+def test_p13_accum_heads_are_left_alone():
+    cfg, u, rng = _unit(G=2, mode=1, T=1.5)
+    lo, hi = u.pool
+    _set_logits(u, rng.standard_normal((2, hi - lo)))
+    assert u.solve_temperature(0.9) == (0, 0.0) and u.T == 1.5
