@@ -481,7 +481,7 @@ def test_p13_root_bracket_and_monotonicity(mode, kernel):
     if mode == 0:
         assert abs(u.T - 1.0) < 1e-2
     else:
-        assert u.T > 1.0    # pooling repeats large logits: the pooled distribution is sharper at T = 1
+        assert u.T < 1.0    # maxima of 7 iid logits spread less (std ~0.6 sigma): flatter at T = 1, so T* < 1
 
 
 def test_p13_accum_heads_are_left_alone():
