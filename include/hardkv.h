@@ -56,7 +56,9 @@ typedef enum {
 } hardkv_status;
 
 typedef enum { HARDKV_F32 = 0, HARDKV_BF16 = 1 } hardkv_dtype;
-typedef enum { HARDKV_SCORE_RAW = 0, HARDKV_SCORE_ACCUM = 1 } hardkv_score_mode;
+/* Importance metric of a KV head (L276-278): raw attention logits (VANILLA), accumulated attention over the
+ * last accum_window steps (H2O-style, L124), or logits max-pooled along the sequence (SNAPKV, L150 / L278). */
+typedef enum { HARDKV_SCORE_RAW = 0, HARDKV_SCORE_ACCUM = 1, HARDKV_SCORE_SNAPKV = 2 } hardkv_score_mode;
 
 /* Static for the lifetime of a ctx (and of any graph captured with it). */
 typedef struct {
@@ -68,6 +70,8 @@ typedef struct {
   int32_t accum_window;   /* ring depth of SCORE_ACCUM heads (<= 0: no ACCUM state)                 */
   int32_t kv_dtype;       /* hardkv_dtype of q, K, V                                                */
   float   sm_scale;       /* <= 0: 1/sqrt(head_dim)                                                 */
+  int32_t pool_kernel;    /* SNAPKV max-pool window: odd, 3..63; 0 or 1: the config has no SNAPKV   */
+                          /* head (the pooling pass is not launched)                                */
 } hardkv_config;
 
 /* Caller-owned device state of one layer.  Pointers marked (opt) may be NULL. */
@@ -77,7 +81,8 @@ typedef struct {
   void *cond_k, *cond_v;            int32_t *cond_pos, *cond_votes, *cond_count; /* [B][Hkv][C], [B][Hkv]  */
   int32_t *ctx_len, *c_lo;          const int32_t *l_lower, *l_upper;           /* [B] each               */
   int32_t *votes;                                                               /* [B][Hkv][max_ctx]      */
-  const float *temperature;         const uint8_t *score_mode;                  /* [B][Hkv], [Hkv]        */
+  const float *temperature;         const uint8_t *score_mode;                  /* [B][Hkv], [Hkv]; temperature is
+                                                                                   written by hardkv_solve_temperature only */
   float *acc, *ring;                int32_t *ring_slot;  /* (opt) ACCUM: [B][Hkv][max_ctx], [B][Hkv][win][max_ctx], [B][Hkv] */
   int32_t *sel_idx, *sel_count, *sel_table;  /* [B][Hkv][k_cap] asc. positions pad -1, [B][Hkv], [B][Hkv][k_cap/page] */
   uint8_t *sel_mask;                /* (opt) [B][Hkv][max_ctx/8], bit i%8 of byte i/8 (L439)                */
@@ -103,8 +108,18 @@ hardkv_status hardkv_append_kv(hardkv_ctx *, const hardkv_state *, const void *k
                                hardkv_stream);
 /* logits[b][h*G+g][i] = sm_scale * q . K[i] over the pool (exponent of Eq. 4). */
 hardkv_status hardkv_score(hardkv_ctx *, const hardkv_state *, const void *q, hardkv_stream);
-/* Logits Calibration (apply-T) -> probs, then hardkv_topp_select. */
+/* Logits Calibration (apply-T) -> probs, then hardkv_topp_select.  SNAPKV heads (cfg.pool_kernel > 1)
+ * are calibrated on their logits max-pooled along the sequence, window clipped to the pool (L278). */
 hardkv_status hardkv_calibrate_topp(hardkv_ctx *, const hardkv_state *, float p, hardkv_stream);
+/* Logits Calibration, solve-T: Algorithm 2 "Binary Search on T" (L625-648) for Problem 1 (L108-110), run at a
+ * request's first compression (L607).  Needs state->logits of a preceding hardkv_score.  Per (b, KV head):
+ * k = Num_Selected_TopP(S, p) with S the raw attention scores (group mean of softmax(z), T = 1, no k_cap clamp);
+ * then T_mid = (T_min + T_max) / 2, S_hat = calibrated metric at T_mid, M_k = integer mass of the k largest
+ * probabilities over the total; M_k(S) < M_k(S_hat) raises T_min, else lowers T_max; stops when
+ * |M_k(S) - M_k(S_hat)| <= eps, T_min >= T_max or after max_iter rounds.  Writes the last T_mid to
+ * state->temperature[b][h] (ACCUM heads and empty pools are left unchanged); state->probs is used as scratch. */
+hardkv_status hardkv_solve_temperature(hardkv_ctx *, const hardkv_state *, float p, float t_min, float t_max,
+                                       float eps, int32_t max_iter, hardkv_stream);
 /* Top-p nucleus (L108) on state->probs as given: integer mass w_i = rn(P_i 2^32),
  * order (P bits desc, position asc), minimal prefix with mass >= ceil(p * sum w),
  * clamped to k_cap (L233).  Writes sel_idx, sel_count, sel_table, (sel_mask), votes += 1.

@@ -11,6 +11,7 @@
 #include "select_kernel.cuh"
 #include "stage_kernels.cuh"
 #include "attend_mma.cuh"
+#include "metric_kernels.cuh"
 
 using namespace hardkv;
 
@@ -29,7 +30,7 @@ namespace {
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout { size_t part, arrive, stats, stage_q, stage_k, stage_v, stage_out, total; };
+struct WsLayout { size_t part, arrive, stats, stage_q, stage_k, stage_v, stage_out, pooled, total; };
 
 size_t esize_of(const hardkv_config &c) { return c.kv_dtype == HARDKV_F32 ? 4 : 2; }
 
@@ -54,6 +55,7 @@ WsLayout ws_layout(const hardkv_config &c) {
   w.stage_k = off;   off += align256(kb * esize_of(c));
   w.stage_v = off;   off += align256(kb * esize_of(c));
   w.stage_out = off; off += align256(qb * sizeof(float));
+  w.pooled = off;    off += c.pool_kernel > 1 ? align256((size_t)c.batch * c.num_q_heads * c.max_ctx * sizeof(float)) : 0;
   w.total = off;
   return w;
 }
@@ -84,6 +86,7 @@ hardkv_status check_config(const hardkv_config *c) {
   if (c->max_ctx <= 0 || c->k_cap <= 0 || c->sink < 0 || c->recent < 0 || c->cond_cap < 0) return HARDKV_ERR_INVALID_ARG;
   if (c->page_size != PAGE) return HARDKV_ERR_UNSUPPORTED;
   if (c->max_ctx % PAGE || c->k_cap % PAGE) return HARDKV_ERR_INVALID_ARG;
+  if (c->pool_kernel < 0 || c->pool_kernel > 63 || (c->pool_kernel > 1 && c->pool_kernel % 2 == 0)) return HARDKV_ERR_INVALID_ARG;
   const int G = c->num_q_heads / c->num_kv_heads;
   const bool gok = G == 1 || G == 2 || G == 4 || G == 5 || G == 7 || G == 8;
   const bool tok = (c->kv_dtype == HARDKV_F32 && c->head_dim == 64) ||
@@ -181,6 +184,14 @@ void launch_select(hardkv_ctx *ctx, const Params &P, float p, int calibrate, cud
   }
 }
 
+// SNAPKV metric transform (L278): only configs that declare a pooling window pay for the launch
+void launch_pool(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
+  if (P.pool_kernel <= 1) return;
+  ctx->launches += 1;
+  dim3 grid((P.max_ctx + POOL_TOK - 1) / POOL_TOK, P.B * P.Hkv);
+  maxpool_kernel<<<grid, 256, 0, st>>>(P);
+}
+
 void launch_rewrite(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
   ctx->launches += 1;
   dim3 grid((P.k_cap + RW_ROWS_PER_CTA - 1) / RW_ROWS_PER_CTA, P.B * P.Hkv);
@@ -256,6 +267,8 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.part = reinterpret_cast<float *>(base + w.part);
   P.score_stats = reinterpret_cast<float2 *>(base + w.stats);
   P.score_chunks = score_chunks_of(*cfg);
+  P.pool_kernel = cfg->pool_kernel;
+  P.pooled = cfg->pool_kernel > 1 ? reinterpret_cast<float *>(base + w.pooled) : nullptr;
   ctx->stage_q = base + w.stage_q; ctx->stage_k = base + w.stage_k; ctx->stage_v = base + w.stage_v;
   ctx->stage_out = reinterpret_cast<float *>(base + w.stage_out);
   select_geometry(*cfg, &P.sel_cluster, &P.sel_slice_cap);
@@ -316,7 +329,19 @@ static bool accum_ok(const hardkv_ctx *ctx, const hardkv_state *s) {
 
 hardkv_status hardkv_calibrate_topp(hardkv_ctx *ctx, const hardkv_state *s, float p, hardkv_stream st) {
   if (!state_ok(ctx, s) || !(p > 0.f) || !accum_ok(ctx, s)) return HARDKV_ERR_INVALID_ARG;
+  launch_pool(ctx, params_of(ctx, s), st);
   launch_select(ctx, params_of(ctx, s), p, 1, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_solve_temperature(hardkv_ctx *ctx, const hardkv_state *s, float p, float t_min, float t_max,
+                                       float eps, int32_t max_iter, hardkv_stream st) {
+  if (!state_ok(ctx, s) || !(p > 0.f) || !(t_min > 0.f) || !(t_max > t_min) || !(eps >= 0.f) || max_iter < 1)
+    return HARDKV_ERR_INVALID_ARG;
+  const Params P = params_of(ctx, s);
+  launch_pool(ctx, P, st);
+  ctx->launches += 1;
+  solve_temperature_kernel<<<P.B * P.Hkv, SOLVE_NT, 0, st>>>(P, p, t_min, t_max, eps, max_iter);
   return launch_status();
 }
 
@@ -357,7 +382,9 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   launch_append(ctx, P, k_new, v_new, st);
   if (do_select) {
     launch_score(ctx, P, q, st);
-    launch_select(ctx, P, p, fast_path(ctx) ? 2 : 1, st);
+    launch_pool(ctx, P, st);
+    // the score kernel's chunk statistics describe the raw logits: configs with pooled heads take them in-kernel
+    launch_select(ctx, P, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
   }
   launch_attend(ctx, P, q, out, lse, do_select != 0, st);
   return launch_status();

@@ -115,7 +115,9 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
   if (CALIBRATE) {
     // softmax in the base-2 domain: exp(z/T - m) = 2^(z*c2 - m2), c2 = log2(e)/T (one FFMA + one MUFU.EX2)
     const float c2 = 1.4426950408889634f / P.st.temperature[unit];
-    const float *lg = P.st.logits + ((size_t)(b * P.Hq + h * G)) * P.max_ctx;
+    // SNAPKV heads calibrate the max-pooled copy of their logits (L278; metric_kernels.cuh), all others the raw logits
+    const float *lg = ((P.pool_kernel > 1 && P.st.score_mode[h] == HARDKV_SCORE_SNAPKV) ? P.pooled : P.st.logits) +
+                      ((size_t)(b * P.Hq + h * G)) * P.max_ctx;
     float mg[GMAX], rs[GMAX];
     if (CALIBRATE == 2) {
       // statistics were produced by the score kernel: one (m2, s) pair per query head and 512-token chunk

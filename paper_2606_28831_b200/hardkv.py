@@ -39,7 +39,7 @@ def build(force: bool = False) -> str:
 class Config(C.Structure):
     _fields_ = [(n, C.c_int32) for n in (
         "batch", "num_q_heads", "num_kv_heads", "head_dim", "page_size", "max_ctx", "sink", "recent", "k_cap",
-        "cond_cap", "accum_window", "kv_dtype")] + [("sm_scale", C.c_float)]
+        "cond_cap", "accum_window", "kv_dtype")] + [("sm_scale", C.c_float), ("pool_kernel", C.c_int32)]
 
 
 _STATE_FIELDS = ["k_pool", "v_pool", "base_table", "sel_k_pool", "sel_v_pool", "sel_pages", "cond_k", "cond_v",
@@ -54,7 +54,7 @@ class StateStruct(C.Structure):
 
 F32, BF16 = 0, 1
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
-           "hardkv_set_variant", "hardkv_append_kv", "hardkv_score", "hardkv_calibrate_topp",
+           "hardkv_set_variant", "hardkv_append_kv", "hardkv_score", "hardkv_calibrate_topp", "hardkv_solve_temperature",
            "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend",
            "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count"]
 
@@ -75,6 +75,7 @@ def _load():
     lib.hardkv_append_kv.argtypes = [vp, sp, vp, vp, vp]
     lib.hardkv_score.argtypes = [vp, sp, vp, vp]
     lib.hardkv_calibrate_topp.argtypes = [vp, sp, C.c_float, vp]
+    lib.hardkv_solve_temperature.argtypes = [vp, sp, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int32, vp]
     lib.hardkv_topp_select.argtypes = [vp, sp, C.c_float, vp]
     lib.hardkv_rewrite.argtypes = [vp, sp, vp]
     lib.hardkv_decode_attn.argtypes = [vp, sp, vp, vp, vp, vp]
@@ -132,9 +133,9 @@ class HardKV:
     """One hardkv_ctx.  Every method enqueues kernels on torch's current stream and returns at once."""
 
     def __init__(self, *, batch, num_q_heads, num_kv_heads, head_dim, max_ctx, sink, recent, k_cap, cond_cap,
-                 kv_dtype, accum_window=0, page_size=16, sm_scale=0.0, device="cuda:0"):
+                 kv_dtype, accum_window=0, page_size=16, sm_scale=0.0, pool_kernel=0, device="cuda:0"):
         self.cfg = Config(batch, num_q_heads, num_kv_heads, head_dim, page_size, max_ctx, sink, recent, k_cap,
-                          cond_cap, accum_window, kv_dtype, sm_scale)
+                          cond_cap, accum_window, kv_dtype, sm_scale, pool_kernel)
         nbytes = C.c_size_t()
         _check(lib.hardkv_workspace_bytes(C.byref(self.cfg), C.byref(nbytes)))
         self.workspace = torch.zeros(nbytes.value + 256, dtype=torch.uint8, device=device)
@@ -159,6 +160,12 @@ class HardKV:
 
     def calibrate_topp(self, st: DeviceState, p: float):
         _check(lib.hardkv_calibrate_topp(self._ctx, C.byref(st.struct()), np.float32(p), _stream()))
+
+    def solve_temperature(self, st: DeviceState, p: float, t_min: float = 0.03125, t_max: float = 32.0,
+                          eps: float = 1e-4, max_iter: int = 40):
+        """Algorithm 2 (L625-648) on the logits of the last score(); writes st.temperature."""
+        _check(lib.hardkv_solve_temperature(self._ctx, C.byref(st.struct()), np.float32(p), np.float32(t_min),
+                                            np.float32(t_max), np.float32(eps), int(max_iter), _stream()))
 
     def topp_select(self, st: DeviceState, p: float):
         _check(lib.hardkv_topp_select(self._ctx, C.byref(st.struct()), np.float32(p), _stream()))

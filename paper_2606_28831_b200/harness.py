@@ -21,7 +21,8 @@ def make_engine(wl: Workload, device="cuda:0", want_accum=None) -> hardkv.HardKV
     return hardkv.HardKV(batch=wl.B, num_q_heads=wl.Hq, num_kv_heads=wl.Hkv, head_dim=wl.d, max_ctx=wl.max_ctx,
                          sink=wl.sink, recent=wl.recent, k_cap=wl.k_cap, cond_cap=wl.cond_cap,
                          kv_dtype=hardkv.BF16 if wl.dtype == "bf16" else hardkv.F32,
-                         accum_window=wl.accum_window if accum else 0, sm_scale=float(wl.sm_scale), device=device)
+                         accum_window=wl.accum_window if accum else 0, sm_scale=float(wl.sm_scale),
+                         pool_kernel=wl.pool_kernel, device=device)
 
 
 def to_dev(x: np.ndarray, wl: Workload, device="cuda:0") -> torch.Tensor:

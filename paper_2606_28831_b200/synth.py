@@ -61,7 +61,7 @@ class Workload:
     cond_cap: int
     l_upper: np.ndarray              # [B]
     max_ctx: int
-    score_mode: np.ndarray           # [Hkv] uint8, 0 RAW / 1 ACCUM
+    score_mode: np.ndarray           # [Hkv] uint8, 0 RAW / 1 ACCUM / 2 SNAPKV
     tau_lo: float
     tau_hi: float
     planted: float = 0.05            # fraction of planted heavy hitters
@@ -69,6 +69,7 @@ class Workload:
     structured: bool = True          # False: config 0 (iid, per-q-head tau, key 0 x8)
     l_lower: np.ndarray = None       # [B]
     accum_window: int = 32
+    pool_kernel: int = 0             # SNAPKV max-pool window (odd; 0: no SNAPKV head)
     seed: int = 0
     temperature: np.ndarray = field(default=None)  # [B][Hkv] calibration T (reading C10: 1)
 

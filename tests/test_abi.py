@@ -32,7 +32,7 @@ def test_header_symbols_exported(lib):
 
 
 def test_struct_layout_matches_header(lib):
-    assert C.sizeof(lib.Config) == 13 * 4
+    assert C.sizeof(lib.Config) == 14 * 4
     assert C.sizeof(lib.StateStruct) == 28 * C.sizeof(C.c_void_p)
 
 
@@ -46,6 +46,11 @@ def test_host_only_validation(lib):
     assert lib.lib.hardkv_workspace_bytes(C.byref(bad_page), C.byref(n)) == 2
     bad_ctx = lib.Config(2, 32, 8, 128, 16, 4100, 4, 128, 1024, 256, 0, lib.BF16, 0.0)
     assert lib.lib.hardkv_workspace_bytes(C.byref(bad_ctx), C.byref(n)) == 1
+    even_pool = lib.Config(2, 32, 8, 128, 16, 4096, 4, 128, 1024, 256, 0, lib.BF16, 0.0, 6)  # SNAPKV window must be odd
+    assert lib.lib.hardkv_workspace_bytes(C.byref(even_pool), C.byref(n)) == 1
+    pooled = lib.Config(2, 32, 8, 128, 16, 4096, 4, 128, 1024, 256, 0, lib.BF16, 0.0, 7)
+    m = C.c_size_t()
+    assert lib.lib.hardkv_workspace_bytes(C.byref(pooled), C.byref(m)) == 0 and m.value >= n.value + 2 * 32 * 4096 * 4
     ctx = C.c_void_p()
     assert lib.lib.hardkv_create(C.byref(ok), None, 0, C.byref(ctx)) == 3                   # no workspace
     assert b"workspace" in lib.lib.hardkv_status_string(3)

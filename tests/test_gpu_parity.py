@@ -33,6 +33,11 @@ def small_workloads():
                                cond_cap=4, steps=4),
         "g2": make_workload(1, Hq=4, Hkv=2, n0=i32(640), max_ctx=656, k_cap=160, l_upper=i32(500), cond_cap=4,
                             steps=4),
+        # SNAPKV heads (logits max-pooled along the sequence, L278) mixed with RAW heads: G = 4 and G = 7
+        "snap4": make_workload(1, n0=i32(2100), max_ctx=2176, k_cap=512, l_upper=i32(1960), cond_cap=32, steps=6,
+                               score_mode=np.array([0, 2, 2, 0, 2, 0, 2, 2], np.uint8), pool_kernel=7),
+        "snap7": make_workload(3, B=2, n0=i32(1300, 1300), max_ctx=1536, k_cap=256, l_upper=i32(1100, 1100),
+                               cond_cap=8, steps=6, score_mode=np.array([2, 2, 0, 2], np.uint8), pool_kernel=5),
         "g8": make_workload(1, Hq=8, Hkv=1, n0=i32(1100), max_ctx=1120, k_cap=1120, l_upper=i32(5000), cond_cap=0,
                             steps=3),
     }
@@ -117,7 +122,7 @@ def test_fused_decode_step(name, teacher, P):
 
 
 @pytest.mark.parametrize("variant", [0, 2])
-@pytest.mark.parametrize("name", ["c1s", "c2s", "c3s", "c4s", "g1d64"])
+@pytest.mark.parametrize("name", ["c1s", "c2s", "c3s", "c4s", "g1d64", "snap4"])
 def test_kernel_variants(name, variant, P):
     """Variant 0 (generic fp32-FMA kernels) and variant 2 (TMA-staged persistent score) against the oracle."""
     wl = WL[name]
@@ -259,3 +264,41 @@ def test_error_paths(P):
     assert int(pr.st.err_flag.item()) == 1 and int(pr.st.ctx_len.item()) == 64
     with pytest.raises(hardkv.HardKVError):
         pr.eng.score(pr.st, None)
+
+
+@pytest.mark.parametrize("name", ["c1s", "c4s", "snap4", "snap7", "c0"])
+def test_solve_temperature(name, P):
+    """hardkv_solve_temperature (Algorithm 2) against the oracle's bisection on the same logits.
+    Floating point decides every branch of the search, so the unique thing compared is the root: T agrees to
+    1e-3 relative (both sides stop within eps = 1e-5 of mass error, which bounds T to ~1e-4 of the root);
+    ACCUM heads keep their T bit for bit.  The solved T then drives one calibrated selection step."""
+    wl = WL[name]
+    pr = P(wl, want_mask=False)
+    eng, st, ob = pr.eng, pr.st, pr.ob
+    q, kn, vn, (qd, knd, vnd) = pr.inputs(0)
+    eng.append_kv(st, knd, vnd)
+    eng.score(st, qd)
+    eng.solve_temperature(st, wl.p, t_min=0.0625, t_max=16.0, eps=1e-5, max_iter=40)
+    T_gpu = st.temperature.cpu().numpy().reshape(-1)
+    qu = q.reshape(-1, wl.G, wl.d)
+    for i, u in enumerate(ob.units):
+        u.append(kn.reshape(-1, wl.d)[i], vn.reshape(-1, wl.d)[i])
+        u.retire()
+        u.score(qu[i])
+        T0 = u.T
+        it, resid = u.solve_temperature(wl.p, t_min=0.0625, t_max=16.0, eps=1e-5, max_iter=40)
+        mode = int(wl.score_mode[i % wl.Hkv])
+        if mode == 1:
+            assert it == 0 and T_gpu[i] == np.float32(T0)
+        else:
+            assert resid <= 1e-5 and it >= 1
+            assert abs(T_gpu[i] - u.T) <= 1e-3 * u.T, (i, mode, T_gpu[i], u.T)
+            if mode == 0:
+                assert abs(T_gpu[i] - 1.0) < 5e-3          # g = id: T* = 1 (pin P13)
+        u.u.T = np.float32(T_gpu[i])                        # teacher-force T, then one calibrated selection
+    eng.calibrate_topp(st, wl.p)
+    for u in ob.units:
+        u.calibrate()
+        u.topp_select(wl.p, True)
+    pr.check_probs()
+    pr.check_selection_band()
