@@ -135,9 +135,22 @@ hardkv_status hardkv_decode_attn(hardkv_ctx *, const hardkv_state *, const void 
  * row is read once; same results as hardkv_rewrite followed by hardkv_decode_attn. */
 hardkv_status hardkv_rewrite_attend(hardkv_ctx *, const hardkv_state *, const void *q, float *out,
                                     float *lse /* nullable */, hardkv_stream);
-/* The whole step on one stream: append, retire, score, calibrate + Top-p, rewrite fused
- * with attention (selected rows are read once).  do_select = 0 skips score/select/rewrite
- * and attends over the previous selected tier (the steps between two compressions, L274). */
+/* HA-Sparse / "Sparse Loading" (L178, L191): attention over dense + selected + condensed where the selected rows
+ * are gathered from the base pool through sel_idx; the selected tier is neither read nor written (no rewrite, no
+ * memory movement; the gather is the "redundant, irregular" load the paper trades against it).  Same result as
+ * hardkv_rewrite followed by hardkv_decode_attn. */
+hardkv_status hardkv_sparse_attend(hardkv_ctx *, const hardkv_state *, const void *q, float *out,
+                                   float *lse /* nullable */, hardkv_stream);
+/* do_select of hardkv_decode_step: which of the paper's regimes the step runs (L191-197, L274). */
+enum {
+  HARDKV_STEP_REUSE_TIER = 0,     /* between two compressions, HA-Max: attend over the selected tier as rewritten  */
+  HARDKV_STEP_SELECT_REWRITE = 1, /* compression step, HA-Max: score, calibrate + Top-p, rewrite fused with attention */
+  HARDKV_STEP_SELECT_SPARSE = 2,  /* compression step, HA-Sparse: score, calibrate + Top-p, attention through sel_idx */
+  HARDKV_STEP_REUSE_SPARSE = 3    /* between two compressions, HA-Sparse: attention through the previous sel_idx      */
+};
+/* The whole step on one stream: append, retire, then per do_select (above): score, calibrate + Top-p, rewrite
+ * fused with attention (selected rows are read once) / attention over the previous selected tier (the steps
+ * between two compressions, L274) / the HA-Sparse forms that never touch the selected tier. */
 hardkv_status hardkv_decode_step(hardkv_ctx *, const hardkv_state *, const void *q, const void *k_new,
                                  const void *v_new, float p, int32_t do_select, float *out,
                                  float *lse /* nullable */, hardkv_stream);

@@ -33,7 +33,7 @@ __device__ __forceinline__ uint32_t pack_bf16(float lo, float hi) {
 }
 __device__ __forceinline__ float bf16_round(float x) { return __bfloat162float(__float2bfloat16_rn(x)); }
 
-template <int D, bool FUSED>
+template <int D, int MODE>
 __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void *q_, float *out, float *lse) {
   constexpr int NKC = D / 32;   // 64-byte chunks of a key row
   constexpr int NVC = D / 64;   // 128-byte chunks of a value row
@@ -91,10 +91,10 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
     } else if (v < n_dense + k) {           // Tier 2: selected rows
       const int j = v - n_dense;
       const uint32_t srow = (uint32_t)(__ldg(stab + (j >> 4)) * PAGE + (j & 15));
-      if (FUSED) {
+      if (MODE != ATT_TIER) {
         const int pos = __ldg(idx + j);
         srcs[r] = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
-        dsts[r] = srow;
+        if (MODE == ATT_REWRITE) dsts[r] = srow;
       } else {
         srcs[r] = (1u << 30) | srow;
       }
@@ -115,7 +115,7 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
     vs[1] = __shfl_sync(0xffffffffu, src, lb + 2 * tig + 1);
     vs[2] = __shfl_sync(0xffffffffu, src, lb + 2 * tig + 8);
     vs[3] = __shfl_sync(0xffffffffu, src, lb + 2 * tig + 9);
-    if (FUSED) {
+    if (MODE == ATT_REWRITE) {
       kd[0] = __shfl_sync(0xffffffffu, dst, lb + gid);
       kd[1] = __shfl_sync(0xffffffffu, dst, lb + gid + 8);
       vd[0] = __shfl_sync(0xffffffffu, dst, lb + 2 * tig);
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
       for (int ch = 0; ch < NVC; ++ch) vr[r][ch] = w != ROW_INVALID ? ldg_nc(rp + ch * 128) : make_uint4(0, 0, 0, 0);
     }
     // ---- Rewrite Cache write-through (L172): the rows go to the selected tier as they arrive ----
-    if (FUSED) {
+    if (MODE == ATT_REWRITE) {
 #pragma unroll
       for (int r = 0; r < 2; ++r)
         if (kd[r] != ROW_INVALID) {
@@ -218,7 +218,7 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
     }
   }
 
-  if (FUSED && k > 0 && (n_dense + k - 1) >= v0 && (n_dense + k - 1) < v1) {
+  if (MODE == ATT_REWRITE && k > 0 && (n_dense + k - 1) >= v0 && (n_dense + k - 1) < v1) {
     // zero tail of the last valid page of the selected tier (DESIGN reading C9)
     constexpr int LPR = ROWB / 16;
     const int kend = (k + PAGE - 1) & ~(PAGE - 1);

@@ -198,25 +198,29 @@ void launch_rewrite(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
   HK_DISPATCH_TD(ctx->cfg, (rewrite_kernel<T, D><<<grid, 256, 0, st>>>(P)));
 }
 
-void launch_attend(hardkv_ctx *ctx, const Params &P, const void *q, float *out, float *lse, bool fused,
+void launch_attend(hardkv_ctx *ctx, const Params &P, const void *q, float *out, float *lse, int mode,
                    cudaStream_t st) {
   ctx->launches += 1;
   if (fast_path(ctx)) {
     dim3 gm((P.att_chunks * ATT_CHUNK + ATT_MMA_CHUNK - 1) / ATT_MMA_CHUNK, P.B * P.Hkv);
     if (P.d == 128) {
-      if (fused) attend_mma_kernel<128, true><<<gm, 256, 0, st>>>(P, q, out, lse);
-      else attend_mma_kernel<128, false><<<gm, 256, 0, st>>>(P, q, out, lse);
+      if (mode == ATT_REWRITE) attend_mma_kernel<128, ATT_REWRITE><<<gm, 256, 0, st>>>(P, q, out, lse);
+      else if (mode == ATT_SPARSE) attend_mma_kernel<128, ATT_SPARSE><<<gm, 256, 0, st>>>(P, q, out, lse);
+      else attend_mma_kernel<128, ATT_TIER><<<gm, 256, 0, st>>>(P, q, out, lse);
     } else {
-      if (fused) attend_mma_kernel<64, true><<<gm, 256, 0, st>>>(P, q, out, lse);
-      else attend_mma_kernel<64, false><<<gm, 256, 0, st>>>(P, q, out, lse);
+      if (mode == ATT_REWRITE) attend_mma_kernel<64, ATT_REWRITE><<<gm, 256, 0, st>>>(P, q, out, lse);
+      else if (mode == ATT_SPARSE) attend_mma_kernel<64, ATT_SPARSE><<<gm, 256, 0, st>>>(P, q, out, lse);
+      else attend_mma_kernel<64, ATT_TIER><<<gm, 256, 0, st>>>(P, q, out, lse);
     }
     return;
   }
   dim3 grid(P.att_chunks, P.B * P.Hkv);
-  if (fused)
-    HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, true><<<grid, 256, 0, st>>>(P, q, out, lse))));
+  if (mode == ATT_REWRITE)
+    HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, ATT_REWRITE><<<grid, 256, 0, st>>>(P, q, out, lse))));
+  else if (mode == ATT_SPARSE)
+    HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, ATT_SPARSE><<<grid, 256, 0, st>>>(P, q, out, lse))));
   else
-    HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, false><<<grid, 256, 0, st>>>(P, q, out, lse))));
+    HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, ATT_TIER><<<grid, 256, 0, st>>>(P, q, out, lse))));
 }
 
 }  // namespace
@@ -360,14 +364,21 @@ hardkv_status hardkv_rewrite(hardkv_ctx *ctx, const hardkv_state *s, hardkv_stre
 hardkv_status hardkv_decode_attn(hardkv_ctx *ctx, const hardkv_state *s, const void *q, float *out, float *lse,
                                  hardkv_stream st) {
   if (!state_ok(ctx, s) || !q || !out) return HARDKV_ERR_INVALID_ARG;
-  launch_attend(ctx, params_of(ctx, s), q, out, lse, false, st);
+  launch_attend(ctx, params_of(ctx, s), q, out, lse, ATT_TIER, st);
   return launch_status();
 }
 
 hardkv_status hardkv_rewrite_attend(hardkv_ctx *ctx, const hardkv_state *s, const void *q, float *out, float *lse,
                                     hardkv_stream st) {
   if (!state_ok(ctx, s) || !q || !out) return HARDKV_ERR_INVALID_ARG;
-  launch_attend(ctx, params_of(ctx, s), q, out, lse, true, st);
+  launch_attend(ctx, params_of(ctx, s), q, out, lse, ATT_REWRITE, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_sparse_attend(hardkv_ctx *ctx, const hardkv_state *s, const void *q, float *out, float *lse,
+                                   hardkv_stream st) {
+  if (!state_ok(ctx, s) || !q || !out) return HARDKV_ERR_INVALID_ARG;
+  launch_attend(ctx, params_of(ctx, s), q, out, lse, ATT_SPARSE, st);
   return launch_status();
 }
 
@@ -379,14 +390,16 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   if (!state_ok(ctx, s) || !q || !k_new || !v_new || !out || !(p > 0.f) || !accum_ok(ctx, s))
     return HARDKV_ERR_INVALID_ARG;
   const Params P = params_of(ctx, s);
+  if (do_select < 0 || do_select > 3) return HARDKV_ERR_INVALID_ARG;
   launch_append(ctx, P, k_new, v_new, st);
-  if (do_select) {
+  if (do_select == HARDKV_STEP_SELECT_REWRITE || do_select == HARDKV_STEP_SELECT_SPARSE) {
     launch_score(ctx, P, q, st);
     launch_pool(ctx, P, st);
     // the score kernel's chunk statistics describe the raw logits: configs with pooled heads take them in-kernel
     launch_select(ctx, P, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
   }
-  launch_attend(ctx, P, q, out, lse, do_select != 0, st);
+  launch_attend(ctx, P, q, out, lse, do_select == HARDKV_STEP_SELECT_REWRITE ? ATT_REWRITE
+                                     : (do_select == HARDKV_STEP_REUSE_TIER ? ATT_TIER : ATT_SPARSE), st);
   return launch_status();
 }
 

@@ -205,12 +205,15 @@ __global__ void __launch_bounds__(256) rewrite_kernel(Params P) {
 // A CTA takes ATT_CHUNK consecutive virtual rows, keeps a max-shifted state (m, l, acc) per
 // query head, and writes it as a partial; the last CTA of the unit to arrive merges the
 // partials with the operator of Eq. 6 (SE = l * e^m, o = acc / l).
-// FUSED: selected rows are gathered from the base pool through sel_idx and written through to
-// the selected tier while they are in registers (rewrite + attend read each row once).
+// MODE: ATT_TIER reads the selected rows from the rewritten selected tier (HA-Max after a rewrite);
+// ATT_REWRITE gathers them from the base pool through sel_idx and writes them through to the selected tier while
+// they are in registers (rewrite + attend read each row once); ATT_SPARSE gathers them and writes nothing
+// (HA-Sparse / "Sparse Loading": regular indices, no memory movement).
 // =============================================================================================
 constexpr int ATT_CHUNK = 128;
+constexpr int ATT_TIER = 0, ATT_REWRITE = 1, ATT_SPARSE = 2;
 
-template <typename T, int D, int G, bool FUSED>
+template <typename T, int D, int G, int MODE>
 __global__ void __launch_bounds__(256) attend_generic_kernel(Params P, const void *q_, float *out, float *lse) {
   constexpr int EPL = Elem<T>::EPL, LPR = D / EPL, ROWB = D * sizeof(T);
   constexpr int NGRP = 256 / LPR;  // row groups per CTA
@@ -266,7 +269,7 @@ __global__ void __launch_bounds__(256) attend_generic_kernel(Params P, const voi
       } else if (v < n_dense + k) {  // Tier 2: selected rows
         const int j = v - n_dense;
         const size_t so = ((size_t)__ldg(stab + (j >> 4)) * PAGE + (j & 15)) * ROWB;
-        if (FUSED) {
+        if (MODE != ATT_TIER) {
           const int pos = __ldg(idx + j);
           kp = paged_row<T, D>(P.st.k_pool, tab, pos);
           vp = paged_row<T, D>(P.st.v_pool, tab, pos);
@@ -276,7 +279,7 @@ __global__ void __launch_bounds__(256) attend_generic_kernel(Params P, const voi
         }
         kr[u] = ldg_nc(kp + lr * 16);
         vr[u] = ldg_nc(vp + lr * 16);
-        if (FUSED) {
+        if (MODE == ATT_REWRITE) {
           stg(reinterpret_cast<char *>(P.st.sel_k_pool) + so + lr * 16, kr[u]);
           stg(reinterpret_cast<char *>(P.st.sel_v_pool) + so + lr * 16, vr[u]);
         }
@@ -323,7 +326,7 @@ __global__ void __launch_bounds__(256) attend_generic_kernel(Params P, const voi
     }
   }
 
-  if (FUSED && k > 0 && (n_dense + k - 1) >= v0 && (n_dense + k - 1) < v1) {
+  if (MODE == ATT_REWRITE && k > 0 && (n_dense + k - 1) >= v0 && (n_dense + k - 1) < v1) {
     // zero tail of the last valid page of the selected tier (DESIGN reading C9)
     const int kend = (k + PAGE - 1) & ~(PAGE - 1);
     for (int vec = tid; vec < (kend - k) * LPR; vec += 256) {

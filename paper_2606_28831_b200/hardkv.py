@@ -53,9 +53,10 @@ class StateStruct(C.Structure):
 
 
 F32, BF16 = 0, 1
+STEP_REUSE_TIER, STEP_SELECT_REWRITE, STEP_SELECT_SPARSE, STEP_REUSE_SPARSE = 0, 1, 2, 3   # do_select of decode_step
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
            "hardkv_set_variant", "hardkv_append_kv", "hardkv_score", "hardkv_calibrate_topp", "hardkv_solve_temperature",
-           "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend",
+           "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend", "hardkv_sparse_attend",
            "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count"]
 
 
@@ -80,6 +81,7 @@ def _load():
     lib.hardkv_rewrite.argtypes = [vp, sp, vp]
     lib.hardkv_decode_attn.argtypes = [vp, sp, vp, vp, vp, vp]
     lib.hardkv_rewrite_attend.argtypes = [vp, sp, vp, vp, vp, vp]
+    lib.hardkv_sparse_attend.argtypes = [vp, sp, vp, vp, vp, vp]
     lib.hardkv_decode_step.argtypes = [vp, sp, vp, vp, vp, C.c_float, C.c_int32, vp, vp, vp]
     lib.hardkv_decode_step_host.argtypes = [vp, sp, vp, vp, vp, C.c_float, C.c_int32, vp, vp]
     lib.hardkv_launch_count.argtypes = [vp]
@@ -178,6 +180,9 @@ class HardKV:
 
     def rewrite_attend(self, st: DeviceState, q, out, lse=None):
         _check(lib.hardkv_rewrite_attend(self._ctx, C.byref(st.struct()), _ptr(q), _ptr(out), _ptr(lse), _stream()))
+
+    def sparse_attend(self, st: DeviceState, q, out, lse=None):
+        _check(lib.hardkv_sparse_attend(self._ctx, C.byref(st.struct()), _ptr(q), _ptr(out), _ptr(lse), _stream()))
 
     def launch_count(self) -> int:
         return int(lib.hardkv_launch_count(self._ctx))

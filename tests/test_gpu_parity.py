@@ -96,6 +96,33 @@ def test_stages_teacher_forced(name, P):
         for i, u in enumerate(ob.units):
             u.attend(qu[i])
         pr.check_out(f"{name} step {t}")
+        # HA-Sparse (L178): the same attention gathered through sel_idx; the selected tier is not touched
+        tier0 = (st.sel_k_pool.clone(), st.sel_v_pool.clone())
+        out2, lse2 = torch.zeros_like(pr.out), torch.zeros_like(pr.lse)
+        eng.sparse_attend(st, qd, out2, lse2)
+        assert torch.equal(out2, pr.out) and torch.equal(lse2, pr.lse)
+        assert torch.equal(tier0[0], st.sel_k_pool) and torch.equal(tier0[1], st.sel_v_pool)
+
+
+@pytest.mark.parametrize("name", ["c0", "c2s", "c3s", "c4s", "snap4"])
+def test_sparse_regime_steps(name, P):
+    """HA-Sparse decode steps (do_select 2 / 3: select every 3rd step, attend through sel_idx in between, no
+    rewrite ever) against the oracle run with the same compression interval (L178, L191, L274)."""
+    from paper_2606_28831_b200 import hardkv
+    wl = WL[name]
+    pr = P(wl, want_mask=False)
+    tier0 = (pr.st.sel_k_pool.clone(), pr.st.sel_v_pool.clone())
+    for t in range(min(wl.steps, 9)):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        sel = t % 3 == 0
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse,
+                           do_select=hardkv.STEP_SELECT_SPARSE if sel else hardkv.STEP_REUSE_SPARSE)
+        pr.ob.step(q, kn, vn, wl.p, do_select=sel)
+        pr.check_out(f"{name} sparse step {t}")
+        if sel:
+            pr.check_selection_band()
+        pr.force_discrete_state()
+    assert torch.equal(tier0[0], pr.st.sel_k_pool) and torch.equal(tier0[1], pr.st.sel_v_pool)
 
 
 @pytest.mark.parametrize("name", list(WL))
