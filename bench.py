@@ -299,6 +299,15 @@ def run_cuda(args):
     unfused_us = timed_loop(five_calls)
     amortised_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out,
                                                         do_select=((t - W) // L) % SI == 0))
+    # HA-Sparse (Sparse Loading, L178 / L191): attention gathers through sel_idx, the selected tier is never written
+    sparse_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out, do_select=2))
+    sparse_amortised_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out,
+                                                               do_select=2 if ((t - W) // L) % SI == 0 else 3))
+    row_b = wl.d * (2 if wl.dtype == "bf16" else 4)
+    units_ = wl.B * wl.Hkv
+    kv_base = float(2 * row_b * wl.Hkv * (wl.n0.sum() + wl.B * (W + K / 2)))     # live base-pool K + V rows
+    kv_cond = float(2 * row_b * units_ * wl.cond_cap)
+    kv_tier = float(2 * row_b * units_ * wl.k_cap)                                # static HA-Max capacity (L191-195)
 
     # ---- (3) end to end through the host-buffer entry point -------------------------------------
     warm()
@@ -355,6 +364,18 @@ def run_cuda(args):
             "amortised": {"select_interval": SI, "us_per_layer_step": amortised_us,
                           "note": "compression every select_interval steps as in the paper (L274); the other steps "
                                   "append and attend over the previous selected tier"},
+            "ha_sparse": {"us_per_layer_step": sparse_us, "amortised_us_per_layer_step": sparse_amortised_us,
+                          "select_interval": SI,
+                          "note": "Sparse Loading (L178, L191): same selection, attention gathered through sel_idx, "
+                                  "no rewrite; eager launches like the other context lines"},
+            "memory_time_integral": {
+                "unit": "GB*us per layer-step", "select_interval": SI,
+                "ha_max": (kv_base + kv_cond + kv_tier) / 1e9 * amortised_us,
+                "ha_sparse": (kv_base + kv_cond) / 1e9 * sparse_amortised_us,
+                "kv_resident_gb": {"ha_max": (kv_base + kv_cond + kv_tier) / 1e9, "ha_sparse": (kv_base + kv_cond) / 1e9},
+                "note": "analogue of the paper's MTI (L205, L504-515): resident KV bytes x time per step in the amortised "
+                        "regime; this build keeps the candidate pool resident in both layouts, so HA-Max pays the static "
+                        "selected tier on top"},
             "roofline": roof,
             "e2e": {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "us_per_layer_step": ms_e2e / K * 1e3, "sync": "stream sync after every step"},
