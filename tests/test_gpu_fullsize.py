@@ -21,7 +21,8 @@ def run_sampled(wl, sample, steps, p=None):
     eng = harness.make_engine(wl, DEV)
     (st,), prefill = harness.make_state(wl, DEV)
     cfg = OracleConfig(G=wl.G, d=wl.d, max_ctx=wl.max_ctx, sink=wl.sink, recent=wl.recent, k_cap=wl.k_cap,
-                       cond_cap=wl.cond_cap, accum_window=wl.accum_window, sm_scale=float(wl.sm_scale))
+                       cond_cap=wl.cond_cap, accum_window=wl.accum_window, sm_scale=float(wl.sm_scale),
+                       pool_kernel=wl.pool_kernel)
     units = [Unit(cfg, *prefill[(b, h)], l_upper=int(wl.l_upper[b]), l_lower=int(wl.l_lower[b]),
                   T=float(wl.temperature[b, h]), score_mode=int(wl.score_mode[h])) for b, h in sample]
     pk = {u: kv[0] for u, kv in prefill.items()} if wl.mix_new_keys else None
@@ -92,3 +93,62 @@ def test_config4_full_size_sampled(p):
     """Config 4 (G = 5, 64k context, RAW and ACCUM heads) at two ends of its p sweep."""
     wl = make_workload(4)
     run_sampled(wl, [(0, 1), (3, 6), (7, 4)], steps=3, p=p)
+
+
+def test_config2_full_size_snapkv_solve_then_step():
+    """Full-size config 2 with half the KV heads on the SNAPKV metric (window 7): Algorithm 2 solves T on the first
+    step's logits (sampled units against the oracle's bisection, 1e-3 relative), then fused steps run with the
+    solved temperatures (L607: solve at the first compression, reuse afterwards)."""
+    wl = make_workload(2, score_mode=np.array([0, 2, 0, 2, 0, 2, 0, 2], np.uint8), pool_kernel=7)
+    order = np.argsort(wl.n0)
+    sample = [(int(order[0]), 1), (int(order[-1]), 7), (int(order[len(order) // 2]), 2), (int(order[-1]), 3)]
+    eng = harness.make_engine(wl, DEV)
+    (st,), prefill = harness.make_state(wl, DEV)
+    cfg = OracleConfig(G=wl.G, d=wl.d, max_ctx=wl.max_ctx, sink=wl.sink, recent=wl.recent, k_cap=wl.k_cap,
+                       cond_cap=wl.cond_cap, accum_window=wl.accum_window, sm_scale=float(wl.sm_scale),
+                       pool_kernel=wl.pool_kernel)
+    units = [Unit(cfg, *prefill[(b, h)], l_upper=int(wl.l_upper[b]), score_mode=int(wl.score_mode[h])) for b, h in sample]
+    q = wl.step_q(0)
+    kn, vn = wl.step_kv(0, None)
+    qd, knd, vnd = (harness.to_dev(x, wl, DEV) for x in (q, kn, vn))
+    eng.append_kv(st, knd, vnd)
+    eng.score(st, qd)
+    eng.solve_temperature(st, wl.p, t_min=0.0625, t_max=16.0, eps=1e-5, max_iter=40)
+    T = st.temperature.cpu().numpy()
+    # sharp heads select fewer tokens than one pooling window holds copies of the top logit: no T matches the mass
+    # (the paper's "failure cases ... illness of the problem", L605) and the bisection runs into T_min
+    assert np.isfinite(T).all() and (T >= 0.0625).all() and (T <= 16.0).all()
+    raw = T[:, 0::2]
+    assert np.abs(raw - 1.0).max() < 5e-3                       # g = id heads: T* = 1 (pin P13)
+    for (b, h), u in zip(sample, units):
+        u.append(kn[b, h], vn[b, h]); u.retire()
+        u.score(q[b, h * wl.G:(h + 1) * wl.G])
+        it, resid = u.solve_temperature(wl.p, t_min=0.0625, t_max=16.0, eps=1e-5, max_iter=40)
+        assert abs(T[b, h] - u.T) <= 1e-3 * u.T, (b, h, T[b, h], u.T)
+        assert resid <= 1e-5 or u.T < 0.0626 or it == 40, (b, h, resid, u.T, it)
+        u.u.T = np.float32(T[b, h])
+    # the rest of step 0 (select + rewrite + attend with the solved T), then one more fused step
+    out = torch.zeros(wl.B, wl.Hq, wl.d, dtype=torch.float32, device=DEV)
+    eng.calibrate_topp(st, wl.p)
+    eng.rewrite_attend(st, qd, out)
+    for (b, h), u in zip(sample, units):
+        u.calibrate(); u.topp_select(wl.p, True); u.rewrite(); u.attend(q[b, h * wl.G:(h + 1) * wl.G])
+    for t in (0, 1):
+        if t == 1:
+            q = wl.step_q(1)
+            kn, vn = wl.step_kv(1, None)
+            eng.decode_step(st, harness.to_dev(q, wl, DEV), harness.to_dev(kn, wl, DEV), harness.to_dev(vn, wl, DEV),
+                            wl.p, out)
+            decode_step_batch(units, np.stack([q[b, h * wl.G:(h + 1) * wl.G] for b, h in sample]),
+                              np.stack([kn[b, h] for b, h in sample]), np.stack([vn[b, h] for b, h in sample]), wl.p)
+        o = out.cpu().numpy()
+        cnt, idx = st.sel_count.cpu().numpy(), st.sel_idx.cpu().numpy()
+        for (b, h), u in zip(sample, units):
+            i = b * wl.Hkv + h
+            diff = sorted(set(idx[i, :cnt[i]].tolist()) ^ set(u.sel_idx[:u.sel_count].tolist()))
+            if diff:
+                tau = np.array([u.tau_bits], np.uint32).view(np.float32)[0]
+                assert np.all(np.abs(u.probs[diff].astype(np.float64) - float(tau)) <= TAU_BAND), (t, b, h, diff[:8])
+            e = np.abs(o[b, h * wl.G:(h + 1) * wl.G] - u.out)
+            assert e.max() <= OUT_MAX_ABS and e.mean() <= OUT_MEAN_ABS, (t, b, h, e.max())
+            st.votes[i].copy_(torch.from_numpy(u.votes))
