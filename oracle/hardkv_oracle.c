@@ -34,11 +34,58 @@ void hko_append(const hko_config *c, hko_unit *u, const float *k_new, const floa
  * resident with the lexicographically smallest (votes, pos) is the candidate
  * victim and t replaces it iff votes[t] >= its votes (t is newer, so it wins
  * ties); else t is evicted for good. */
-int hko_retire(const hko_config *c, hko_unit *u) {
+/* Store rounding of a merged row element: the tier holds kv_dtype values, so a bf16 tier
+ * rounds the exact (fp64) combination once, to nearest-even, to 8 significant bits. */
+static float hko_store_round(const hko_config *c, double x) {
+  if (!c->kv_bf16 || x == 0.0 || !isfinite(x)) return (float)x;
+  int e;
+  double m = frexp(x, &e);                       /* x = m 2^e, 0.5 <= |m| < 1 */
+  return (float)ldexp(nearbyint(m * 256.0), e - 8);
+}
+
+/* ---- LSE-preserving weighted merging (Appendix G, Eq. 9 / Thm G.1; reading
+ * C17): the evictee e is not dropped but folded into the resident a with the highest
+ * score under the current queries ("let q K_j >> q K_k", Eq. 11), with the softmax
+ * weights of the pair:  K_hat = w_a K_a + w_e K_e,  w_a = e^{x_a} / (e^{x_a} + e^{x_e}),
+ * x = group mean of sm_scale q_g . K (one pair of weights per KV head); V takes the same
+ * weights (the paper leaves g(V_j, V_k) open, L806-811).  pos / votes of a are unchanged. */
+static void hko_merge_evictee(const hko_config *c, hko_unit *u, const float *q,
+                              const float *Ke, const float *Ve) {
+  if (u->cond_count <= 0) return;
+  int32_t a = 0;
+  double xa = -INFINITY, xe = 0.0;
+  for (int32_t r = 0; r < u->cond_count; ++r) {
+    double x = 0.0;
+    for (int32_t g = 0; g < c->G; ++g) {
+      double dot = 0.0;
+      for (int32_t e = 0; e < c->d; ++e)
+        dot += (double)q[(size_t)g * c->d + e] * (double)u->cond_k[(size_t)r * c->d + e];
+      x += (double)c->sm_scale * dot;
+    }
+    x /= (double)c->G;
+    if (x > xa) { xa = x; a = r; }               /* ties: the lowest slot */
+  }
+  for (int32_t g = 0; g < c->G; ++g) {
+    double dot = 0.0;
+    for (int32_t e = 0; e < c->d; ++e) dot += (double)q[(size_t)g * c->d + e] * (double)Ke[e];
+    xe += (double)c->sm_scale * dot;
+  }
+  xe /= (double)c->G;
+  double wa = 1.0 / (1.0 + exp(xe - xa)), we = 1.0 - wa;
+  for (int32_t e = 0; e < c->d; ++e) {
+    float *ka = u->cond_k + (size_t)a * c->d + e, *va = u->cond_v + (size_t)a * c->d + e;
+    *ka = hko_store_round(c, wa * (double)*ka + we * (double)Ke[e]);
+    *va = hko_store_round(c, wa * (double)*va + we * (double)Ve[e]);
+  }
+}
+
+int hko_retire_q(const hko_config *c, hko_unit *u, const float *q) {
   int retired = 0;
+  float *ek = (float *)malloc(sizeof(float) * (size_t)c->d), *ev = (float *)malloc(sizeof(float) * (size_t)c->d);
   while (u->n - c->recent - u->c_lo > u->l_upper) {
     int32_t t = u->c_lo;
     int32_t slot = -1;
+    int have_evictee = 0;
     if (u->cond_count < c->cond_cap) {
       slot = u->cond_count;
       u->cond_count += 1;
@@ -49,7 +96,15 @@ int hko_retire(const hko_config *c, hko_unit *u) {
             (u->cond_votes[j] == u->cond_votes[m] && u->cond_pos[j] < u->cond_pos[m]))
           m = j;
       }
-      if (u->votes[t] >= u->cond_votes[m]) slot = m;
+      if (u->votes[t] >= u->cond_votes[m]) {
+        slot = m;                                  /* the displaced resident is the evictee */
+        memcpy(ek, u->cond_k + (size_t)m * c->d, sizeof(float) * c->d);
+        memcpy(ev, u->cond_v + (size_t)m * c->d, sizeof(float) * c->d);
+      } else {                                     /* the newcomer itself is the evictee */
+        memcpy(ek, u->K + (size_t)t * c->d, sizeof(float) * c->d);
+        memcpy(ev, u->V + (size_t)t * c->d, sizeof(float) * c->d);
+      }
+      have_evictee = 1;
     }
     if (slot >= 0) {
       memcpy(u->cond_k + (size_t)slot * c->d, u->K + (size_t)t * c->d, sizeof(float) * c->d);
@@ -57,11 +112,15 @@ int hko_retire(const hko_config *c, hko_unit *u) {
       u->cond_pos[slot] = t;
       u->cond_votes[slot] = u->votes[t];
     }
+    if (have_evictee && c->cond_merge && q) hko_merge_evictee(c, u, q, ek, ev);
     u->c_lo += 1;
     retired += 1;
   }
+  free(ek); free(ev);
   return retired;
 }
+
+int hko_retire(const hko_config *c, hko_unit *u) { return hko_retire_q(c, u, NULL); }
 
 /* ---- score: exponent of Eq. 4 (L735-739) with the scale of reading C1 ---------- */
 void hko_score(const hko_config *c, hko_unit *u, const float *q) {
@@ -377,7 +436,7 @@ void hko_attend(const hko_config *c, hko_unit *u, const float *q) {
 void hko_decode_step(const hko_config *c, hko_unit *u, const float *q,
                      const float *k_new, const float *v_new, float p, int do_select) {
   hko_append(c, u, k_new, v_new);
-  hko_retire(c, u);
+  hko_retire_q(c, u, q);
   if (do_select) {
     hko_score(c, u, q);
     hko_calibrate(c, u);

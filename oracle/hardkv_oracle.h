@@ -23,7 +23,8 @@
  * P9 rewrite copies, P10 condensed tier == top-C_cap of the retirement log,
  * P11 bookkeeping invariants, P12 integer mass vs fp64 cumsum, P13 temperature
  * solve (g = id => T* = 1; g = a z => T* = a; M_k decreasing in T), P14 SNAPKV
- * max-pool == torch.nn.functional.max_pool1d.
+ * max-pool == torch.nn.functional.max_pool1d, P15 weighted merging (Eq. 9 weights ==
+ * torch.softmax of the pair, SE_evict <= SE_merge <= SE_keep, Thm G.1 limit).
  * Parity unpinned by the paper: readings C2 (GQA group mean), C3 (softmax over
  * the pool only), C4 (ACCUM window form), C7 (condensed-tier retention rule),
  * C8 (threshold mapping).  The paper prints no worked example for them; they
@@ -49,6 +50,8 @@ typedef struct {
   int32_t accum_window; /* ACCUM ring depth (32)                                   */
   float   sm_scale;     /* reading C1: 1/sqrt(d) by default                        */
   int32_t pool_kernel;  /* SNAPKV max-pool window (odd; <= 1: identity), C15       */
+  int32_t cond_merge;   /* 1: evictees of a full condensed tier are merged (App. G) */
+  int32_t kv_bf16;      /* 1: merged rows are stored rounded to bf16 (RNE)          */
 } hko_config;
 
 typedef struct {
@@ -82,6 +85,9 @@ typedef struct {
 void hko_append(const hko_config *c, hko_unit *u, const float *k_new, const float *v_new);
 /* Step 4 of L78 / Tier 3 of L76 / votes ranking L86 (reading C7). Returns #retired. */
 int  hko_retire(const hko_config *c, hko_unit *u);
+/* The same with the step's queries q [G][d]: when c->cond_merge, the evictee of a full tier is folded into the
+ * highest-scoring resident with the LSE-preserving weights of Appendix G (Eq. 9; reading C17). */
+int  hko_retire_q(const hko_config *c, hko_unit *u, const float *q);
 /* z[g][i] = sm_scale * q_g . k_i over the pool (Eq. 4 exponent, reading C1). */
 void hko_score(const hko_config *c, hko_unit *u, const float *q);
 /* Logits Calibration, apply-T form (L120 Solution 1), group mean (reading C2). */

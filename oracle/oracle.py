@@ -34,6 +34,7 @@ class HkoConfig(C.Structure):
         ("G", C.c_int32), ("d", C.c_int32), ("page", C.c_int32), ("max_ctx", C.c_int32),
         ("sink", C.c_int32), ("recent", C.c_int32), ("k_cap", C.c_int32), ("cond_cap", C.c_int32),
         ("accum_window", C.c_int32), ("sm_scale", C.c_float), ("pool_kernel", C.c_int32),
+        ("cond_merge", C.c_int32), ("kv_bf16", C.c_int32),
     ]
 
 
@@ -66,6 +67,8 @@ def lib():
         _lib.hko_append.argtypes = [cp, up, _F, _F]
         _lib.hko_retire.argtypes = [cp, up]
         _lib.hko_retire.restype = C.c_int
+        _lib.hko_retire_q.argtypes = [cp, up, _F]
+        _lib.hko_retire_q.restype = C.c_int
         _lib.hko_score.argtypes = [cp, up, _F]
         _lib.hko_calibrate.argtypes = [cp, up]
         _lib.hko_solve_temperature.argtypes = [cp, up, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int,
@@ -111,11 +114,14 @@ class OracleConfig:
     accum_window: int = 32
     sm_scale: float | None = None
     pool_kernel: int = 0
+    cond_merge: int = 0
+    kv_bf16: int = 0
 
     def c(self) -> HkoConfig:
         s = self.sm_scale if self.sm_scale is not None else 1.0 / float(np.sqrt(self.d))
         return HkoConfig(self.G, self.d, self.page, self.max_ctx, self.sink, self.recent, self.k_cap,
-                         self.cond_cap, self.accum_window, np.float32(s), self.pool_kernel)
+                         self.cond_cap, self.accum_window, np.float32(s), self.pool_kernel,
+                         self.cond_merge, self.kv_bf16)
 
 
 class Unit:
@@ -178,6 +184,9 @@ class Unit:
 
     def retire(self) -> int:
         return lib().hko_retire(C.byref(self.ccfg), C.byref(self.u))
+
+    def retire_q(self, q) -> int:
+        return lib().hko_retire_q(C.byref(self.ccfg), C.byref(self.u), _fp(_f32(q)))
 
     def score(self, q):
         lib().hko_score(C.byref(self.ccfg), C.byref(self.u), _fp(_f32(q)))

@@ -489,3 +489,87 @@ def test_p13_accum_heads_are_left_alone():
     lo, hi = u.pool
     _set_logits(u, rng.standard_normal((2, hi - lo)))
     assert u.solve_temperature(0.9) == (0, 0.0) and u.T == 1.5
+
+
+# ---- P15: LSE-preserving weighted merging of the condensed tier (Appendix G, Eq. 9, Thm G.1) -----
+def _merge_case(gap, G=1, seed=15, bf16=0):
+    """A full 4-slot tier, l_upper tiny so the next step retires one token that loses on votes (votes 0 < residents' 5):
+    the newcomer is the evictee and must be folded into the best-scoring resident."""
+    rng = np.random.default_rng(seed)
+    d = 64
+    cfg = OracleConfig(G=G, d=d, max_ctx=128, sink=4, recent=8, k_cap=128, cond_cap=4, cond_merge=1, kv_bf16=bf16,
+                       sm_scale=1.0)
+    K0 = rng.standard_normal((60, d)).astype(np.float32) * 0.3
+    V0 = rng.standard_normal((60, d)).astype(np.float32)
+    u = Unit(cfg, K0, V0, l_upper=60 - 8 - 4 - 1)       # pool 48 > 47: exactly one retirement
+    q = rng.standard_normal((G, d)).astype(np.float32) * 0.3
+    qbar = q.mean(0)
+    # residents: slot 2 is aligned with the queries (the anchor), the others are weak
+    u.u.cond_count = 4
+    for j in range(4):
+        u.cond_k[j] = rng.standard_normal(d).astype(np.float32) * 0.05
+        u.cond_v[j] = rng.standard_normal(d).astype(np.float32)
+        u.cond_pos[j] = 100 + j; u.cond_votes[j] = 5
+    u.cond_k[2] = (qbar / np.dot(qbar, qbar) * 2.0).astype(np.float32)            # x_anchor = 2
+    u.K[4] = (qbar / np.dot(qbar, qbar) * (2.0 - gap)).astype(np.float32)         # evictee t = c_lo = 4: x_e = 2 - gap
+    return cfg, u, q
+
+
+@pytest.mark.parametrize("G,gap", [(1, 0.5), (4, 1.5), (1, 0.0)])
+def test_p15_merge_weights_are_the_pair_softmax(G, gap):
+    cfg, u, q = _merge_case(gap, G=G)
+    Ka, Va, Ke, Ve = u.cond_k[2].copy(), u.cond_v[2].copy(), u.K[4].copy(), u.V[4].copy()
+    others = (u.cond_k[[0, 1, 3]].copy(), u.cond_v[[0, 1, 3]].copy(), u.cond_pos.copy(), u.cond_votes.copy())
+    assert u.retire_q(q) == 1 and u.c_lo == 5 and u.cond_count == 4
+    xa = float(np.mean(q.astype(np.float64) @ Ka.astype(np.float64)))
+    xe = float(np.mean(q.astype(np.float64) @ Ke.astype(np.float64)))
+    w = torch.softmax(torch.tensor([xa, xe], dtype=torch.float64), 0).numpy()       # Eq. 9's weights, library softmax
+    np.testing.assert_allclose(u.cond_k[2], w[0] * Ka + w[1] * Ke, rtol=0, atol=1e-6)
+    np.testing.assert_allclose(u.cond_v[2], w[0] * Va + w[1] * Ve, rtol=0, atol=1e-6)
+    np.testing.assert_array_equal(u.cond_k[[0, 1, 3]], others[0])                     # only the anchor changes
+    np.testing.assert_array_equal(u.cond_v[[0, 1, 3]], others[1])
+    np.testing.assert_array_equal(u.cond_pos, others[2]); np.testing.assert_array_equal(u.cond_votes, others[3])
+    if gap == 0.0:
+        assert abs(w[0] - 0.5) < 1e-6                                                  # equal scores: the midpoint
+
+
+def test_p15_se_between_eviction_and_keeping_and_theorem_g1_limit():
+    """G = 1: the merged key scores the weighted mean of the pair's scores (Eq. 9.a is linear in K), so its
+    exponential lies between the pair's and below keeping both (h(t) > 0, Eq. 13-14), and the SE error of Eq. 10
+    relative to keeping both vanishes as x_a - x_e grows (Thm G.1, Eq. 11 / 15)."""
+    errs = []
+    for gap in (0.5, 2.0, 6.0, 12.0):
+        cfg, u, q = _merge_case(gap, G=1)
+        Ka, Ke = u.cond_k[2].astype(np.float64), u.K[4].astype(np.float64)
+        u.retire_q(q)
+        x = lambda K: float(q[0].astype(np.float64) @ K)
+        se_merge, se_keep, se_evict = math.exp(x(u.cond_k[2].astype(np.float64))), math.exp(x(Ka)) + math.exp(x(Ke)), math.exp(x(Ka))
+        w = torch.softmax(torch.tensor([x(Ka), x(Ke)], dtype=torch.float64), 0).numpy()
+        assert abs(math.log(se_merge) - (w[0] * x(Ka) + w[1] * x(Ke))) < 1e-5           # Eq. 9.a
+        assert math.exp(x(Ke)) * (1 - 1e-6) <= se_merge <= se_evict * (1 + 1e-6) <= se_keep
+        errs.append((se_keep - se_merge) / se_keep)
+    assert all(a > b for a, b in zip(errs, errs[1:])) and errs[-1] < 1e-4
+
+
+def test_p15_displaced_resident_is_merged_and_bf16_store():
+    """The newcomer wins on votes: it takes the weakest slot and the displaced resident is the evictee; the merged
+    anchor row of a bf16 tier is bf16-representable and within half an ulp (at most 2^-8 relative) of the exact combination."""
+    cfg, u, q = _merge_case(1.0, G=2, bf16=1)
+    u.votes[4] = 9                                       # newcomer outranks every resident (votes 5)
+    u.cond_votes[1] = 3                                  # slot 1 is the weakest: displaced
+    Ka, Ke = u.cond_k[2].copy(), u.cond_k[1].copy()
+    Kt = u.K[4].copy()
+    u.retire_q(q)
+    assert u.cond_pos[1] == 4 and u.cond_votes[1] == 9
+    np.testing.assert_array_equal(u.cond_k[1], Kt)
+    xs = [float(np.mean(q.astype(np.float64) @ u.cond_k[j].astype(np.float64))) for j in range(4)]
+    # the anchor is the best-scoring resident after the replacement (the aligned newcomer, slot 1, or slot 2)
+    a = 1 if float(np.mean(q.astype(np.float64) @ Kt.astype(np.float64))) > 2.0 else 2
+    base = Kt if a == 1 else Ka
+    xa = float(np.mean(q.astype(np.float64) @ base.astype(np.float64)))
+    xe = float(np.mean(q.astype(np.float64) @ Ke.astype(np.float64)))
+    wa = 1.0 / (1.0 + math.exp(xe - xa))
+    exact = wa * base.astype(np.float64) + (1 - wa) * Ke.astype(np.float64)
+    got = u.cond_k[a]
+    assert np.all((got.view(np.uint32) & 0xffff) == 0)                                # bf16-representable
+    np.testing.assert_allclose(got, exact, rtol=2.0 ** -8, atol=1e-30)
