@@ -72,6 +72,8 @@ typedef struct {
   float   sm_scale;       /* <= 0: 1/sqrt(head_dim)                                                 */
   int32_t pool_kernel;    /* SNAPKV max-pool window: odd, 3..63; 0 or 1: the config has no SNAPKV   */
                           /* head (the pooling pass is not launched)                                */
+  int32_t cond_merge;     /* 1: the evictee of a full condensed tier is merged into a resident with  */
+                          /* the LSE-preserving weights of Appendix G (Eq. 9) instead of dropped     */
 } hardkv_config;
 
 /* Caller-owned device state of one layer.  Pointers marked (opt) may be NULL. */
@@ -106,6 +108,14 @@ hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant);
  * condensed tier of every head, ranked on its Cautious-Update votes (L76, L86). */
 hardkv_status hardkv_append_kv(hardkv_ctx *, const hardkv_state *, const void *k_new, const void *v_new,
                                hardkv_stream);
+/* hardkv_append_kv with the step's queries q [B][Hq][d]: when cfg.cond_merge is set, every retirement from a full
+ * condensed tier folds its evictee (the displaced resident, or the newcomer when it loses on votes) into the
+ * resident a with the highest group-mean score x = mean_g sm_scale q_g . K (Thm G.1: "q K_j >> q K_k"):
+ * K_a <- w_a K_a + w_e K_e, V_a likewise, w_a = e^{x_a} / (e^{x_a} + e^{x_e}) (Eq. 9), stored rounded to
+ * kv_dtype; cond_pos / cond_votes of a are unchanged.  hardkv_decode_step takes this path when cfg.cond_merge is set;
+ * hardkv_append_kv (no queries) always evicts. */
+hardkv_status hardkv_append_kv_merge(hardkv_ctx *, const hardkv_state *, const void *k_new, const void *v_new,
+                                     const void *q, hardkv_stream);
 /* logits[b][h*G+g][i] = sm_scale * q . K[i] over the pool (exponent of Eq. 4). */
 hardkv_status hardkv_score(hardkv_ctx *, const hardkv_state *, const void *q, hardkv_stream);
 /* Logits Calibration (apply-T) -> probs, then hardkv_topp_select.  SNAPKV heads (cfg.pool_kernel > 1)

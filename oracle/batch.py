@@ -15,7 +15,8 @@ class OracleBatch:
         self.wl = wl
         self.cfg = OracleConfig(G=wl.G, d=wl.d, max_ctx=wl.max_ctx, sink=wl.sink, recent=wl.recent, k_cap=wl.k_cap,
                                 cond_cap=wl.cond_cap, accum_window=wl.accum_window, sm_scale=float(wl.sm_scale),
-                                pool_kernel=wl.pool_kernel)
+                                pool_kernel=wl.pool_kernel, cond_merge=wl.cond_merge,
+                                kv_bf16=int(wl.dtype == "bf16"))
         self.units = []
         for b in range(wl.B):
             for h in range(wl.Hkv):

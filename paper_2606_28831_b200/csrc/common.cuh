@@ -1,5 +1,6 @@
 // common.cuh -- shared device helpers of libhardkv (sm_100a). Product code: never includes oracle/.
 #pragma once
+#include <cuda_bf16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include "../../include/hardkv.h"
@@ -25,6 +26,7 @@ struct Params {
   int sel_slice_cap;     // capacity (tokens) of one CTA's probability slice in shared memory
   float *pooled;         // [B][Hq][max_ctx] max-pooled logits of SNAPKV heads (NULL when pool_kernel <= 1)
   int pool_kernel;       // SNAPKV max-pool window (odd), <= 1: no SNAPKV head in this config
+  int cond_merge;        // 1: evictees of a full condensed tier are merged into a resident (Appendix G)
 };
 
 // ---- 16-byte vector access -------------------------------------------------------------------
@@ -45,6 +47,9 @@ template <> struct Elem<float> {
     f[0] = __uint_as_float(r.x); f[1] = __uint_as_float(r.y);
     f[2] = __uint_as_float(r.z); f[3] = __uint_as_float(r.w);
   }
+  __device__ static __forceinline__ uint4 pack(const float (&f)[4]) {
+    return make_uint4(__float_as_uint(f[0]), __float_as_uint(f[1]), __float_as_uint(f[2]), __float_as_uint(f[3]));
+  }
 };
 struct bf16_t { uint16_t bits; };
 template <> struct Elem<bf16_t> {
@@ -54,6 +59,12 @@ template <> struct Elem<bf16_t> {
     f[2] = __uint_as_float(r.y << 16); f[3] = __uint_as_float(r.y & 0xffff0000u);
     f[4] = __uint_as_float(r.z << 16); f[5] = __uint_as_float(r.z & 0xffff0000u);
     f[6] = __uint_as_float(r.w << 16); f[7] = __uint_as_float(r.w & 0xffff0000u);
+  }
+  __device__ static __forceinline__ uint4 pack(const float (&f)[8]) {   // round to nearest even
+    auto two = [](float lo, float hi) {
+      return (uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(lo)) | ((uint32_t)__bfloat16_as_ushort(__float2bfloat16_rn(hi)) << 16);
+    };
+    return make_uint4(two(f[0], f[1]), two(f[2], f[3]), two(f[4], f[5]), two(f[6], f[7]));
   }
 };
 

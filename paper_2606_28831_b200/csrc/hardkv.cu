@@ -137,9 +137,10 @@ Params params_of(const hardkv_ctx *ctx, const hardkv_state *s) {
 // bf16 tensor-core paths (variant 1); fp32 K/V and variant 0 run the generic FMA kernels
 bool fast_path(const hardkv_ctx *ctx) { return ctx->variant >= 1 && ctx->cfg.kv_dtype == HARDKV_BF16; }
 
-void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, cudaStream_t st) {
+void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, const void *q,
+                   cudaStream_t st) {
   ctx->launches += 1;
-  HK_DISPATCH_TD(ctx->cfg, (append_retire_kernel<T, D><<<P.B, 256, 0, st>>>(P, k_new, v_new)));
+  HK_DISPATCH_TD(ctx->cfg, (append_retire_kernel<T, D><<<P.B, 256, 0, st>>>(P, k_new, v_new, q)));
 }
 
 void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
@@ -272,6 +273,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.score_stats = reinterpret_cast<float2 *>(base + w.stats);
   P.score_chunks = score_chunks_of(*cfg);
   P.pool_kernel = cfg->pool_kernel;
+  P.cond_merge = cfg->cond_merge != 0;
   P.pooled = cfg->pool_kernel > 1 ? reinterpret_cast<float *>(base + w.pooled) : nullptr;
   ctx->stage_q = base + w.stage_q; ctx->stage_k = base + w.stage_k; ctx->stage_v = base + w.stage_v;
   ctx->stage_out = reinterpret_cast<float *>(base + w.stage_out);
@@ -315,7 +317,14 @@ hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant) {
 hardkv_status hardkv_append_kv(hardkv_ctx *ctx, const hardkv_state *s, const void *k_new, const void *v_new,
                                hardkv_stream st) {
   if (!state_ok(ctx, s) || !k_new || !v_new) return HARDKV_ERR_INVALID_ARG;
-  launch_append(ctx, params_of(ctx, s), k_new, v_new, st);
+  launch_append(ctx, params_of(ctx, s), k_new, v_new, nullptr, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_append_kv_merge(hardkv_ctx *ctx, const hardkv_state *s, const void *k_new, const void *v_new,
+                                     const void *q, hardkv_stream st) {
+  if (!state_ok(ctx, s) || !k_new || !v_new || !q) return HARDKV_ERR_INVALID_ARG;
+  launch_append(ctx, params_of(ctx, s), k_new, v_new, q, st);
   return launch_status();
 }
 
@@ -391,7 +400,7 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
     return HARDKV_ERR_INVALID_ARG;
   const Params P = params_of(ctx, s);
   if (do_select < 0 || do_select > 3) return HARDKV_ERR_INVALID_ARG;
-  launch_append(ctx, P, k_new, v_new, st);
+  launch_append(ctx, P, k_new, v_new, q, st);
   if (do_select == HARDKV_STEP_SELECT_REWRITE || do_select == HARDKV_STEP_SELECT_SPARSE) {
     launch_score(ctx, P, q, st);
     launch_pool(ctx, P, st);

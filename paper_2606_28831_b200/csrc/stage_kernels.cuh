@@ -13,9 +13,12 @@ namespace hardkv {
 // every warp before the barrier and written by thread 0 after it).
 // =============================================================================================
 template <typename T, int D>
-__global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void *k_new, const void *v_new) {
+__global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void *k_new, const void *v_new, const void *q_) {
   constexpr int ROWB = D * sizeof(T);
   constexpr int LPR = ROWB / 16;  // 16-byte vectors per row
+  constexpr int EPL = Elem<T>::EPL;
+  __shared__ float s_qbar[8][D];  // per warp: group mean of the step's queries (merging only)
+  const bool merging = P.cond_merge && q_ != nullptr && P.cond_cap > 0;
   const int b = blockIdx.x, lane = threadIdx.x & 31;
   const int n = P.st.ctx_len[b];
   const int clo0 = P.st.c_lo[b];
@@ -46,9 +49,11 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
     int32_t *cvot = P.st.cond_votes + (size_t)unit * P.cond_cap;
     const int32_t *votes = P.st.votes + (size_t)unit * P.max_ctx;
     clo = clo0;
+    bool qbar_ready = false;
     while (n1 - P.recent - clo > lup) {
       const int t = clo;
       int slot = -1;
+      const bool full = cnt >= P.cond_cap && P.cond_cap > 0;   // a full tier produces an evictee (merging, reading C17)
       if (cnt < P.cond_cap) {
         slot = cnt++;
       } else if (P.cond_cap > 0) {
@@ -67,11 +72,19 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
         }
         if (votes[t] >= (int32_t)(best >> 32)) slot = best_slot;  // newcomer wins ties (it is newer)
       }
+      const char *sk = paged_row<T, D>(P.st.k_pool, tab, t);
+      const char *sv = paged_row<T, D>(P.st.v_pool, tab, t);
+      char *ck = reinterpret_cast<char *>(P.st.cond_k) + (size_t)unit * P.cond_cap * ROWB;
+      char *cv = reinterpret_cast<char *>(P.st.cond_v) + (size_t)unit * P.cond_cap * ROWB;
+      uint4 ek = make_uint4(0, 0, 0, 0), ev = ek;   // evictee pieces (lanes < LPR)
+      if (merging && full && lane < LPR) {
+        // the displaced resident (newcomer won) or the newcomer itself (it lost) is the evictee
+        ek = slot >= 0 ? ldg_ca(ck + (size_t)slot * ROWB + lane * 16) : ldg_ca(sk + lane * 16);
+        ev = slot >= 0 ? ldg_ca(cv + (size_t)slot * ROWB + lane * 16) : ldg_ca(sv + lane * 16);
+      }
       if (slot >= 0) {
-        const char *sk = paged_row<T, D>(P.st.k_pool, tab, t);
-        const char *sv = paged_row<T, D>(P.st.v_pool, tab, t);
-        char *dk = reinterpret_cast<char *>(P.st.cond_k) + ((size_t)unit * P.cond_cap + slot) * ROWB;
-        char *dv = reinterpret_cast<char *>(P.st.cond_v) + ((size_t)unit * P.cond_cap + slot) * ROWB;
+        char *dk = ck + (size_t)slot * ROWB;
+        char *dv = cv + (size_t)slot * ROWB;
         for (int c = lane; c < LPR; c += 32) {
           stg(dk + c * 16, ldg_ca(sk + c * 16));
           stg(dv + c * 16, ldg_ca(sv + c * 16));
@@ -79,6 +92,66 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
         if (lane == 0) { cpos[slot] = t; cvot[slot] = votes[t]; }
       }
       __syncwarp();
+      if (merging && full) {
+        // ---- LSE-preserving weighted merging (Appendix G Eq. 9, Thm G.1; reading C17): fold the evictee into
+        //      the resident with the highest group-mean score under this step's queries ----
+        const int w = threadIdx.x >> 5;
+        if (!qbar_ready) {
+          for (int e = lane; e < D; e += 32) {
+            float acc = 0.f;
+            for (int g = 0; g < P.G; ++g) {
+              const T *qp = reinterpret_cast<const T *>(q_) + ((size_t)(b * P.Hq + h * P.G + g)) * D + e;
+              float f;
+              if (sizeof(T) == 4) f = *reinterpret_cast<const float *>(qp);
+              else f = __uint_as_float((uint32_t)*reinterpret_cast<const uint16_t *>(qp) << 16);
+              acc += f;
+            }
+            s_qbar[w][e] = acc / (float)P.G;
+          }
+          __syncwarp();
+          qbar_ready = true;
+        }
+        float bx = -INFINITY;
+        int br = 0x7fffffff;
+        for (int r = lane; r < cnt; r += 32) {
+          float dot = 0.f;
+#pragma unroll 4
+          for (int c = 0; c < LPR; ++c) {
+            float f[EPL];
+            Elem<T>::unpack(ldg_ca(ck + (size_t)r * ROWB + c * 16), f);
+#pragma unroll
+            for (int i = 0; i < EPL; ++i) dot = fmaf(f[i], s_qbar[w][c * EPL + i], dot);
+          }
+          const float x = P.sm_scale * dot;
+          if (x > bx) { bx = x; br = r; }
+        }
+#pragma unroll
+        for (int o = 16; o; o >>= 1) {
+          const float ox = __shfl_xor_sync(0xffffffffu, bx, o);
+          const int orr = __shfl_xor_sync(0xffffffffu, br, o);
+          if (ox > bx || (ox == bx && orr < br)) { bx = ox; br = orr; }
+        }
+        float fe[EPL], fv[EPL];
+        Elem<T>::unpack(ek, fe);
+        Elem<T>::unpack(ev, fv);
+        float de = 0.f;
+        if (lane < LPR) {
+#pragma unroll
+          for (int i = 0; i < EPL; ++i) de = fmaf(fe[i], s_qbar[w][lane * EPL + i], de);
+        }
+        const float xe = P.sm_scale * warp_sum_f32(de);
+        const float wa = 1.0f / (1.0f + expf(xe - bx)), we = 1.0f - wa;
+        if (lane < LPR) {
+          float fa[EPL], fb[EPL];
+          Elem<T>::unpack(ldg_ca(ck + (size_t)br * ROWB + lane * 16), fa);
+          Elem<T>::unpack(ldg_ca(cv + (size_t)br * ROWB + lane * 16), fb);
+#pragma unroll
+          for (int i = 0; i < EPL; ++i) { fa[i] = fmaf(wa, fa[i], we * fe[i]); fb[i] = fmaf(wa, fb[i], we * fv[i]); }
+          stg(ck + (size_t)br * ROWB + lane * 16, Elem<T>::pack(fa));
+          stg(cv + (size_t)br * ROWB + lane * 16, Elem<T>::pack(fb));
+        }
+        __syncwarp();
+      }
       ++clo;
     }
     if (lane == 0) P.st.cond_count[unit] = cnt;

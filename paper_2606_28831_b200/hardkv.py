@@ -39,7 +39,7 @@ def build(force: bool = False) -> str:
 class Config(C.Structure):
     _fields_ = [(n, C.c_int32) for n in (
         "batch", "num_q_heads", "num_kv_heads", "head_dim", "page_size", "max_ctx", "sink", "recent", "k_cap",
-        "cond_cap", "accum_window", "kv_dtype")] + [("sm_scale", C.c_float), ("pool_kernel", C.c_int32)]
+        "cond_cap", "accum_window", "kv_dtype")] + [("sm_scale", C.c_float), ("pool_kernel", C.c_int32), ("cond_merge", C.c_int32)]
 
 
 _STATE_FIELDS = ["k_pool", "v_pool", "base_table", "sel_k_pool", "sel_v_pool", "sel_pages", "cond_k", "cond_v",
@@ -55,7 +55,7 @@ class StateStruct(C.Structure):
 F32, BF16 = 0, 1
 STEP_REUSE_TIER, STEP_SELECT_REWRITE, STEP_SELECT_SPARSE, STEP_REUSE_SPARSE = 0, 1, 2, 3   # do_select of decode_step
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
-           "hardkv_set_variant", "hardkv_append_kv", "hardkv_score", "hardkv_calibrate_topp", "hardkv_solve_temperature",
+           "hardkv_set_variant", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_calibrate_topp", "hardkv_solve_temperature",
            "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend", "hardkv_sparse_attend",
            "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count"]
 
@@ -74,6 +74,7 @@ def _load():
     lib.hardkv_status_string.restype = C.c_char_p
     lib.hardkv_set_variant.argtypes = [vp, C.c_int32]
     lib.hardkv_append_kv.argtypes = [vp, sp, vp, vp, vp]
+    lib.hardkv_append_kv_merge.argtypes = [vp, sp, vp, vp, vp, vp]
     lib.hardkv_score.argtypes = [vp, sp, vp, vp]
     lib.hardkv_calibrate_topp.argtypes = [vp, sp, C.c_float, vp]
     lib.hardkv_solve_temperature.argtypes = [vp, sp, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int32, vp]
@@ -135,9 +136,9 @@ class HardKV:
     """One hardkv_ctx.  Every method enqueues kernels on torch's current stream and returns at once."""
 
     def __init__(self, *, batch, num_q_heads, num_kv_heads, head_dim, max_ctx, sink, recent, k_cap, cond_cap,
-                 kv_dtype, accum_window=0, page_size=16, sm_scale=0.0, pool_kernel=0, device="cuda:0"):
+                 kv_dtype, accum_window=0, page_size=16, sm_scale=0.0, pool_kernel=0, cond_merge=0, device="cuda:0"):
         self.cfg = Config(batch, num_q_heads, num_kv_heads, head_dim, page_size, max_ctx, sink, recent, k_cap,
-                          cond_cap, accum_window, kv_dtype, sm_scale, pool_kernel)
+                          cond_cap, accum_window, kv_dtype, sm_scale, pool_kernel, cond_merge)
         nbytes = C.c_size_t()
         _check(lib.hardkv_workspace_bytes(C.byref(self.cfg), C.byref(nbytes)))
         self.workspace = torch.zeros(nbytes.value + 256, dtype=torch.uint8, device=device)
@@ -156,6 +157,9 @@ class HardKV:
 
     def append_kv(self, st: DeviceState, k_new, v_new):
         _check(lib.hardkv_append_kv(self._ctx, C.byref(st.struct()), _ptr(k_new), _ptr(v_new), _stream()))
+
+    def append_kv_merge(self, st: DeviceState, k_new, v_new, q):
+        _check(lib.hardkv_append_kv_merge(self._ctx, C.byref(st.struct()), _ptr(k_new), _ptr(v_new), _ptr(q), _stream()))
 
     def score(self, st: DeviceState, q):
         _check(lib.hardkv_score(self._ctx, C.byref(st.struct()), _ptr(q), _stream()))

@@ -22,7 +22,7 @@ def make_engine(wl: Workload, device="cuda:0", want_accum=None) -> hardkv.HardKV
                          sink=wl.sink, recent=wl.recent, k_cap=wl.k_cap, cond_cap=wl.cond_cap,
                          kv_dtype=hardkv.BF16 if wl.dtype == "bf16" else hardkv.F32,
                          accum_window=wl.accum_window if accum else 0, sm_scale=float(wl.sm_scale),
-                         pool_kernel=wl.pool_kernel, device=device)
+                         pool_kernel=wl.pool_kernel, cond_merge=wl.cond_merge, device=device)
 
 
 def to_dev(x: np.ndarray, wl: Workload, device="cuda:0") -> torch.Tensor:

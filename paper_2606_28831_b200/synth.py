@@ -70,6 +70,7 @@ class Workload:
     l_lower: np.ndarray = None       # [B]
     accum_window: int = 32
     pool_kernel: int = 0             # SNAPKV max-pool window (odd; 0: no SNAPKV head)
+    cond_merge: int = 0              # 1: condensed-tier evictees are merged (Appendix G) instead of dropped
     seed: int = 0
     temperature: np.ndarray = field(default=None)  # [B][Hkv] calibration T (reading C10: 1)
 

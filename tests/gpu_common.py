@@ -51,8 +51,13 @@ class Pair:
             c = u.cond_count
             np.testing.assert_array_equal(cpos[i, :c], u.cond_pos[:c])
             np.testing.assert_array_equal(cvot[i, :c], u.cond_votes[:c])
-            np.testing.assert_array_equal(ck[i, :c], u.cond_k[:c])   # row copies: bit exact
-            np.testing.assert_array_equal(cv[i, :c], u.cond_v[:c])
+            if wl.cond_merge:    # merged rows: fp32 vs fp64 arithmetic before the store rounding, one ulp of kv_dtype
+                tol = dict(rtol=2.0 ** -7, atol=1e-6) if wl.dtype == "bf16" else dict(rtol=1e-5, atol=1e-6)
+                np.testing.assert_allclose(ck[i, :c], u.cond_k[:c], **tol)
+                np.testing.assert_allclose(cv[i, :c], u.cond_v[:c], **tol)
+            else:
+                np.testing.assert_array_equal(ck[i, :c], u.cond_k[:c])   # row copies: bit exact
+                np.testing.assert_array_equal(cv[i, :c], u.cond_v[:c])
 
     def check_votes(self):
         votes = np_of(self.st.votes)

@@ -32,7 +32,7 @@ def test_header_symbols_exported(lib):
 
 
 def test_struct_layout_matches_header(lib):
-    assert C.sizeof(lib.Config) == 14 * 4
+    assert C.sizeof(lib.Config) == 15 * 4
     assert C.sizeof(lib.StateStruct) == 28 * C.sizeof(C.c_void_p)
 
 

@@ -329,3 +329,50 @@ def test_solve_temperature(name, P):
         u.topp_select(wl.p, True)
     pr.check_probs()
     pr.check_selection_band()
+
+
+MERGE_WL = {
+    # fp32, G = 4: the first step retires 45 tokens at once into 4 slots (loop of merges inside one call)
+    "merge0": make_workload(0, l_upper=i32(400), cond_cap=4, cond_merge=1),
+    # bf16, G = 4, three sequences of different lengths, one retirement per step, tier full after 6 steps
+    "merge4": make_workload(2, B=3, n0=i32(900, 2300, 1500), max_ctx=2400, k_cap=256,
+                            l_upper=i32(900 - 132, 2300 - 132, 1500 - 132), cond_cap=6, steps=14, cond_merge=1),
+    # bf16, G = 7 with mixed new keys: the first step retires 11 tokens into 8 slots, then one per step
+    "merge7": make_workload(3, B=2, n0=i32(300, 300), max_ctx=512, k_cap=64, l_upper=i32(30, 30), cond_cap=8,
+                            steps=14, cond_merge=1),
+}
+
+
+@pytest.mark.parametrize("name", list(MERGE_WL))
+def test_condensed_tier_weighted_merging(name, P):
+    """cfg.cond_merge: evictees of the full condensed tier are folded into the best-scoring resident with the
+    LSE-preserving weights of Appendix G (Eq. 9) -- stand-alone entry and fused step against the oracle.  Slots,
+    positions and votes are exact; merged rows agree to one ulp of kv_dtype (fp32 vs fp64 before the store
+    rounding); the state is teacher-forced after every step."""
+    wl = MERGE_WL[name]
+    pr = P(wl, want_mask=False)
+    merged_any = False
+    for t in range(min(wl.steps, 14)):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        full_before = [u.cond_count == wl.cond_cap for u in pr.ob.units]
+        if t % 2 == 0:     # the stand-alone entry, then the rest of the step from its stages
+            pr.eng.append_kv_merge(pr.st, knd, vnd, qd)
+            qu = q.reshape(-1, wl.G, wl.d)
+            for i, u in enumerate(pr.ob.units):
+                u.append(kn.reshape(-1, wl.d)[i], vn.reshape(-1, wl.d)[i])
+                merged_any |= bool(u.retire_q(qu[i]) and full_before[i])
+            pr.check_bookkeeping()
+            pr.force_discrete_state()
+            pr.eng.score(pr.st, qd)
+            pr.eng.calibrate_topp(pr.st, wl.p)
+            pr.eng.rewrite_attend(pr.st, qd, pr.out, pr.lse)
+            for i, u in enumerate(pr.ob.units):
+                u.score(qu[i]); u.calibrate(); u.topp_select(wl.p, True); u.rewrite(); u.attend(qu[i])
+        else:
+            pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)
+            pr.ob.step(q, kn, vn, wl.p)
+            pr.check_bookkeeping()
+        pr.check_out(f"{name} step {t}")
+        pr.check_selection_band()
+        pr.force_discrete_state()
+    assert merged_any
