@@ -175,6 +175,12 @@ def run_cuda(args):
     if args.n0:
         B0 = sharding.rank_workload(args.config, 0).B
         over["n0"] = np.full(B0, args.n0, np.int32)
+    if args.snapkv_window:
+        hk = sharding.rank_workload(args.config, 0).Hkv
+        over["score_mode"] = np.array([2 * (h % 2) for h in range(hk)], np.uint8)
+        over["pool_kernel"] = args.snapkv_window
+    if args.cond_merge:
+        over["cond_merge"] = 1
     wl = sharding.rank_workload(args.config, rank, **over)   # every rank: its own batch of the same shape
     if args.p:
         wl.p = args.p
@@ -303,6 +309,16 @@ def run_cuda(args):
     sparse_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out, do_select=2))
     sparse_amortised_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out,
                                                                do_select=2 if ((t - W) // L) % SI == 0 else 3))
+    solve_us = None
+    if args.snapkv_window:   # Algorithm 2 (L625-648), run once per request (L607): timed on the first step's logits
+        warm()
+        eng.append_kv(states[0], k_d[W], v_d[W]); eng.score(states[0], q_d[W])
+        a_, b2_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a_.record(stream)
+        eng.solve_temperature(states[0], wl.p, t_min=0.0625, t_max=16.0, eps=1e-5, max_iter=40)
+        b2_.record(stream)
+        torch.cuda.synchronize()
+        solve_us = a_.elapsed_time(b2_) * 1e3
     row_b = wl.d * (2 if wl.dtype == "bf16" else 4)
     units_ = wl.B * wl.Hkv
     kv_base = float(2 * row_b * wl.Hkv * (wl.n0.sum() + wl.B * (W + K / 2)))     # live base-pool K + V rows
@@ -348,6 +364,7 @@ def run_cuda(args):
             "config": {"workload": f"BASELINE.json configs[{args.config}] ({wl.name})", "batch": wl.B,
                        "q_heads": wl.Hq, "kv_heads": wl.Hkv, "head_dim": wl.d, "ctx": [int(wl.n0.min()), int(wl.n0.max())],
                        "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": L, "variant": args.variant,
+                       "snapkv_window": args.snapkv_window, "cond_merge": bool(args.cond_merge),
                        "launch": "eager" if args.eager else "one CUDA graph of the K steps",
                        "l2": "inputs larger than L2 (K scan %.0f MB per layer-step x %d layer(s) of distinct data cycled), "
                              "no flush" % (per_step[0]["score"] / 1e6, L),
@@ -376,6 +393,7 @@ def run_cuda(args):
                 "note": "analogue of the paper's MTI (L205, L504-515): resident KV bytes x time per step in the amortised "
                         "regime; this build keeps the candidate pool resident in both layouts, so HA-Max pays the static "
                         "selected tier on top"},
+            "solve_temperature_us": solve_us,
             "roofline": roof,
             "e2e": {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "us_per_layer_step": ms_e2e / K * 1e3, "sync": "stream sync after every step"},
@@ -412,6 +430,10 @@ def main():
                     "single-layer K fits L2, else 1)")
     ap.add_argument("--n0", type=int, default=0, help="override: uniform prefill context (config 3 checkpoints)")
     ap.add_argument("--variant", type=int, default=1, help="kernel variant (hardkv_set_variant): 1 default, 2 TMA score, 3 async attention")
+    ap.add_argument("--snapkv-window", type=int, default=0, help="odd window: odd KV heads use the SNAPKV max-pool metric "
+                    "(L278) and the line reports the Algorithm 2 temperature solve; not the BASELINE workload")
+    ap.add_argument("--cond-merge", action="store_true", help="condensed-tier evictees are merged (Appendix G) instead "
+                    "of dropped; not the BASELINE workload")
     ap.add_argument("--p", type=float, default=0.0, help="override the nucleus mass (config 4 sweep)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup

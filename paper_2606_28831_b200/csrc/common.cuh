@@ -29,6 +29,15 @@ struct Params {
   int cond_merge;        // 1: evictees of a full condensed tier are merged into a resident (Appendix G)
 };
 
+// ---- programmatic dependent launch (PDL): every hot kernel waits here for the preceding kernel of the stream to complete
+// and flush before it touches memory, then lets its own successor be scheduled onto SMs as they drain -- the launch
+// latency between the dependent kernels of a step overlaps the tail of the previous kernel.  Both are no-ops when the
+// kernel was launched without the attribute.
+__device__ __forceinline__ void pdl_wait_then_trigger() {
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+
 // ---- 16-byte vector access -------------------------------------------------------------------
 __device__ __forceinline__ uint4 ldg_nc(const void *p) {   // streaming read-only data (K, V rows)
   uint4 v;

@@ -72,6 +72,7 @@ __host__ __device__ __forceinline__ int sel_slice_len(int span, int C) {
 // GMAX: compile-time bound of the GQA group (4 or 8) -- sizes the register arrays of the calibration.
 template <int CALIBRATE, int GMAX>
 __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
+  pdl_wait_then_trigger();
   extern __shared__ __align__(16) unsigned char sel_smem[];
   cg::cluster_group cluster = cg::this_cluster();
   const int C = P.sel_cluster;

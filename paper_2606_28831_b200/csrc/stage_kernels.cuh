@@ -14,6 +14,7 @@ namespace hardkv {
 // =============================================================================================
 template <typename T, int D>
 __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void *k_new, const void *v_new, const void *q_) {
+  pdl_wait_then_trigger();
   constexpr int ROWB = D * sizeof(T);
   constexpr int LPR = ROWB / 16;  // 16-byte vectors per row
   constexpr int EPL = Elem<T>::EPL;
