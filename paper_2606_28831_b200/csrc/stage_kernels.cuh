@@ -33,6 +33,9 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
   for (int h = threadIdx.x >> 5; h < P.Hkv; h += blockDim.x >> 5) {
     const int unit = b * P.Hkv + h;
     const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
+    // the kernel is a chain of dependent loads (latency bound): everything the retirement needs that does not depend
+    // on the append is loaded before the append's stores, so the loads overlap instead of queueing behind them
+    int cnt = P.st.cond_count[unit];
     // Step 1: "linearly append KV pairs to the Tier 1 Dense Cache" (L78)
     {
       char *dk = const_cast<char *>(paged_row<T, D>(P.st.k_pool, tab, n));
@@ -45,7 +48,6 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
       }
     }
     // Step 4: while the pool exceeds l_upper its oldest token t = c_lo retires.
-    int cnt = P.st.cond_count[unit];
     int32_t *cpos = P.st.cond_pos + (size_t)unit * P.cond_cap;
     int32_t *cvot = P.st.cond_votes + (size_t)unit * P.cond_cap;
     const int32_t *votes = P.st.votes + (size_t)unit * P.max_ctx;
@@ -55,15 +57,28 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
       const int t = clo;
       int slot = -1;
       const bool full = cnt >= P.cond_cap && P.cond_cap > 0;   // a full tier produces an evictee (merging, reading C17)
+      const int votes_t = votes[t];                             // in flight together with the scan below
+      const char *sk = paged_row<T, D>(P.st.k_pool, tab, t);
+      const char *sv = paged_row<T, D>(P.st.v_pool, tab, t);
       if (cnt < P.cond_cap) {
         slot = cnt++;
       } else if (P.cond_cap > 0) {
-        // resident with the lexicographically smallest (votes, pos)
+        // resident with the lexicographically smallest (votes, pos): 8 slots per lane loaded as one batch
         unsigned long long best = ~0ull;
         int best_slot = 0;
-        for (int j = lane; j < P.cond_cap; j += 32) {
-          unsigned long long key = ((unsigned long long)(uint32_t)cvot[j] << 32) | (uint32_t)cpos[j];
-          if (key < best) { best = key; best_slot = j; }
+        for (int j0 = 0; j0 < P.cond_cap; j0 += 256) {
+          int32_t kv[8], kp[8];
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const int j = j0 + lane + 32 * i;
+            kv[i] = j < P.cond_cap ? cvot[j] : 0x7fffffff;
+            kp[i] = j < P.cond_cap ? cpos[j] : 0x7fffffff;
+          }
+#pragma unroll
+          for (int i = 0; i < 8; ++i) {
+            const unsigned long long key = ((unsigned long long)(uint32_t)kv[i] << 32) | (uint32_t)kp[i];
+            if (key < best) { best = key; best_slot = j0 + lane + 32 * i; }
+          }
         }
 #pragma unroll
         for (int o = 16; o; o >>= 1) {
@@ -71,10 +86,8 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
           int os = __shfl_xor_sync(0xffffffffu, best_slot, o);
           if (ob < best) { best = ob; best_slot = os; }
         }
-        if (votes[t] >= (int32_t)(best >> 32)) slot = best_slot;  // newcomer wins ties (it is newer)
+        if (votes_t >= (int32_t)(best >> 32)) slot = best_slot;  // newcomer wins ties (it is newer)
       }
-      const char *sk = paged_row<T, D>(P.st.k_pool, tab, t);
-      const char *sv = paged_row<T, D>(P.st.v_pool, tab, t);
       char *ck = reinterpret_cast<char *>(P.st.cond_k) + (size_t)unit * P.cond_cap * ROWB;
       char *cv = reinterpret_cast<char *>(P.st.cond_v) + (size_t)unit * P.cond_cap * ROWB;
       uint4 ek = make_uint4(0, 0, 0, 0), ev = ek;   // evictee pieces (lanes < LPR)
@@ -90,7 +103,7 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
           stg(dk + c * 16, ldg_ca(sk + c * 16));
           stg(dv + c * 16, ldg_ca(sv + c * 16));
         }
-        if (lane == 0) { cpos[slot] = t; cvot[slot] = votes[t]; }
+        if (lane == 0) { cpos[slot] = t; cvot[slot] = votes_t; }
       }
       __syncwarp();
       if (merging && full) {

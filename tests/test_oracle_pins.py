@@ -573,3 +573,29 @@ def test_p15_displaced_resident_is_merged_and_bf16_store():
     got = u.cond_k[a]
     assert np.all((got.view(np.uint32) & 0xffff) == 0)                                # bf16-representable
     np.testing.assert_allclose(got, exact, rtol=2.0 ** -8, atol=1e-30)
+
+
+# ---- golden fixtures: closed-form roots T* of Problem 1 (tests/golden/temperature_roots.txt; written by
+#      tests/golden/make_temperature_roots.py from the geometric sums, scipy only) -------------------------------
+def _root_rows():
+    import os
+    path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "temperature_roots.txt")
+    rows = []
+    for line in open(path):
+        line = line.strip()
+        if line and not line.startswith("#"):
+            lam, N, r, p, k, T = line.split()
+            rows.append((float(lam), int(N), int(r), float(p), int(k), float(T)))
+    return rows
+
+
+@pytest.mark.parametrize("lam,N,r,p,k,Tstar", _root_rows())
+def test_golden_temperature_roots(lam, N, r, p, k, Tstar):
+    cfg = OracleConfig(G=1, d=64, max_ctx=(N + 20 + 15) // 16 * 16, sink=4, recent=16, k_cap=(N + 20 + 15) // 16 * 16,
+                       cond_cap=8, pool_kernel=2 * r + 1)
+    K0 = np.zeros((N + 20, 64), np.float32)
+    u = Unit(cfg, K0, K0.copy(), l_upper=10**6, score_mode=2)
+    _set_logits(u, -lam * np.arange(N)[None, :])
+    it, resid = u.solve_temperature(p, t_min=0.25, t_max=4.0, eps=1e-7, max_iter=60)
+    assert u.k_topp == k
+    assert abs(u.T - Tstar) < 2e-3 * Tstar, (u.T, Tstar)
