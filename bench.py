@@ -392,6 +392,10 @@ def run_cuda(args):
                        "parallelism": f"units sharded, {world} rank(s), no collective"},
             "us_per_layer_step": us_step,
             "tokens_per_s_layer": wl.B * world / (us_step * 1e-6),
+            # attention-path only: a model of L_model layers runs L_model layer-steps per token
+            "tokens_per_s_model_attention_path": wl.B * world / (us_step * 1e-6) / L_MODEL.get(args.config, 32),
+            "l_model": L_MODEL.get(args.config, 32),
+            "traffic_vs_dense_attention": float(np.mean([p["total"] / max(p["dense_attention_bytes"], 1) for p in per_step])),
             "frac_of_8TBs": gbs / world / NOMINAL_HBM_GBS,
             "frac_of_measured_copy": gbs / world / peak,
             "algorithmic_bytes_per_step": bytes_all / K / world,
@@ -437,6 +441,9 @@ def run_cuda(args):
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
+
+
+L_MODEL = {0: 1, 1: 32, 2: 32, 3: 28, 4: 40}   # layers of the model each config is shaped after
 
 
 def main():

@@ -376,3 +376,23 @@ def test_condensed_tier_weighted_merging(name, P):
         pr.check_selection_band()
         pr.force_discrete_state()
     assert merged_any
+
+
+@pytest.mark.parametrize("name,steps", [("c2s", 64), ("c4s", 48), ("snap7", 40)])
+def test_long_teacher_forced_trajectory(name, steps, P):
+    """Many fused steps in a row (votes accumulate, the condensed tier fills and turns over, the ACCUM ring wraps
+    several times, the context grows across page and chunk boundaries): every step judged against the oracle."""
+    import dataclasses
+    wl = dataclasses.replace(WL[name], steps=steps, max_ctx=WL[name].max_ctx + 64)
+    pr = P(wl, want_mask=False)
+    for t in range(steps):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)
+        pr.ob.step(q, kn, vn, wl.p)
+        pr.check_out(f"{name} step {t}")
+        if pr.check_selection_band() == 0:
+            pr.check_bookkeeping()
+            pr.check_votes()
+        pr.force_discrete_state()
+    if name != "snap7":
+        assert all(u.cond_count == wl.cond_cap for u in pr.ob.units)      # the condensed tier did fill
