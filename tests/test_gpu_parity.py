@@ -396,3 +396,35 @@ def test_long_teacher_forced_trajectory(name, steps, P):
         pr.force_discrete_state()
     if name != "snap7":
         assert all(u.cond_count == wl.cond_cap for u in pr.ob.units)      # the condensed tier did fill
+
+
+def test_paper_regime_hysteresis_and_interval(P):
+    """The paper's periodic regime on one trajectory (L197, L270, L274): compression every 4th step, L_lower =
+    L_upper - 20.  The pool starts below L_lower (everything is selected: no sparsity yet), grows past it (Top-p
+    selection), then past L_upper (the oldest tokens retire into the condensed tier); the steps in between reuse the
+    rewritten tier (HA-Max, do_select = 0)."""
+    wl = make_workload(1, Hq=8, Hkv=2, n0=i32(700), max_ctx=800, k_cap=640, l_upper=i32(620), cond_cap=8, steps=72)
+    wl.l_lower = i32(600)
+    pr = P(wl, want_mask=False)
+    phases = set()
+    for t in range(72):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        sel = t % 4 == 0
+        pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse, do_select=sel)
+        pr.ob.step(q, kn, vn, wl.p, do_select=sel)
+        pr.check_out(f"paper regime step {t}")
+        u = pr.ob.units[0]
+        lo, hi = u.pool
+        if sel:
+            pr.check_selection_band()
+            if hi - lo <= 600:
+                assert u.sel_count == hi - lo
+                phases.add("all")
+            else:
+                assert u.sel_count < hi - lo
+                phases.add("topp")
+        if u.cond_count > 0:
+            phases.add("retire")
+        pr.check_bookkeeping()
+        pr.force_discrete_state()
+    assert phases == {"all", "topp", "retire"}
