@@ -181,6 +181,8 @@ def run_cuda(args):
         over["pool_kernel"] = args.snapkv_window
     if args.cond_merge:
         over["cond_merge"] = 1
+    if args.contiguous_pages:
+        over["contiguous_pages"] = True
     wl = sharding.rank_workload(args.config, rank, **over)   # every rank: its own batch of the same shape
     if args.p:
         wl.p = args.p
@@ -386,6 +388,7 @@ def run_cuda(args):
                        "q_heads": wl.Hq, "kv_heads": wl.Hkv, "head_dim": wl.d, "ctx": [int(wl.n0.min()), int(wl.n0.max())],
                        "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": L, "variant": args.variant,
                        "snapkv_window": args.snapkv_window, "cond_merge": bool(args.cond_merge),
+                       "page_ids": "identity (diagnostic)" if args.contiguous_pages else "seeded permutation (random block ids, L460)",
                        "launch": "eager" if args.eager else "one CUDA graph of the K steps",
                        "l2": "inputs larger than L2 (K scan %.0f MB per layer-step x %d layer(s) of distinct data cycled), "
                              "no flush" % (per_step[0]["score"] / 1e6, L),
@@ -463,6 +466,8 @@ def main():
     ap.add_argument("--variant", type=int, default=1, help="kernel variant (hardkv_set_variant): 1 default, 2 TMA score, 3 async attention")
     ap.add_argument("--snapkv-window", type=int, default=0, help="odd window: odd KV heads use the SNAPKV max-pool metric "
                     "(L278) and the line reports the Algorithm 2 temperature solve; not the BASELINE workload")
+    ap.add_argument("--contiguous-pages", action="store_true", help="diagnostic: identity page ids instead of the seeded "
+                    "random block ids (L460); not the BASELINE workload")
     ap.add_argument("--cond-merge", action="store_true", help="condensed-tier evictees are merged (Appendix G) instead "
                     "of dropped; not the BASELINE workload")
     ap.add_argument("--p", type=float, default=0.0, help="override the nucleus mass (config 4 sweep)")

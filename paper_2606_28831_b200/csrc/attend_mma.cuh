@@ -151,14 +151,14 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
         if (kd[r] != ROW_INVALID) {
           char *wp = kp1 + (size_t)kd[r] * ROWB + tig * 16;
 #pragma unroll
-          for (int ch = 0; ch < NKC; ++ch) stg(wp + ch * 64, kr[r][ch]);
+          for (int ch = 0; ch < NKC; ++ch) stg_cs(wp + ch * 64, kr[r][ch]);
         }
 #pragma unroll
       for (int r = 0; r < 4; ++r)
         if (vd[r] != ROW_INVALID) {
           char *wp = vp1 + (size_t)vd[r] * ROWB + gid * 16;
 #pragma unroll
-          for (int ch = 0; ch < NVC; ++ch) stg(wp + ch * 128, vr[r][ch]);
+          for (int ch = 0; ch < NVC; ++ch) stg_cs(wp + ch * 128, vr[r][ch]);
         }
     }
     // ---- S^T = Q K^T for the two 8-token blocks ----

@@ -47,6 +47,12 @@ __device__ __forceinline__ uint4 ldg_nc(const void *p) {   // streaming read-onl
 }
 __device__ __forceinline__ uint4 ldg_ca(const void *p) { return *reinterpret_cast<const uint4 *>(p); }
 __device__ __forceinline__ void stg(void *p, uint4 v) { *reinterpret_cast<uint4 *>(p) = v; }
+// streaming store (evict-first in L2): the rewritten tier is not read again before the next step's K scan has pushed
+// it out of L2 anyway, so its write-back should drain during the attention kernel (DRAM at ~40 %) rather than sit
+// dirty in L2 and compete with the bandwidth-bound score kernel of the next step
+__device__ __forceinline__ void stg_cs(void *p, uint4 v) {
+  asm volatile("st.global.cs.v4.u32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
+}
 
 // Elements per 16-byte vector and their widening to fp32 (bf16 -> fp32 is exact: a 16-bit shift).
 template <typename T> struct Elem;

@@ -71,6 +71,7 @@ class Workload:
     accum_window: int = 32
     pool_kernel: int = 0             # SNAPKV max-pool window (odd; 0: no SNAPKV head)
     cond_merge: int = 0              # 1: condensed-tier evictees are merged (Appendix G) instead of dropped
+    contiguous_pages: bool = False   # diagnostic: identity page ids instead of the seeded permutations (L460)
     seed: int = 0
     temperature: np.ndarray = field(default=None)  # [B][Hkv] calibration T (reading C10: 1)
 
@@ -178,6 +179,9 @@ class Workload:
         """base_table [B][Hkv][max_ctx/16], sel_pages [B][Hkv][k_cap/16]: seeded permutations."""
         nb = self.B * self.Hkv * self.pages_per_unit
         ns = self.B * self.Hkv * self.sel_pages_per_unit
+        if self.contiguous_pages:
+            return (np.arange(nb, dtype=np.int32).reshape(self.B, self.Hkv, self.pages_per_unit),
+                    np.arange(ns, dtype=np.int32).reshape(self.B, self.Hkv, self.sel_pages_per_unit))
         g = _rng(self.seed, _T_PAGES)
         base = g.permutation(nb).astype(np.int32).reshape(self.B, self.Hkv, self.pages_per_unit)
         sel = g.permutation(ns).astype(np.int32).reshape(self.B, self.Hkv, self.sel_pages_per_unit)
