@@ -31,8 +31,8 @@ METRIC = "decode_step_kv_bandwidth"      # B_min / time of the fused select+rewr
 UNIT = "GB/s"
 NOMINAL_HBM_GBS = 8000.0                 # the contract's "8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                # B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1_02_final.md), config 2
-NCU_TRAFFIC_BYTES = {2: {"score": 582.6e6, "rewrite_attend": 281.1e6, "calibrate_topp": 41.3e6}}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1_03_final.md), config 2
+NCU_TRAFFIC_BYTES = {2: {"score": 586.3e6, "rewrite_attend": 279.5e6, "calibrate_topp": 41.6e6}}
 
 
 def log(*a):
@@ -370,7 +370,8 @@ def run_cuda(args):
         us_step = ms_total / K * 1e3
         dom = max(("score", "rewrite_attend", "calibrate_topp"), key=lambda s: stage_us[s])
         roof = {"kernel": dom, "bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
-                "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(dom) if not (args.n0 or args.p) else None}
+                "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(dom)
+                if not (args.n0 or args.p or args.snapkv_window or args.cond_merge or args.contiguous_pages) else None}
         if dom in bytes_stage:
             roof["achieved"] = bytes_stage[dom] / (stage_us[dom] * 1e-6) / 1e9
             roof["algorithmic_bytes_per_launch"] = bytes_stage[dom]
