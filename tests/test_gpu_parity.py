@@ -428,3 +428,40 @@ def test_paper_regime_hysteresis_and_interval(P):
         pr.check_bookkeeping()
         pr.force_discrete_state()
     assert phases == {"all", "topp", "retire"}
+
+
+def test_cuda_graph_replay_widened_entries(P):
+    """The widened entry points are capturable too (no allocation, no synchronisation, no host read-back): one graph
+    holding append + merge, score, the Algorithm 2 solve, calibrate + Top-p and the HA-Sparse attention is replayed
+    and compared with the same calls made eagerly on a second, identical engine."""
+    import dataclasses
+    wl = dataclasses.replace(WL["snap4"], cond_merge=1)
+    a, b = P(wl, want_mask=False), P(wl, want_mask=False)
+
+    def calls(pr, qd, knd, vnd):
+        pr.eng.append_kv_merge(pr.st, knd, vnd, qd)
+        pr.eng.score(pr.st, qd)
+        pr.eng.solve_temperature(pr.st, wl.p, t_min=0.0625, t_max=16.0, eps=1e-5, max_iter=30)
+        pr.eng.calibrate_topp(pr.st, wl.p)
+        pr.eng.sparse_attend(pr.st, qd, pr.out, pr.lse)
+
+    q, kn, vn, (qd, knd, vnd) = a.inputs(0)
+    qb, kb, vb = qd.clone(), knd.clone(), vnd.clone()
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        calls(a, qd, knd, vnd)                              # warm-up outside capture (step 0)
+    torch.cuda.current_stream().wait_stream(s)
+    calls(b, qb, kb, vb)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        calls(a, qd, knd, vnd)
+    for t in range(1, 4):
+        _, _, _, (q2, k2, v2) = a.inputs(t)
+        qd.copy_(q2); knd.copy_(k2); vnd.copy_(v2)
+        g.replay()
+        calls(b, q2, k2, v2)
+        torch.cuda.synchronize()
+        for f in ("temperature", "sel_count", "sel_idx", "cond_k", "cond_pos", "votes", "ctx_len", "c_lo"):
+            assert torch.equal(getattr(a.st, f), getattr(b.st, f)), (t, f)
+        assert torch.equal(a.out, b.out) and torch.equal(a.lse, b.lse)
