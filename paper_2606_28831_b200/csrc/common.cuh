@@ -45,6 +45,14 @@ __device__ __forceinline__ uint4 ldg_nc(const void *p) {   // streaming read-onl
                : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
   return v;
 }
+// the same at base + OFF with the offset as an immediate of the instruction (no per-load address arithmetic)
+template <int OFF>
+__device__ __forceinline__ uint4 ldg_nc_off(const void *base) {
+  uint4 v;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4+%5];"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(base), "n"(OFF));
+  return v;
+}
 __device__ __forceinline__ uint4 ldg_ca(const void *p) { return *reinterpret_cast<const uint4 *>(p); }
 __device__ __forceinline__ void stg(void *p, uint4 v) { *reinterpret_cast<uint4 *>(p) = v; }
 // streaming store (evict-first in L2): the rewritten tier is not read again before the next step's K scan has pushed

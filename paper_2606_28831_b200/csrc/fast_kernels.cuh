@@ -56,6 +56,7 @@ __global__ void __launch_bounds__(256) score_mma_kernel(Params P, const void *q_
     }
   }
   const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
+  const char *klane = reinterpret_cast<const char *>(P.st.k_pool) + gid * ROWB + tig * 16;   // this lane's bytes of row gid of page 0
   float *lg = P.st.logits + ((size_t)(b * P.Hq + h * G)) * P.max_ctx;
   const int h0 = 2 * tig, h1 = 2 * tig + 1;
   const float c2 = P.sm_scale * 1.4426950408889634f / P.st.temperature[unit];  // logit -> base-2 exponent of z/T
@@ -74,11 +75,17 @@ __global__ void __launch_bounds__(256) score_mma_kernel(Params P, const void *q_
 #pragma unroll
     for (int u = 0; u < 2; ++u) {
       phys[u] = __shfl_sync(0xffffffffu, my_page, j0 + u);
-      const char *src = reinterpret_cast<const char *>(P.st.k_pool) + (size_t)(phys[u] < 0 ? 0 : phys[u]) * (PAGE * ROWB);
+      if (phys[u] >= 0) {   // warp-uniform; one base per page, every load at an immediate offset from it
+        const char *src = klane + (size_t)phys[u] * (PAGE * ROWB);
+        ka[u][0] = ldg_nc_off<0>(src);             kb[u][0] = ldg_nc_off<8 * ROWB>(src);
+        ka[u][1] = ldg_nc_off<64>(src);            kb[u][1] = ldg_nc_off<8 * ROWB + 64>(src);
+        if (NCH > 2) {
+          ka[u][NCH - 2] = ldg_nc_off<128>(src);   kb[u][NCH - 2] = ldg_nc_off<8 * ROWB + 128>(src);
+          ka[u][NCH - 1] = ldg_nc_off<192>(src);   kb[u][NCH - 1] = ldg_nc_off<8 * ROWB + 192>(src);
+        }
+      } else {
 #pragma unroll
-      for (int c = 0; c < NCH; ++c) {
-        ka[u][c] = phys[u] >= 0 ? ldg_nc(src + gid * ROWB + c * 64 + tig * 16) : make_uint4(0, 0, 0, 0);
-        kb[u][c] = phys[u] >= 0 ? ldg_nc(src + (gid + 8) * ROWB + c * 64 + tig * 16) : make_uint4(0, 0, 0, 0);
+        for (int c = 0; c < NCH; ++c) ka[u][c] = kb[u][c] = make_uint4(0, 0, 0, 0);
       }
     }
 #pragma unroll
