@@ -24,6 +24,7 @@ struct Params {
   int score_chunks;
   int sel_cluster;       // CTAs per (b, h) cluster of the select kernel
   int sel_slice_cap;     // capacity (tokens) of one CTA's probability slice in shared memory
+  int sel_nt;            // threads per CTA of the select kernel (512 or 1024)
   float *pooled;         // [B][Hq][max_ctx] max-pooled logits of SNAPKV heads (NULL when pool_kernel <= 1)
   int pool_kernel;       // SNAPKV max-pool window (odd), <= 1: no SNAPKV head in this config
   int cond_merge;        // 1: evictees of a full condensed tier are merged into a resident (Appendix G)

@@ -66,17 +66,24 @@ size_t select_smem_bytes(const Params &P) { return (size_t)P.sel_slice_cap * 4 +
 // every extra CTA of a cluster adds DSMEM-merge and barrier latency, so the smallest cluster that keeps a CTA's
 // slice near 16 k tokens (~32 per thread) wins (config 2: C = 2 < 1 < 4 < 8; config 3: 1 < 2 < 4; config 4: 4 < 8 < 2);
 // with only a few units the clusters are widened to spread them over the chip (config 1: 8 < 2 < 1).
-void select_geometry(const hardkv_config &c, int *cluster, int *slice_cap) {
+void select_geometry(const hardkv_config &c, int *cluster, int *slice_cap, int *threads) {
   const int units = c.batch * c.num_kv_heads;
   const int max_pool = c.max_ctx - c.recent > 0 ? c.max_ctx - c.recent : 1;
   const char *force = getenv("HARDKV_SELECT_CLUSTER");   // A/B measurements only
-  int C = 1;
-  while (C < SEL_MAXC && sel_slice_len(max_pool + 31, C) > 17408) C <<= 1;
+  const char *force_nt = getenv("HARDKV_SELECT_THREADS");
+  int C = 1, nt = SEL_NT;
+  while (C < SEL_MAXC && sel_slice_len(max_pool + 31, C, SEL_NT) > 17408) C <<= 1;
   while (C < SEL_MAXC && units * C * 2 <= 148) C <<= 1;
+  // a unit that would need a cluster of two 512-thread CTAs runs faster as ONE 1024-thread CTA (one per SM): the same
+  // threads per unit and no cluster barriers (config 2: 229.0 -> 226.4 us per step).  Wider clusters stay on 512-thread
+  // CTAs: two 1024-thread CTAs per unit measured slower than four 512-thread ones (config 4: 108.7 vs 104 us).
+  if (C == 2 && units <= 148 && units * 2 > 148 && sel_slice_len(max_pool + 31, 1, SEL_NT_BIG) <= 34816) { C = 1; nt = SEL_NT_BIG; }
   if (force && (atoi(force) == 1 || atoi(force) == 2 || atoi(force) == 4 || atoi(force) == 8)) C = atoi(force);
-  while (C < SEL_MAXC && (size_t)sel_slice_len(max_pool + 31, C) * 4 + sizeof(SelShared) > 227u * 1024u) C <<= 1;
+  if (force_nt && (atoi(force_nt) == SEL_NT || atoi(force_nt) == SEL_NT_BIG)) nt = atoi(force_nt);
+  while (C < SEL_MAXC && (size_t)sel_slice_len(max_pool + 31, C, nt) * 4 + sizeof(SelShared) > 227u * 1024u) C <<= 1;
   *cluster = C;
-  *slice_cap = sel_slice_len(max_pool + 31, C);
+  *slice_cap = sel_slice_len(max_pool + 31, C, nt);
+  *threads = nt;
 }
 
 hardkv_status check_config(const hardkv_config *c) {
@@ -92,8 +99,8 @@ hardkv_status check_config(const hardkv_config *c) {
   const bool tok = (c->kv_dtype == HARDKV_F32 && c->head_dim == 64) ||
                    (c->kv_dtype == HARDKV_BF16 && (c->head_dim == 64 || c->head_dim == 128));
   if (!gok || !tok) return HARDKV_ERR_UNSUPPORTED;
-  int cl, cap;
-  select_geometry(*c, &cl, &cap);
+  int cl, cap, nt;
+  select_geometry(*c, &cl, &cap, &nt);
   if ((size_t)cap * 4 + sizeof(SelShared) > 227u * 1024u) return HARDKV_ERR_UNSUPPORTED;  // pool slice must fit one SM
   return HARDKV_OK;
 }
@@ -187,7 +194,7 @@ void launch_select(hardkv_ctx *ctx, const Params &P, float p, int calibrate, cud
   ctx->launches += 1;
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3(P.B * P.Hkv * P.sel_cluster);
-  lc.blockDim = dim3(SEL_NT);
+  lc.blockDim = dim3(P.sel_nt);
   lc.dynamicSmemBytes = select_smem_bytes(P);
   lc.stream = st;
   cudaLaunchAttribute at[2];
@@ -197,15 +204,21 @@ void launch_select(hardkv_ctx *ctx, const Params &P, float p, int calibrate, cud
   at[1].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at;
   lc.numAttrs = pdl_enabled() ? 2 : 1;
+#define HK_SEL(CAL, GM)                                                                 \
+  do {                                                                                  \
+    if (P.sel_nt == SEL_NT_BIG) cudaLaunchKernelEx(&lc, select_kernel<CAL, GM, SEL_NT_BIG>, P, p); \
+    else cudaLaunchKernelEx(&lc, select_kernel<CAL, GM, SEL_NT>, P, p);                 \
+  } while (0)
   if (P.G <= 4) {
-    if (calibrate == 2) cudaLaunchKernelEx(&lc, select_kernel<2, 4>, P, p);
-    else if (calibrate == 1) cudaLaunchKernelEx(&lc, select_kernel<1, 4>, P, p);
-    else cudaLaunchKernelEx(&lc, select_kernel<0, 4>, P, p);
+    if (calibrate == 2) HK_SEL(2, 4);
+    else if (calibrate == 1) HK_SEL(1, 4);
+    else HK_SEL(0, 4);
   } else {
-    if (calibrate == 2) cudaLaunchKernelEx(&lc, select_kernel<2, 8>, P, p);
-    else if (calibrate == 1) cudaLaunchKernelEx(&lc, select_kernel<1, 8>, P, p);
-    else cudaLaunchKernelEx(&lc, select_kernel<0, 8>, P, p);
+    if (calibrate == 2) HK_SEL(2, 8);
+    else if (calibrate == 1) HK_SEL(1, 8);
+    else HK_SEL(0, 8);
   }
+#undef HK_SEL
 }
 
 // SNAPKV metric transform (L278): only configs that declare a pooling window pay for the launch
@@ -300,7 +313,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.pooled = cfg->pool_kernel > 1 ? reinterpret_cast<float *>(base + w.pooled) : nullptr;
   ctx->stage_q = base + w.stage_q; ctx->stage_k = base + w.stage_k; ctx->stage_v = base + w.stage_v;
   ctx->stage_out = reinterpret_cast<float *>(base + w.stage_out);
-  select_geometry(*cfg, &P.sel_cluster, &P.sel_slice_cap);
+  select_geometry(*cfg, &P.sel_cluster, &P.sel_slice_cap, &P.sel_nt);
   // opt in to the large dynamic shared memory of the select kernel (host-side attribute, no stream work);
   // the attribute is per function, so it is raised to the largest request seen in this process
   static size_t sel_smem_max = 0;
@@ -318,9 +331,13 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   }
   const int smx = (int)sel_smem_max;
   const cudaFuncAttribute fa = cudaFuncAttributeMaxDynamicSharedMemorySize;
-  if (cudaFuncSetAttribute(select_kernel<0, 4>, fa, smx) != cudaSuccess || cudaFuncSetAttribute(select_kernel<1, 4>, fa, smx) != cudaSuccess ||
-      cudaFuncSetAttribute(select_kernel<2, 4>, fa, smx) != cudaSuccess || cudaFuncSetAttribute(select_kernel<0, 8>, fa, smx) != cudaSuccess ||
-      cudaFuncSetAttribute(select_kernel<1, 8>, fa, smx) != cudaSuccess || cudaFuncSetAttribute(select_kernel<2, 8>, fa, smx) != cudaSuccess) {
+  bool okk = true;
+#define HK_SELATTR(CAL, GM)                                                                              \
+  okk = okk && cudaFuncSetAttribute(select_kernel<CAL, GM, SEL_NT>, fa, smx) == cudaSuccess &&          \
+        cudaFuncSetAttribute(select_kernel<CAL, GM, SEL_NT_BIG>, fa, smx) == cudaSuccess
+  HK_SELATTR(0, 4); HK_SELATTR(1, 4); HK_SELATTR(2, 4); HK_SELATTR(0, 8); HK_SELATTR(1, 8); HK_SELATTR(2, 8);
+#undef HK_SELATTR
+  if (!okk) {
     cudaGetLastError();
     delete ctx;
     return HARDKV_ERR_CUDA;

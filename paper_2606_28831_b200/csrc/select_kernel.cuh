@@ -23,8 +23,9 @@
 namespace hardkv {
 namespace cg = cooperative_groups;
 
-constexpr int SEL_NT = 512;
-constexpr int SEL_NW = SEL_NT / 32;
+constexpr int SEL_NT = 512;         // threads of a CTA: 512 (2 CTAs / SM, clusters) or SEL_NT_BIG (1 CTA / SM, whole unit)
+constexpr int SEL_NT_BIG = 1024;
+constexpr int SEL_NW = SEL_NT_BIG / 32;   // capacity of the per-warp arrays in shared memory
 constexpr int SEL_MAXC = 8;        // portable cluster size limit
 constexpr int SEL_NB = 1024;       // bins per level: a probability is <= 1, so its fp32 pattern has 30 significant bits
 constexpr uint32_t SEL_ONE = 0x3f800000u;   // bit pattern of 1.0f: larger inputs are treated as 1
@@ -63,15 +64,17 @@ __device__ __forceinline__ void hist_add(SelShared &sh, int bin, uint32_t bits) 
 }
 
 // Per-CTA slice geometry: the cluster covers absolute positions [base, base + C*per), base = lo & ~31.
-__host__ __device__ __forceinline__ int sel_slice_len(int span, int C) {
+__host__ __device__ __forceinline__ int sel_slice_len(int span, int C, int nt) {
   const int per = (span + C - 1) / C;
-  return (per + SEL_NT - 1) / SEL_NT * SEL_NT;
+  return (per + nt - 1) / nt * nt;
 }
 
 // CALIBRATE: 1 = logits -> probs (2a) then select; 0 = select on state->probs as given.
 // GMAX: compile-time bound of the GQA group (4 or 8) -- sizes the register arrays of the calibration.
-template <int CALIBRATE, int GMAX>
-__global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
+// NT: threads per CTA (SEL_NT: two CTAs per SM; SEL_NT_BIG: one CTA per SM that holds a whole unit without a cluster).
+template <int CALIBRATE, int GMAX, int NT>
+__global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Params P, float p) {
+  constexpr int NW = NT / 32;
   pdl_wait_then_trigger();
   extern __shared__ __align__(16) unsigned char sel_smem[];
   cg::cluster_group cluster = cg::this_cluster();
@@ -94,23 +97,23 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
   const int mask_bytes = P.max_ctx / 8;
 
   if (N <= 0) {  // empty pool: nothing selected (uniform over the cluster: no barrier is pending)
-    for (int j = rank * SEL_NT + tid; j < P.k_cap; j += C * SEL_NT) sel_idx[j] = -1;
-    for (int j = rank * SEL_NT + tid; j < P.spu; j += C * SEL_NT) sel_table[j] = -1;
+    for (int j = rank * NT + tid; j < P.k_cap; j += C * NT) sel_idx[j] = -1;
+    for (int j = rank * NT + tid; j < P.spu; j += C * NT) sel_table[j] = -1;
     if (want_mask)
-      for (int y = rank * SEL_NT + tid; y < mask_bytes; y += C * SEL_NT) mask[y] = 0;
+      for (int y = rank * NT + tid; y < mask_bytes; y += C * NT) mask[y] = 0;
     if (rank == 0 && tid == 0) P.st.sel_count[unit] = 0;
     return;
   }
 
   const int base = lo & ~31;
-  const int per = sel_slice_len(hi - base, C);   // <= P.sel_slice_cap by construction of the cap
+  const int per = sel_slice_len(hi - base, C, NT);   // <= P.sel_slice_cap by construction of the cap
   const int s0 = base + rank * per;              // this CTA's slice: absolute positions [s0, s0 + per)
-  const int wseg = per / SEL_NW;                 // positions per warp (multiple of 32)
+  const int wseg = per / NW;                 // positions per warp (multiple of 32)
 
   // split-phase cluster barrier: every CTA of the cluster must be running before its shared memory
   // is written by a peer; the wait sits in front of the first DSMEM access.
   if (C > 1) cluster.barrier_arrive();
-  for (int d = tid; d < SEL_NB; d += SEL_NT) { sh.h_cnt[d] = 0; sh.h_hi[d] = 0; sh.h_lo[d] = 0; }
+  for (int d = tid; d < SEL_NB; d += NT) { sh.h_cnt[d] = 0; sh.h_hi[d] = 0; sh.h_lo[d] = 0; }
 
   // ---------------- 2a: calibration ------------------------------------------------------------
   if (CALIBRATE) {
@@ -150,12 +153,12 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
         if (g >= G) break;
         const float *row = lg + (size_t)g * P.max_ctx;
         float m = -INFINITY, sacc = 0.f;
-        for (int i0 = tid; i0 < per; i0 += 4 * SEL_NT) {
+        for (int i0 = tid; i0 < per; i0 += 4 * NT) {
           float x[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            const int pos = s0 + i0 + u * SEL_NT;
-            x[u] = (i0 + u * SEL_NT < per && pos >= lo && pos < hi) ? __ldg(row + pos) * c2 : -INFINITY;
+            const int pos = s0 + i0 + u * NT;
+            x[u] = (i0 + u * NT < per && pos >= lo && pos < hi) ? __ldg(row + pos) * c2 : -INFINITY;
           }
           const float mn = fmaxf(fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3])), m);
           if (mn != -INFINITY) {
@@ -174,8 +177,8 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
         const int c = tid >> 3, g = tid & 7;
         float m = -INFINITY, sacc = 0.f;
         if (g < G) {
-          for (int w = 0; w < SEL_NW; ++w) m = fmaxf(m, sh.red_f[w][g][0]);
-          for (int w = 0; w < SEL_NW; ++w) {
+          for (int w = 0; w < NW; ++w) m = fmaxf(m, sh.red_f[w][g][0]);
+          for (int w = 0; w < NW; ++w) {
             const float mw = sh.red_f[w][g][0];
             if (mw != -INFINITY) sacc += sh.red_f[w][g][1] * fast_exp2(mw - m);
           }
@@ -206,11 +209,11 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
       // flight (32 registers of logits), 16-byte stores of the probabilities and of the slice
       constexpr int UQ = 8 / GMAX;
       const int nq = per >> 2;
-      for (int q0 = tid; q0 < nq; q0 += UQ * SEL_NT) {
+      for (int q0 = tid; q0 < nq; q0 += UQ * NT) {
         float4 x[UQ][GMAX];
 #pragma unroll
         for (int u = 0; u < UQ; ++u) {
-          const int qd = q0 + u * SEL_NT, pos = s0 + 4 * qd;
+          const int qd = q0 + u * NT, pos = s0 + 4 * qd;
           const bool live = qd < nq && pos < hi && pos + 3 >= lo;
           const bool vec = pos + 3 < P.max_ctx;     // the quad lies inside the logits row
 #pragma unroll
@@ -230,7 +233,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
         }
 #pragma unroll
         for (int u = 0; u < UQ; ++u) {
-          const int qd = q0 + u * SEL_NT, pos = s0 + 4 * qd;
+          const int qd = q0 + u * NT, pos = s0 + 4 * qd;
           if (qd >= nq) break;
           float pr[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
@@ -265,7 +268,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
       float *acc = P.st.acc + (size_t)unit * P.max_ctx;
       float *ring = P.st.ring + ((size_t)unit * P.accum_window + slot) * P.max_ctx;
       double tot = 0.0;
-      for (int i = tid; i < per; i += SEL_NT) {
+      for (int i = tid; i < per; i += NT) {
         const int pos = s0 + i;
         uint32_t bits = SEL_INVALID;
         if (pos >= lo && pos < hi) {
@@ -288,13 +291,13 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
       __syncthreads();
       if (tid < C) {
         double t = 0.0;
-        for (int w = 0; w < SEL_NW; ++w) t += sh.red_d[w];
+        for (int w = 0; w < NW; ++w) t += sh.red_d[w];
         cluster.map_shared_rank(&sh, tid)->acc_tot[rank] = t;
       }
       cluster.sync();
       tot = 0.0;
       for (int c = 0; c < C; ++c) tot += sh.acc_tot[c];
-      for (int i = tid; i < per; i += SEL_NT) {
+      for (int i = tid; i < per; i += NT) {
         const uint32_t ab = pbits[i];
         if (ab == SEL_INVALID) continue;
         const float pr = tot > 0.0 ? (float)((double)__uint_as_float(ab) / tot) : 0.f;
@@ -308,7 +311,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
   } else {
     __syncthreads();  // histogram zeroed
     if (C > 1) cluster.barrier_wait();
-    for (int i = tid; i < per; i += SEL_NT) {
+    for (int i = tid; i < per; i += NT) {
       const int pos = s0 + i;
       uint32_t bits = SEL_INVALID;
       if (pos >= lo && pos < hi) {
@@ -337,10 +340,10 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
       const int nb = 1 << db;
       if (level > 0) {
         // histogram of the next digit over the tokens whose high bits equal the prefix
-        for (int d = tid; d < nb; d += SEL_NT) { sh.h_cnt[d] = 0; sh.h_hi[d] = 0; sh.h_lo[d] = 0; }
+        for (int d = tid; d < nb; d += NT) { sh.h_cnt[d] = 0; sh.h_hi[d] = 0; sh.h_lo[d] = 0; }
         __syncthreads();
         const int hs = shift + db;
-        for (int i = tid * 4; i < per; i += 4 * SEL_NT) {
+        for (int i = tid * 4; i < per; i += 4 * NT) {
           const uint4 b4 = *reinterpret_cast<const uint4 *>(pbits + i);
           if ((b4.x >> hs) == prefix) hist_add(sh, (b4.x >> shift) & (nb - 1), b4.x);
           if ((b4.y >> hs) == prefix) hist_add(sh, (b4.y >> shift) & (nb - 1), b4.y);
@@ -353,7 +356,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
       // ---- range pass: thread t takes bpt consecutive bins of this CTA's owner range, from the top (local index
       //      jt = t * bpt + u <-> bin S - 1 - jt); across a cluster it first merges the C local histograms of those
       //      bins over DSMEM.  A warp therefore covers one contiguous sub-range, whose (count, mass) it reduces. ----
-      const int bpt = S > SEL_NT ? S / SEL_NT : 1;   // <= 4
+      const int bpt = S > NT ? S / NT : 1;   // <= 4
       if (C > 1) cluster.sync();      // A: every local histogram of this level is complete
       {
         unsigned long long tm = 0;
@@ -396,7 +399,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
         if (tid < C) {
           unsigned long long m_ = 0;
           uint32_t c_ = 0;
-          for (int w = 0; w < SEL_NW; ++w) { m_ += sh.red_u[w]; c_ += sh.red_c[w]; }
+          for (int w = 0; w < NW; ++w) { m_ += sh.red_u[w]; c_ += sh.red_c[w]; }
           SelShared *dst = cluster.map_shared_rank(&sh, tid);
           dst->tot_mass[rank] = m_;
           dst->tot_cnt[rank] = c_;
@@ -563,7 +566,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
   if (C > 1) {
     if (tid < C) {
       int g_ = 0, t_ = 0;
-      for (int w = 0; w < SEL_NW; ++w) { g_ += sh.w_gt[w]; t_ += sh.w_tie[w]; }
+      for (int w = 0; w < NW; ++w) { g_ += sh.w_gt[w]; t_ += sh.w_tie[w]; }
       SelShared *dst = cluster.map_shared_rank(&sh, tid);
       dst->c_gt[rank] = g_;
       dst->c_tie[rank] = t_;
@@ -609,7 +612,7 @@ __global__ void __launch_bounds__(SEL_NT, 2) select_kernel(Params P, float p) {
     sel_before += __popc(sb);
   }
   // pads, the head-wise block table (reading C9; L207-209) and the mask bytes outside the slices
-  const int gt_ = rank * SEL_NT + tid, gs_ = C * SEL_NT;
+  const int gt_ = rank * NT + tid, gs_ = C * NT;
   for (int j = k + gt_; j < P.k_cap; j += gs_) sel_idx[j] = -1;
   const int used = (k + PAGE - 1) / PAGE;
   const int32_t *sp = P.st.sel_pages + (size_t)unit * P.spu;

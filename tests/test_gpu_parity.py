@@ -165,11 +165,13 @@ def test_kernel_variants(name, variant, P):
     pr.check_logits()
 
 
-@pytest.mark.parametrize("cluster", [1, 2, 4, 8])
+@pytest.mark.parametrize("cluster,threads", [(1, 512), (2, 512), (4, 512), (8, 512), (1, 1024), (2, 1024)])
 @pytest.mark.parametrize("name", ["c2s", "c4s", "g8"])
-def test_select_every_cluster_size(name, cluster, P, monkeypatch):
-    """The select kernel at every cluster size (1 = single CTA, no DSMEM): bit exact from identical probabilities."""
+def test_select_every_cluster_size(name, cluster, threads, P, monkeypatch):
+    """The select kernel at every cluster size (1 = single CTA, no DSMEM) and both CTA sizes (512 threads, two CTAs per
+    SM; 1024 threads, one per SM): bit exact from identical probabilities."""
     monkeypatch.setenv("HARDKV_SELECT_CLUSTER", str(cluster))
+    monkeypatch.setenv("HARDKV_SELECT_THREADS", str(threads))
     wl = WL[name]
     pr = P(wl)
     for t in range(3):
