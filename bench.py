@@ -32,7 +32,7 @@ UNIT = "GB/s"
 NOMINAL_HBM_GBS = 8000.0                 # the contract's "8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                # B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1_03_final.md), config 2
-NCU_TRAFFIC_BYTES = {2: {"score": 585.7e6, "rewrite_attend": 279.6e6, "calibrate_topp": 41.6e6}}
+NCU_TRAFFIC_BYTES = {2: {"score": 586.4e6, "rewrite_attend": 279.6e6, "calibrate_topp": 41.6e6}}
 
 
 def log(*a):
