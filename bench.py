@@ -104,7 +104,7 @@ def oracle_leg(cfg_index: int, steps: int, warmup: int, budget_s: float, sample_
     from oracle import oracle as ora
     from oracle.batch import OracleBatch
     from paper_2606_28831_b200 import accounting
-    from paper_2606_28831_b200.synth import make_workload
+    from workloads.synth import make_workload
     ora.build()
     wl = make_workload(cfg_index, B=sample_B) if cfg_index in (2, 3, 4) else make_workload(cfg_index)
     prefill = {(b, h): wl.prefill_unit(b, h) for b in range(wl.B) for h in range(wl.Hkv)}

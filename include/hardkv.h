@@ -102,6 +102,13 @@ const char   *hardkv_status_string(hardkv_status s);
 /* Kernel variant switch for A/B measurements: 0 = generic FMA kernels, 1 = tuned paths (default),
  * 2 = tuned paths with the TMA-staged (cp.async.bulk + mbarrier ring) persistent score kernel. */
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant);
+/* Geometry of the select kernel, for A/B measurements and tests: cluster = CTAs per (b, h) in {1, 2, 4, 8}, threads per
+ * CTA in {512, 1024}; 0 keeps the automatic choice for that argument.  HARDKV_ERR_UNSUPPORTED when a CTA's slice of the
+ * pool would not fit one SM's shared memory.  Host-side only; call it before capturing a graph with this ctx. */
+hardkv_status hardkv_set_select_geometry(hardkv_ctx *ctx, int32_t cluster, int32_t threads);
+/* 1: launch the hot kernels with the programmatic-dependent-launch attribute (each kernel waits for its predecessor at
+ * its top, so ordering is that of a plain stream launch).  Default 0: measured slower inside a captured graph. */
+hardkv_status hardkv_set_pdl(hardkv_ctx *ctx, int32_t on);
 
 /* Step 1 + Step 4 of L78.  Writes (k_new, v_new) [B][Hkv][d] at position ctx_len[b];
  * ctx_len += 1; while the pool exceeds l_upper[b] its oldest token retires into the

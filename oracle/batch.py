@@ -7,7 +7,7 @@ from __future__ import annotations
 import numpy as np
 
 from oracle.oracle import OracleConfig, Unit, decode_step_batch
-from paper_2606_28831_b200.synth import Workload
+from workloads.synth import Workload
 
 
 class OracleBatch:

@@ -117,6 +117,12 @@ int hko_retire_q(const hko_config *c, hko_unit *u, const float *q) {
     retired += 1;
   }
   free(ek); free(ev);
+  /* a compression step re-anchors the dense tier at sinks + the last W tokens (L71, L276-277) */
+  {
+    int32_t s_end = c->sink < u->n ? c->sink : u->n;
+    int32_t r_lo = u->n - c->recent;
+    u->dense_lo = r_lo > s_end ? r_lo : s_end;
+  }
   return retired;
 }
 
@@ -401,12 +407,13 @@ void hko_merge(int32_t d, double *o_a, double *m_a, double *l_a,
 
 /* ---- attention over D u I u C (L84: "exact full-sequence attention from the
  * partial attention outputs of three tiers").  D = sinks [0,min(s,n)) and recent
- * [max(s,n-W), n) read from the base rows; I = the rewritten selected tier;
+ * [dense_lo, n) read from the base rows (dense_lo = max(s, n-W) at the last compression step); I = the rewritten selected tier;
  * C = condensed residents.  The calibration temperature is NOT applied here. */
 void hko_attend(const hko_config *c, hko_unit *u, const float *q) {
   int32_t d = c->d;
   int32_t s_end = c->sink < u->n ? c->sink : u->n;
-  int32_t r_lo = u->n - c->recent; if (r_lo < s_end) r_lo = s_end;
+  int32_t r_lo = u->dense_lo; if (r_lo < s_end) r_lo = s_end;   /* [dense_lo, n): W tokens at a compression step,
+                                                                    growing by one per step until the next (L78) */
   int32_t n_dense = s_end + (u->n - r_lo);
   int32_t *didx = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_dense > 0 ? n_dense : 1));
   int32_t t = 0;
@@ -431,13 +438,13 @@ void hko_attend(const hko_config *c, hko_unit *u, const float *q) {
 /* ---- one decode step in the order of L78 (Step 1 append; Step 4 compaction of the
  * oldest "before new dense blocks are allocated"; Step 2 calibrated Top-p; Step 3
  * rewrite) followed by the tiered attention of L84.  do_select = 0 reproduces the
- * steps between two compressions (L274 "every 128 steps"): the previous selected
- * tier is reused. */
+ * steps between two compressions (L274 "every 128 steps"): only Step 1 runs, the dense
+ * tier grows (L78 steps 1-2), the previous selected tier and condensed tier are reused. */
 void hko_decode_step(const hko_config *c, hko_unit *u, const float *q,
                      const float *k_new, const float *v_new, float p, int do_select) {
   hko_append(c, u, k_new, v_new);
-  hko_retire_q(c, u, q);
   if (do_select) {
+    hko_retire_q(c, u, q);      /* Step 4 belongs to the compression step; it also re-anchors dense_lo */
     hko_score(c, u, q);
     hko_calibrate(c, u);
     hko_topp_select(c, u, p, 1);

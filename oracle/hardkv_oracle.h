@@ -59,6 +59,9 @@ typedef struct {
   float   *K, *V;              /* [max_ctx][d]  base KV rows, inputs widened exactly */
   int32_t  n;                  /* current context length                            */
   int32_t  c_lo;               /* first pool position                               */
+  int32_t  dense_lo;           /* first position of the recent part of the dense tier: n - W at the last
+                                  compression step; the dense tier grows from there until the next one (L78
+                                  steps 1-2: "append ... to the Tier 1 Dense Cache" until the threshold)      */
   int32_t  l_lower, l_upper;   /* thresholds (reading C8)                           */
   int32_t *votes;              /* [max_ctx] Cautious-Update votes (L86)             */
   float   *cond_k, *cond_v;    /* [cond_cap][d] condensed tier rows                 */
@@ -101,7 +104,11 @@ void hko_topp_select(const hko_config *c, hko_unit *u, float p, int count_votes)
 void hko_rewrite(const hko_config *c, hko_unit *u);
 /* Eq. 4-6 (L735-762): three tier states merged with the operator of Eq. 6. */
 void hko_attend(const hko_config *c, hko_unit *u, const float *q);
-/* One whole decode step in the order of L78 (append, retire, select, rewrite, attend). */
+/* One whole decode step in the order of L78 (append, retire, select, rewrite, attend).
+ * do_select = 0 is a step BETWEEN two compressions (L274): only Step 1 runs -- the new token joins the dense tier,
+ * which keeps growing from dense_lo (L78 steps 1-2); nothing retires, nothing is re-selected, and attention covers
+ * sinks + [dense_lo, n) + the tier selected at the last compression + the condensed tier: every live token exactly
+ * once.  Retirement of the tokens that aged meanwhile happens at the next compression step. */
 void hko_decode_step(const hko_config *c, hko_unit *u, const float *q,
                      const float *k_new, const float *v_new, float p, int do_select);
 /* The same over many units; q is [n_units][G][d], k_new/v_new [n_units][d].

@@ -45,7 +45,7 @@ _I = C.POINTER(C.c_int32)
 class HkoUnit(C.Structure):
     _fields_ = [
         ("K", _F), ("V", _F),
-        ("n", C.c_int32), ("c_lo", C.c_int32), ("l_lower", C.c_int32), ("l_upper", C.c_int32),
+        ("n", C.c_int32), ("c_lo", C.c_int32), ("dense_lo", C.c_int32), ("l_lower", C.c_int32), ("l_upper", C.c_int32),
         ("votes", _I),
         ("cond_k", _F), ("cond_v", _F), ("cond_pos", _I), ("cond_votes", _I), ("cond_count", C.c_int32),
         ("score_mode", C.c_int32), ("T", C.c_float),
@@ -154,6 +154,7 @@ class Unit:
         u = self.u
         u.K, u.V = _fp(self.K), _fp(self.V)
         u.n, u.c_lo, u.l_lower, u.l_upper = n0, cfg.sink, l_lower, l_upper
+        u.dense_lo = max(min(cfg.sink, n0), n0 - cfg.recent)
         u.votes = _ip(self.votes)
         u.cond_k, u.cond_v = _fp(self.cond_k), _fp(self.cond_v)
         u.cond_pos, u.cond_votes, u.cond_count = _ip(self.cond_pos), _ip(self.cond_votes), 0
@@ -168,6 +169,7 @@ class Unit:
     # --- scalars -------------------------------------------------------------------
     n = property(lambda s: s.u.n)
     c_lo = property(lambda s: s.u.c_lo)
+    dense_lo = property(lambda s: s.u.dense_lo)
     sel_count = property(lambda s: s.u.sel_count)
     k_topp = property(lambda s: s.u.k_topp)
     cond_count = property(lambda s: s.u.cond_count)
@@ -241,7 +243,7 @@ def decode_step_batch(units: list[Unit], q: np.ndarray, k_new: np.ndarray, v_new
     nt = lib().hko_decode_step_batch(C.byref(units[0].ccfg), arr, len(units), _fp(q), _fp(k_new), _fp(v_new),
                                      np.float32(p), int(do_select))
     for u, cu in zip(units, arr):   # copy the scalar fields back (arrays are shared by pointer)
-        for f in ("n", "c_lo", "cond_count", "ring_slot", "sel_count", "k_topp", "tau_bits"):
+        for f in ("n", "c_lo", "dense_lo", "cond_count", "ring_slot", "sel_count", "k_topp", "tau_bits"):
             setattr(u.u, f, getattr(cu, f))
     return nt
 

@@ -2,6 +2,5 @@
 
 `paper_2606_28831_b200.hardkv` is the thin ctypes binding over libhardkv.so (C ABI in
 include/hardkv.h); importing it fails loudly if the CUDA library has not been built.
-`paper_2606_28831_b200.synth` holds the seeded synthetic workloads (numpy only).
+The seeded synthetic workloads live outside the package, in `workloads.synth` (numpy only).
 """
-__all__ = ["synth"]

@@ -19,6 +19,7 @@ struct hardkv_ctx {
   hardkv_config cfg;
   Params base;      // config-derived fields + workspace pointers; `st` is filled per call
   int variant;
+  int pdl;                       // 1: launches carry the programmatic-stream-serialization attribute (hardkv_set_pdl)
   int num_sms;
   size_t ws_bytes;
   int64_t launches;              // kernels launched through this ctx (hardkv_launch_count)
@@ -66,11 +67,11 @@ size_t select_smem_bytes(const Params &P) { return (size_t)P.sel_slice_cap * 4 +
 // every extra CTA of a cluster adds DSMEM-merge and barrier latency, so the smallest cluster that keeps a CTA's
 // slice near 16 k tokens (~32 per thread) wins (config 2: C = 2 < 1 < 4 < 8; config 3: 1 < 2 < 4; config 4: 4 < 8 < 2);
 // with only a few units the clusters are widened to spread them over the chip (config 1: 8 < 2 < 1).
-void select_geometry(const hardkv_config &c, int *cluster, int *slice_cap, int *threads) {
+// force_c / force_nt (0 = automatic) come from hardkv_set_select_geometry: A/B measurements and the tests that run
+// the kernel at every cluster size.
+void select_geometry(const hardkv_config &c, int force_c, int force_nt, int *cluster, int *slice_cap, int *threads) {
   const int units = c.batch * c.num_kv_heads;
   const int max_pool = c.max_ctx - c.recent > 0 ? c.max_ctx - c.recent : 1;
-  const char *force = getenv("HARDKV_SELECT_CLUSTER");   // A/B measurements only
-  const char *force_nt = getenv("HARDKV_SELECT_THREADS");
   int C = 1, nt = SEL_NT;
   while (C < SEL_MAXC && sel_slice_len(max_pool + 31, C, SEL_NT) > 17408) C <<= 1;
   while (C < SEL_MAXC && units * C * 2 <= 148) C <<= 1;
@@ -78,12 +79,28 @@ void select_geometry(const hardkv_config &c, int *cluster, int *slice_cap, int *
   // threads per unit and no cluster barriers (config 2: 229.0 -> 226.4 us per step).  Wider clusters stay on 512-thread
   // CTAs: two 1024-thread CTAs per unit measured slower than four 512-thread ones (config 4: 108.7 vs 104 us).
   if (C == 2 && units <= 148 && units * 2 > 148 && sel_slice_len(max_pool + 31, 1, SEL_NT_BIG) <= 34816) { C = 1; nt = SEL_NT_BIG; }
-  if (force && (atoi(force) == 1 || atoi(force) == 2 || atoi(force) == 4 || atoi(force) == 8)) C = atoi(force);
-  if (force_nt && (atoi(force_nt) == SEL_NT || atoi(force_nt) == SEL_NT_BIG)) nt = atoi(force_nt);
+  if (force_c == 1 || force_c == 2 || force_c == 4 || force_c == 8) C = force_c;
+  if (force_nt == SEL_NT || force_nt == SEL_NT_BIG) nt = force_nt;
   while (C < SEL_MAXC && (size_t)sel_slice_len(max_pool + 31, C, nt) * 4 + sizeof(SelShared) > 227u * 1024u) C <<= 1;
   *cluster = C;
   *slice_cap = sel_slice_len(max_pool + 31, C, nt);
   *threads = nt;
+}
+
+// Opt in to the large dynamic shared memory of the select kernel (host-side attribute, no stream work); the attribute
+// is per function, so it is raised to the largest request seen in this process.
+bool raise_select_smem(const Params &P) {
+  static size_t sel_smem_max = 0;
+  if (select_smem_bytes(P) > sel_smem_max) sel_smem_max = select_smem_bytes(P);
+  const int smx = (int)sel_smem_max;
+  const cudaFuncAttribute fa = cudaFuncAttributeMaxDynamicSharedMemorySize;
+  bool okk = true;
+#define HK_SELATTR(CAL, GM)                                                                              \
+  okk = okk && cudaFuncSetAttribute(select_kernel<CAL, GM, SEL_NT>, fa, smx) == cudaSuccess &&          \
+        cudaFuncSetAttribute(select_kernel<CAL, GM, SEL_NT_BIG>, fa, smx) == cudaSuccess
+  HK_SELATTR(0, 4); HK_SELATTR(1, 4); HK_SELATTR(2, 4); HK_SELATTR(0, 8); HK_SELATTR(1, 8); HK_SELATTR(2, 8);
+#undef HK_SELATTR
+  return okk;
 }
 
 hardkv_status check_config(const hardkv_config *c) {
@@ -100,7 +117,7 @@ hardkv_status check_config(const hardkv_config *c) {
                    (c->kv_dtype == HARDKV_BF16 && (c->head_dim == 64 || c->head_dim == 128));
   if (!gok || !tok) return HARDKV_ERR_UNSUPPORTED;
   int cl, cap, nt;
-  select_geometry(*c, &cl, &cap, &nt);
+  select_geometry(*c, 0, 0, &cl, &cap, &nt);
   if ((size_t)cap * 4 + sizeof(SelShared) > 227u * 1024u) return HARDKV_ERR_UNSUPPORTED;  // pool slice must fit one SM
   return HARDKV_OK;
 }
@@ -143,22 +160,19 @@ Params params_of(const hardkv_ctx *ctx, const hardkv_state *s) {
 
 // Launch with the programmatic-stream-serialization attribute (PDL, see pdl_wait_then_trigger in common.cuh); the
 // kernels wait for their predecessor at the top, so ordering and visibility are those of a plain stream launch.
-// Off by default (HARDKV_PDL=1 turns it on): measured on B200 it shortens eager launch loops (config 2 amortised
+// Off by default (hardkv_set_pdl turns it on): measured on B200 it shortens eager launch loops (config 2 amortised
 // regime 59.3 -> 56.1 us, host entry 295.7 -> 293.7 us) but lengthens the captured graph of the headline step
 // (234.5 -> 239.8 us): the graph already has no launch gap, and early-resident successors take SM slots from the tail.
-bool pdl_enabled() {
-  static const bool on = [] { const char *e = getenv("HARDKV_PDL"); return e && atoi(e) == 1; }();   // A/B switch
-  return on;
-}
 template <typename... KArgs, typename... Args>
-void launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+void launch_pdl(const hardkv_ctx *ctx, void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st,
+                Args... args) {
   cudaLaunchConfig_t lc = {};
   lc.gridDim = grid; lc.blockDim = block; lc.dynamicSmemBytes = smem; lc.stream = st;
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at;
-  lc.numAttrs = pdl_enabled() ? 1 : 0;
+  lc.numAttrs = ctx->pdl ? 1 : 0;
   cudaLaunchKernelEx(&lc, kernel, KArgs(args)...);
 }
 
@@ -168,7 +182,7 @@ bool fast_path(const hardkv_ctx *ctx) { return ctx->variant >= 1 && ctx->cfg.kv_
 void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, const void *q,
                    cudaStream_t st) {
   ctx->launches += 1;
-  HK_DISPATCH_TD(ctx->cfg, (launch_pdl(append_retire_kernel<T, D>, dim3(P.B), dim3(256), 0, st, P, k_new, v_new, q)));
+  HK_DISPATCH_TD(ctx->cfg, (launch_pdl(ctx, append_retire_kernel<T, D>, dim3(P.B), dim3(256), 0, st, P, k_new, v_new, q)));
 }
 
 void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
@@ -181,8 +195,8 @@ void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t 
     return;
   }
   if (fast_path(ctx)) {
-    if (P.d == 128) launch_pdl(score_mma_kernel<128>, grid, dim3(256), 0, st, P, q);
-    else launch_pdl(score_mma_kernel<64>, grid, dim3(256), 0, st, P, q);
+    if (P.d == 128) launch_pdl(ctx, score_mma_kernel<128>, grid, dim3(256), 0, st, P, q);
+    else launch_pdl(ctx, score_mma_kernel<64>, grid, dim3(256), 0, st, P, q);
     return;
   }
   HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (score_generic_kernel<T, D, G><<<grid, 256, 0, st>>>(P, q))));
@@ -203,7 +217,7 @@ void launch_select(hardkv_ctx *ctx, const Params &P, float p, int calibrate, cud
   at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[1].val.programmaticStreamSerializationAllowed = 1;
   lc.attrs = at;
-  lc.numAttrs = pdl_enabled() ? 2 : 1;
+  lc.numAttrs = ctx->pdl ? 2 : 1;
 #define HK_SEL(CAL, GM)                                                                 \
   do {                                                                                  \
     if (P.sel_nt == SEL_NT_BIG) cudaLaunchKernelEx(&lc, select_kernel<CAL, GM, SEL_NT_BIG>, P, p); \
@@ -241,13 +255,13 @@ void launch_attend(hardkv_ctx *ctx, const Params &P, const void *q, float *out, 
   if (fast_path(ctx)) {
     dim3 gm((P.att_chunks * ATT_CHUNK + ATT_MMA_CHUNK - 1) / ATT_MMA_CHUNK, P.B * P.Hkv);
     if (P.d == 128) {
-      if (mode == ATT_REWRITE) launch_pdl(attend_mma_kernel<128, ATT_REWRITE>, gm, dim3(256), 0, st, P, q, out, lse);
-      else if (mode == ATT_SPARSE) launch_pdl(attend_mma_kernel<128, ATT_SPARSE>, gm, dim3(256), 0, st, P, q, out, lse);
-      else launch_pdl(attend_mma_kernel<128, ATT_TIER>, gm, dim3(256), 0, st, P, q, out, lse);
+      if (mode == ATT_REWRITE) launch_pdl(ctx, attend_mma_kernel<128, ATT_REWRITE>, gm, dim3(256), 0, st, P, q, out, lse);
+      else if (mode == ATT_SPARSE) launch_pdl(ctx, attend_mma_kernel<128, ATT_SPARSE>, gm, dim3(256), 0, st, P, q, out, lse);
+      else launch_pdl(ctx, attend_mma_kernel<128, ATT_TIER>, gm, dim3(256), 0, st, P, q, out, lse);
     } else {
-      if (mode == ATT_REWRITE) launch_pdl(attend_mma_kernel<64, ATT_REWRITE>, gm, dim3(256), 0, st, P, q, out, lse);
-      else if (mode == ATT_SPARSE) launch_pdl(attend_mma_kernel<64, ATT_SPARSE>, gm, dim3(256), 0, st, P, q, out, lse);
-      else launch_pdl(attend_mma_kernel<64, ATT_TIER>, gm, dim3(256), 0, st, P, q, out, lse);
+      if (mode == ATT_REWRITE) launch_pdl(ctx, attend_mma_kernel<64, ATT_REWRITE>, gm, dim3(256), 0, st, P, q, out, lse);
+      else if (mode == ATT_SPARSE) launch_pdl(ctx, attend_mma_kernel<64, ATT_SPARSE>, gm, dim3(256), 0, st, P, q, out, lse);
+      else launch_pdl(ctx, attend_mma_kernel<64, ATT_TIER>, gm, dim3(256), 0, st, P, q, out, lse);
     }
     return;
   }
@@ -313,11 +327,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.pooled = cfg->pool_kernel > 1 ? reinterpret_cast<float *>(base + w.pooled) : nullptr;
   ctx->stage_q = base + w.stage_q; ctx->stage_k = base + w.stage_k; ctx->stage_v = base + w.stage_v;
   ctx->stage_out = reinterpret_cast<float *>(base + w.stage_out);
-  select_geometry(*cfg, &P.sel_cluster, &P.sel_slice_cap, &P.sel_nt);
-  // opt in to the large dynamic shared memory of the select kernel (host-side attribute, no stream work);
-  // the attribute is per function, so it is raised to the largest request seen in this process
-  static size_t sel_smem_max = 0;
-  if (select_smem_bytes(P) > sel_smem_max) sel_smem_max = select_smem_bytes(P);
+  select_geometry(*cfg, 0, 0, &P.sel_cluster, &P.sel_slice_cap, &P.sel_nt);
   int dev = 0, nsm = 148;
   cudaGetDevice(&dev);
   if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
@@ -329,15 +339,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
     cudaFuncSetAttribute(score_tma_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
     cudaFuncSetAttribute(score_tma_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
   }
-  const int smx = (int)sel_smem_max;
-  const cudaFuncAttribute fa = cudaFuncAttributeMaxDynamicSharedMemorySize;
-  bool okk = true;
-#define HK_SELATTR(CAL, GM)                                                                              \
-  okk = okk && cudaFuncSetAttribute(select_kernel<CAL, GM, SEL_NT>, fa, smx) == cudaSuccess &&          \
-        cudaFuncSetAttribute(select_kernel<CAL, GM, SEL_NT_BIG>, fa, smx) == cudaSuccess
-  HK_SELATTR(0, 4); HK_SELATTR(1, 4); HK_SELATTR(2, 4); HK_SELATTR(0, 8); HK_SELATTR(1, 8); HK_SELATTR(2, 8);
-#undef HK_SELATTR
-  if (!okk) {
+  if (!raise_select_smem(P)) {
     cudaGetLastError();
     delete ctx;
     return HARDKV_ERR_CUDA;
@@ -351,6 +353,23 @@ void hardkv_destroy(hardkv_ctx *ctx) { delete ctx; }
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant) {
   if (!ctx || variant < 0 || variant > 2) return HARDKV_ERR_INVALID_ARG;
   ctx->variant = variant;
+  return HARDKV_OK;
+}
+
+hardkv_status hardkv_set_select_geometry(hardkv_ctx *ctx, int32_t cluster, int32_t threads) {
+  if (!ctx) return HARDKV_ERR_INVALID_ARG;
+  if (cluster != 0 && cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8) return HARDKV_ERR_INVALID_ARG;
+  if (threads != 0 && threads != SEL_NT && threads != SEL_NT_BIG) return HARDKV_ERR_INVALID_ARG;
+  int cl, cap, nt;
+  select_geometry(ctx->cfg, cluster, threads, &cl, &cap, &nt);
+  if ((size_t)cap * 4 + sizeof(SelShared) > 227u * 1024u) return HARDKV_ERR_UNSUPPORTED;
+  ctx->base.sel_cluster = cl; ctx->base.sel_slice_cap = cap; ctx->base.sel_nt = nt;
+  return raise_select_smem(ctx->base) ? HARDKV_OK : HARDKV_ERR_CUDA;
+}
+
+hardkv_status hardkv_set_pdl(hardkv_ctx *ctx, int32_t on) {
+  if (!ctx || (on != 0 && on != 1)) return HARDKV_ERR_INVALID_ARG;
+  ctx->pdl = on;
   return HARDKV_OK;
 }
 

@@ -16,7 +16,10 @@
 
 namespace hardkv {
 
-constexpr int SCORE_STAGES = 40;            // pages in flight per SM (multiple of 8): 160 KiB at d = 128
+#ifndef HARDKV_SCORE_STAGES
+#define HARDKV_SCORE_STAGES 40
+#endif
+constexpr int SCORE_STAGES = HARDKV_SCORE_STAGES;   // pages in flight per SM (multiple of 8): 160 KiB at d = 128
 constexpr int SCORE_CONSUMERS = 8;          // consumer warps
 constexpr int SCORE_PRODUCERS = 4;          // producer warps (one issuing lane each): a copy costs ~150 issue cycles
 constexpr int SCORE_TMA_THREADS = (SCORE_CONSUMERS + SCORE_PRODUCERS) * 32;

@@ -55,7 +55,7 @@ class StateStruct(C.Structure):
 F32, BF16 = 0, 1
 STEP_REUSE_TIER, STEP_SELECT_REWRITE, STEP_SELECT_SPARSE, STEP_REUSE_SPARSE = 0, 1, 2, 3   # do_select of decode_step
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
-           "hardkv_set_variant", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_calibrate_topp", "hardkv_solve_temperature",
+           "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_calibrate_topp", "hardkv_solve_temperature",
            "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend", "hardkv_sparse_attend",
            "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count"]
 
@@ -73,6 +73,8 @@ def _load():
     lib.hardkv_status_string.argtypes = [C.c_int]
     lib.hardkv_status_string.restype = C.c_char_p
     lib.hardkv_set_variant.argtypes = [vp, C.c_int32]
+    lib.hardkv_set_select_geometry.argtypes = [vp, C.c_int32, C.c_int32]
+    lib.hardkv_set_pdl.argtypes = [vp, C.c_int32]
     lib.hardkv_append_kv.argtypes = [vp, sp, vp, vp, vp]
     lib.hardkv_append_kv_merge.argtypes = [vp, sp, vp, vp, vp, vp]
     lib.hardkv_score.argtypes = [vp, sp, vp, vp]
@@ -154,6 +156,12 @@ class HardKV:
 
     def set_variant(self, v: int):
         _check(lib.hardkv_set_variant(self._ctx, v))
+
+    def set_select_geometry(self, cluster: int = 0, threads: int = 0):
+        _check(lib.hardkv_set_select_geometry(self._ctx, cluster, threads))
+
+    def set_pdl(self, on: bool):
+        _check(lib.hardkv_set_pdl(self._ctx, int(on)))
 
     def append_kv(self, st: DeviceState, k_new, v_new):
         _check(lib.hardkv_append_kv(self._ctx, C.byref(st.struct()), _ptr(k_new), _ptr(v_new), _stream()))

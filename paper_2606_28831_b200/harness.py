@@ -9,7 +9,7 @@ import numpy as np
 import torch
 
 from . import hardkv
-from .synth import PAGE, Workload
+from workloads.synth import PAGE, Workload
 
 
 def torch_dtype(wl: Workload):

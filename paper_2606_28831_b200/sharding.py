@@ -11,7 +11,7 @@ from __future__ import annotations
 import torch
 import torch.distributed as dist
 
-from .synth import Workload, make_workload
+from workloads.synth import Workload, make_workload
 
 
 def rank_workload(cfg_index: int, rank: int, **over) -> Workload:

@@ -8,9 +8,9 @@ from __future__ import annotations
 import numpy as np
 import torch
 
-from oracle_harness import OracleBatch
+from oracle.batch import OracleBatch
 from paper_2606_28831_b200 import harness
-from paper_2606_28831_b200.synth import PAGE, Workload
+from workloads.synth import PAGE, Workload
 
 OUT_MAX_ABS, OUT_MEAN_ABS, TAU_BAND = 2e-2, 2e-3, 1e-6
 DEV = "cuda:0"

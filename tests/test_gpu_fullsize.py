@@ -9,7 +9,7 @@ import torch
 
 from oracle.oracle import OracleConfig, Unit, decode_step_batch
 from paper_2606_28831_b200 import harness
-from paper_2606_28831_b200.synth import PAGE, make_workload
+from workloads.synth import PAGE, make_workload
 
 pytestmark = pytest.mark.gpu
 DEV = "cuda:0"

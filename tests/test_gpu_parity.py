@@ -11,7 +11,7 @@ import numpy as np
 import pytest
 import torch
 
-from paper_2606_28831_b200.synth import make_workload
+from workloads.synth import make_workload
 
 pytestmark = pytest.mark.gpu
 
@@ -167,13 +167,12 @@ def test_kernel_variants(name, variant, P):
 
 @pytest.mark.parametrize("cluster,threads", [(1, 512), (2, 512), (4, 512), (8, 512), (1, 1024), (2, 1024)])
 @pytest.mark.parametrize("name", ["c2s", "c4s", "g8"])
-def test_select_every_cluster_size(name, cluster, threads, P, monkeypatch):
+def test_select_every_cluster_size(name, cluster, threads, P):
     """The select kernel at every cluster size (1 = single CTA, no DSMEM) and both CTA sizes (512 threads, two CTAs per
     SM; 1024 threads, one per SM): bit exact from identical probabilities."""
-    monkeypatch.setenv("HARDKV_SELECT_CLUSTER", str(cluster))
-    monkeypatch.setenv("HARDKV_SELECT_THREADS", str(threads))
     wl = WL[name]
     pr = P(wl)
+    pr.eng.set_select_geometry(cluster, threads)
     for t in range(3):
         q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
         pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)

@@ -599,3 +599,42 @@ def test_golden_temperature_roots(lam, N, r, p, k, Tstar):
     it, resid = u.solve_temperature(p, t_min=0.25, t_max=4.0, eps=1e-7, max_iter=60)
     assert u.k_topp == k
     assert abs(u.T - Tstar) < 2e-3 * Tstar, (u.T, Tstar)
+
+
+# ---- P16: the steps between two compressions (do_select = 0, L274) attend every live token exactly once ----------
+@pytest.mark.parametrize("interval,p", [(4, 1.0), (5, 0.9), (3, 0.6)])
+def test_p16_reuse_steps_partition_the_live_tokens(interval, p):
+    """Between compressions only Step 1 of L78 runs: the new token joins the dense tier, which grows from the anchor
+    of the last compression; nothing retires.  So the attended positions are sinks + [dense_lo, n) + the selection of
+    the last compression + the condensed residents: no position twice, none of them dropped.  Checked against a
+    library log-sum-exp / SDPA over that explicit position list (a duplicate or a dropped token changes both), and at
+    p = 1 with large caps against dense attention over all n tokens."""
+    G, d = 3, 64
+    cfg, u, rng = _unit(G=G, d=d, n0=150, max_ctx=256, s=4, W=12, k_cap=256, C=6,
+                        l_upper=10**6 if p == 1.0 else 110)
+    sel_at = None
+    for t in range(22):
+        q = (rng.standard_normal((G, d)) * 1.5).astype(np.float32)
+        kn, vn = rng.standard_normal(d).astype(np.float32), rng.standard_normal(d).astype(np.float32)
+        do_sel = t % interval == 0
+        n_before, clo_before, cc_before = u.n, u.c_lo, u.cond_count
+        u.decode_step(q, kn, vn, p=p, do_select=do_sel)
+        assert u.n == n_before + 1
+        if do_sel:
+            sel_at = u.n
+            assert u.dense_lo == max(cfg.sink, u.n - cfg.recent)
+        else:   # no retirement, no re-anchoring between compressions
+            assert (u.c_lo, u.cond_count) == (clo_before, cc_before) and u.dense_lo == max(cfg.sink, sel_at - cfg.recent)
+        pos = list(range(min(cfg.sink, u.n))) + list(range(u.dense_lo, u.n)) + list(u.sel_idx[:u.sel_count]) + \
+            list(u.cond_pos[:u.cond_count])
+        assert len(set(pos)) == len(pos), "a position is attended twice"
+        if p == 1.0:
+            assert sorted(pos) == list(range(u.n)), "a live token is dropped"
+        Kt = torch.tensor(u.K[pos], dtype=torch.float64)[None].expand(G, -1, -1)
+        Vt = torch.tensor(u.V[pos], dtype=torch.float64)[None].expand(G, -1, -1)
+        qt = torch.tensor(q, dtype=torch.float64)
+        ref = torch.nn.functional.scaled_dot_product_attention(qt[:, None], Kt, Vt)
+        np.testing.assert_allclose(u.out, ref[:, 0].numpy(), atol=1e-5, rtol=0)
+        x = (qt @ Kt[0].T) / math.sqrt(d)
+        np.testing.assert_allclose(u.lse, torch.logsumexp(x, -1).numpy(), atol=1e-5, rtol=0)
+    assert p == 1.0 or u.cond_count > 0     # the deferred retirements did happen at the compression steps
