@@ -33,7 +33,9 @@
  *      logits                 [B][Hq][max_ctx] f32 (valid on the pool)
  *      probs                  [B][Hkv][max_ctx] f32 (valid on the pool)
  *  - "pool" of sequence b = positions [c_lo[b], max(c_lo[b], ctx_len[b]-recent)):
- *    Tier-2 candidates (L72); dense tier = [0,sink) u [ctx_len-recent, ctx_len) (L71).
+ *    Tier-2 candidates (L72); dense tier = [0,sink) u [dense_lo, ctx_len) (L71) with dense_lo =
+ *    ctx_len-recent at every compression step; between two compressions it stays put and the
+ *    dense tier grows (L78 steps 1-2).
  */
 #ifndef HARDKV_H
 #define HARDKV_H
@@ -74,6 +76,9 @@ typedef struct {
                           /* head (the pooling pass is not launched)                                */
   int32_t cond_merge;     /* 1: the evictee of a full condensed tier is merged into a resident with  */
                           /* the LSE-preserving weights of Appendix G (Eq. 9) instead of dropped     */
+  int32_t reuse_max;      /* most decode steps between two compressions (L274: 128; 0 when every step */
+                          /* selects): the dense tier grows by one token per such step (L78 steps 1-2) */
+                          /* and the attention grid is sized for recent + reuse_max dense rows        */
 } hardkv_config;
 
 /* Caller-owned device state of one layer.  Pointers marked (opt) may be NULL. */
@@ -90,6 +95,9 @@ typedef struct {
   uint8_t *sel_mask;                /* (opt) [B][Hkv][max_ctx/8], bit i%8 of byte i/8 (L439)                */
   float *logits, *probs;
   int32_t *err_flag;                /* one device int                                                    */
+  int32_t *dense_lo;                /* [B] first position of the recent part of the dense tier: ctx_len - recent at the
+                                       last compression step (written by the append stage of a compression step); the
+                                       caller initialises it to max(min(sink, n), n - recent)                     */
 } hardkv_state;
 
 /* Scratch the caller must provide to hardkv_create (device memory, 256-byte aligned). */
@@ -110,9 +118,9 @@ hardkv_status hardkv_set_select_geometry(hardkv_ctx *ctx, int32_t cluster, int32
  * its top, so ordering is that of a plain stream launch).  Default 0: measured slower inside a captured graph. */
 hardkv_status hardkv_set_pdl(hardkv_ctx *ctx, int32_t on);
 
-/* Step 1 + Step 4 of L78.  Writes (k_new, v_new) [B][Hkv][d] at position ctx_len[b];
- * ctx_len += 1; while the pool exceeds l_upper[b] its oldest token retires into the
- * condensed tier of every head, ranked on its Cautious-Update votes (L76, L86). */
+/* Step 1 + Step 4 of L78 (the bookkeeping of a compression step).  Writes (k_new, v_new) [B][Hkv][d] at position
+ * ctx_len[b]; ctx_len += 1; while the pool exceeds l_upper[b] its oldest token retires into the
+ * condensed tier of every head, ranked on its Cautious-Update votes (L76, L86); dense_lo = ctx_len - recent. */
 hardkv_status hardkv_append_kv(hardkv_ctx *, const hardkv_state *, const void *k_new, const void *v_new,
                                hardkv_stream);
 /* hardkv_append_kv with the step's queries q [B][Hq][d]: when cfg.cond_merge is set, every retirement from a full
@@ -165,9 +173,11 @@ enum {
   HARDKV_STEP_SELECT_SPARSE = 2,  /* compression step, HA-Sparse: score, calibrate + Top-p, attention through sel_idx */
   HARDKV_STEP_REUSE_SPARSE = 3    /* between two compressions, HA-Sparse: attention through the previous sel_idx      */
 };
-/* The whole step on one stream: append, retire, then per do_select (above): score, calibrate + Top-p, rewrite
- * fused with attention (selected rows are read once) / attention over the previous selected tier (the steps
- * between two compressions, L274) / the HA-Sparse forms that never touch the selected tier. */
+/* The whole step on one stream.  Compression steps (do_select 1, 2): append, retire, score, calibrate + Top-p, then
+ * rewrite fused with attention (selected rows are read once) or the HA-Sparse attention.  Steps between two
+ * compressions (do_select 0, 3; L274): append only -- the token joins the dense tier, which grows from dense_lo (L78
+ * steps 1-2), nothing retires -- then attention over dense + the tier / indices of the last compression + condensed:
+ * every live token exactly once.  At most cfg.reuse_max such steps may follow one compression (err_flag = 2 beyond). */
 hardkv_status hardkv_decode_step(hardkv_ctx *, const hardkv_state *, const void *q, const void *k_new,
                                  const void *v_new, float p, int32_t do_select, float *out,
                                  float *lse /* nullable */, hardkv_stream);

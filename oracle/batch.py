@@ -53,3 +53,6 @@ class OracleBatch:
 
     def c_lo(self) -> np.ndarray:
         return np.array([self.units[b * self.wl.Hkv].c_lo for b in range(self.wl.B)], np.int32)
+
+    def dense_lo(self) -> np.ndarray:
+        return np.array([self.units[b * self.wl.Hkv].dense_lo for b in range(self.wl.B)], np.int32)

@@ -248,6 +248,19 @@ def decode_step_batch(units: list[Unit], q: np.ndarray, k_new: np.ndarray, v_new
     return nt
 
 
+def topp_select_row(cfg: OracleConfig, probs: np.ndarray, lo: int, hi: int, l_lower: int, p: float):
+    """hko_topp_select on a caller-supplied probability row probs[max_ctx] with pool [lo, hi).
+    Returns (sel_idx[:k] ascending, k, k_topp, tau_bits).  Marshalling only: votes are not counted."""
+    probs = np.ascontiguousarray(probs, np.float32)
+    sel = np.full(max(cfg.k_cap, 1), -1, np.int32)
+    u = HkoUnit()
+    u.n, u.c_lo, u.l_lower = hi + cfg.recent, lo, l_lower
+    u.probs, u.sel_idx = _fp(probs), _ip(sel)
+    cc = cfg.c()
+    lib().hko_topp_select(C.byref(cc), C.byref(u), np.float32(p), 0)
+    return sel[:u.sel_count].copy(), int(u.sel_count), int(u.k_topp), int(u.tau_bits)
+
+
 def state_of_set(cfg: OracleConfig, q_g, K, V, idx=None):
     """(o[d], m, l) of Eq. 5 for rows idx of K/V (float32 [rows][d])."""
     K, V, q_g = _f32(K), _f32(V), _f32(q_g)

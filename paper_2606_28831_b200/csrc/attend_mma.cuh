@@ -41,8 +41,11 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   constexpr int ROWB = D * 2;
   const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
   const int n = P.st.ctx_len[b];
-  const int s_end = min(P.sink, n);
-  const int r_lo = max(n - P.recent, s_end);
+  int s_end, r_lo;
+  if (!dense_bounds(P, b, n, s_end, r_lo)) {   // more reuse steps than cfg.reuse_max: flag, leave the unit untouched
+    if (threadIdx.x == 0 && blockIdx.x == 0) atomicExch(P.st.err_flag, 2);
+    return;
+  }
   const int n_dense = s_end + (n - r_lo);
   const int k = P.st.sel_count[unit];
   const int cc = P.st.cond_count[unit];

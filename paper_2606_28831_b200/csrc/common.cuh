@@ -12,6 +12,7 @@ constexpr int PAGE = 16;
 // Everything a kernel needs, passed by value (no device-side config object to keep in sync).
 struct Params {
   int B, Hq, Hkv, G, d, max_ctx, sink, recent, k_cap, cond_cap, accum_window;
+  int reuse_max;  // most steps between two compressions: the dense tier may hold recent + reuse_max rows
   int ppu;        // base pages per unit  = max_ctx / PAGE
   int spu;        // selected pages per unit = k_cap / PAGE
   int att_chunks; // static number of attention chunks per unit
@@ -122,6 +123,15 @@ __device__ __forceinline__ float warp_sum_f32(float v) {
   for (int o = 16; o; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
   return v;
 }
+// Dense tier of sequence b with context n (PAPER.md L71, L78 steps 1-2): sinks [0, s_end) and [r_lo, n), r_lo = dense_lo
+// = n - recent at the last compression step.  Returns false (the caller flags the unit) when the tier outgrew the
+// recent + reuse_max rows the attention grid was sized for.
+__device__ __forceinline__ bool dense_bounds(const Params &P, int b, int n, int &s_end, int &r_lo) {
+  s_end = min(P.sink, n);
+  r_lo = min(max(P.st.dense_lo[b], s_end), n);
+  return n - r_lo <= P.recent + P.reuse_max;
+}
+
 constexpr int SCORE_PAGES_PER_CTA = 64;  // score kernel: 8 warps x 8 pages = 1024 tokens = 256 KiB of K per CTA
 
 __device__ __forceinline__ unsigned long long shfl_xor_u64(unsigned long long v, int off) {

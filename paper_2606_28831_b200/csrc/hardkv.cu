@@ -36,7 +36,7 @@ struct WsLayout { size_t part, arrive, stats, stage_q, stage_k, stage_v, stage_o
 size_t esize_of(const hardkv_config &c) { return c.kv_dtype == HARDKV_F32 ? 4 : 2; }
 
 int att_chunks_of(const hardkv_config &c) {
-  return (c.sink + c.recent + c.k_cap + c.cond_cap + ATT_CHUNK - 1) / ATT_CHUNK;
+  return (c.sink + c.recent + c.reuse_max + c.k_cap + c.cond_cap + ATT_CHUNK - 1) / ATT_CHUNK;
 }
 
 int score_chunks_of(const hardkv_config &c) {
@@ -107,7 +107,8 @@ hardkv_status check_config(const hardkv_config *c) {
   if (!c) return HARDKV_ERR_INVALID_ARG;
   if (c->batch <= 0 || c->num_q_heads <= 0 || c->num_kv_heads <= 0 || c->head_dim <= 0) return HARDKV_ERR_INVALID_ARG;
   if (c->num_q_heads % c->num_kv_heads) return HARDKV_ERR_INVALID_ARG;
-  if (c->max_ctx <= 0 || c->k_cap <= 0 || c->sink < 0 || c->recent < 0 || c->cond_cap < 0) return HARDKV_ERR_INVALID_ARG;
+  if (c->max_ctx <= 0 || c->k_cap <= 0 || c->sink < 0 || c->recent < 0 || c->cond_cap < 0 || c->reuse_max < 0)
+    return HARDKV_ERR_INVALID_ARG;
   if (c->page_size != PAGE) return HARDKV_ERR_UNSUPPORTED;
   if (c->max_ctx % PAGE || c->k_cap % PAGE) return HARDKV_ERR_INVALID_ARG;
   if (c->pool_kernel < 0 || c->pool_kernel > 63 || (c->pool_kernel > 1 && c->pool_kernel % 2 == 0)) return HARDKV_ERR_INVALID_ARG;
@@ -128,7 +129,7 @@ bool state_ok(const hardkv_ctx *ctx, const hardkv_state *s) {
   if (!ctx || !s) return false;
   return s->k_pool && s->v_pool && s->base_table && s->sel_k_pool && s->sel_v_pool && s->sel_pages &&
          s->cond_count && s->ctx_len && s->c_lo && s->l_lower && s->l_upper && s->votes && s->temperature &&
-         s->score_mode && s->sel_idx && s->sel_count && s->sel_table && s->logits && s->probs && s->err_flag &&
+         s->score_mode && s->sel_idx && s->sel_count && s->sel_table && s->logits && s->probs && s->err_flag && s->dense_lo &&
          (ctx->cfg.cond_cap == 0 || (s->cond_k && s->cond_v && s->cond_pos && s->cond_votes));
 }
 
@@ -180,9 +181,10 @@ void launch_pdl(const hardkv_ctx *ctx, void (*kernel)(KArgs...), dim3 grid, dim3
 bool fast_path(const hardkv_ctx *ctx) { return ctx->variant >= 1 && ctx->cfg.kv_dtype == HARDKV_BF16; }
 
 void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, const void *q,
-                   cudaStream_t st) {
+                   int do_retire, cudaStream_t st) {
   ctx->launches += 1;
-  HK_DISPATCH_TD(ctx->cfg, (launch_pdl(ctx, append_retire_kernel<T, D>, dim3(P.B), dim3(256), 0, st, P, k_new, v_new, q)));
+  HK_DISPATCH_TD(ctx->cfg, (launch_pdl(ctx, append_retire_kernel<T, D>, dim3(P.B), dim3(256), 0, st, P, k_new, v_new, q,
+                                       do_retire)));
 }
 
 void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
@@ -313,7 +315,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   Params &P = ctx->base;
   P.B = cfg->batch; P.Hq = cfg->num_q_heads; P.Hkv = cfg->num_kv_heads; P.G = P.Hq / P.Hkv;
   P.d = cfg->head_dim; P.max_ctx = cfg->max_ctx; P.sink = cfg->sink; P.recent = cfg->recent;
-  P.k_cap = cfg->k_cap; P.cond_cap = cfg->cond_cap; P.accum_window = cfg->accum_window;
+  P.k_cap = cfg->k_cap; P.cond_cap = cfg->cond_cap; P.accum_window = cfg->accum_window; P.reuse_max = cfg->reuse_max;
   P.ppu = cfg->max_ctx / PAGE; P.spu = cfg->k_cap / PAGE;
   P.att_chunks = att_chunks_of(*cfg);
   P.sm_scale = cfg->sm_scale > 0.f ? cfg->sm_scale : 1.0f / sqrtf((float)cfg->head_dim);
@@ -376,14 +378,14 @@ hardkv_status hardkv_set_pdl(hardkv_ctx *ctx, int32_t on) {
 hardkv_status hardkv_append_kv(hardkv_ctx *ctx, const hardkv_state *s, const void *k_new, const void *v_new,
                                hardkv_stream st) {
   if (!state_ok(ctx, s) || !k_new || !v_new) return HARDKV_ERR_INVALID_ARG;
-  launch_append(ctx, params_of(ctx, s), k_new, v_new, nullptr, st);
+  launch_append(ctx, params_of(ctx, s), k_new, v_new, nullptr, 1, st);
   return launch_status();
 }
 
 hardkv_status hardkv_append_kv_merge(hardkv_ctx *ctx, const hardkv_state *s, const void *k_new, const void *v_new,
                                      const void *q, hardkv_stream st) {
   if (!state_ok(ctx, s) || !k_new || !v_new || !q) return HARDKV_ERR_INVALID_ARG;
-  launch_append(ctx, params_of(ctx, s), k_new, v_new, q, st);
+  launch_append(ctx, params_of(ctx, s), k_new, v_new, q, 1, st);
   return launch_status();
 }
 
@@ -459,8 +461,9 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
     return HARDKV_ERR_INVALID_ARG;
   const Params P = params_of(ctx, s);
   if (do_select < 0 || do_select > 3) return HARDKV_ERR_INVALID_ARG;
-  launch_append(ctx, P, k_new, v_new, q, st);
-  if (do_select == HARDKV_STEP_SELECT_REWRITE || do_select == HARDKV_STEP_SELECT_SPARSE) {
+  const bool compress = do_select == HARDKV_STEP_SELECT_REWRITE || do_select == HARDKV_STEP_SELECT_SPARSE;
+  launch_append(ctx, P, k_new, v_new, q, compress ? 1 : 0, st);   // between compressions: Step 1 only (L78, L274)
+  if (compress) {
     launch_score(ctx, P, q, st);
     launch_pool(ctx, P, st);
     // the score kernel's chunk statistics describe the raw logits: configs with pooled heads take them in-kernel

@@ -69,21 +69,28 @@ __host__ __device__ __forceinline__ int sel_slice_len(int span, int C, int nt) {
   return (per + nt - 1) / nt * nt;
 }
 
-// CALIBRATE: 1 = logits -> probs (2a) then select; 0 = select on state->probs as given.
+// Loads of data that another CTA of the SAME launch may have written (the fused score -> select kernel): L2-coherent
+// ld.global.cg; otherwise the read-only path.
+template <bool COHERENT> __device__ __forceinline__ float4 sel_ld4(const float4 *p) { return COHERENT ? __ldcg(p) : __ldg(p); }
+template <bool COHERENT> __device__ __forceinline__ float sel_ld(const float *p) { return COHERENT ? __ldcg(p) : __ldg(p); }
+template <bool COHERENT> __device__ __forceinline__ float2 sel_ld2(const float2 *p) { return COHERENT ? __ldcg(p) : __ldg(p); }
+
+// Stages 2a-2c for ONE (sequence, KV head) unit, run by every thread of the CTA (and of its cluster when CLUSTERED).
+// CALIBRATE: 1 = logits -> probs (2a) with in-kernel statistics, 2 = with the chunk statistics of the score kernel,
+//            0 = select on state->probs as given.
 // GMAX: compile-time bound of the GQA group (4 or 8) -- sizes the register arrays of the calibration.
 // NT: threads per CTA (SEL_NT: two CTAs per SM; SEL_NT_BIG: one CTA per SM that holds a whole unit without a cluster).
-template <int CALIBRATE, int GMAX, int NT>
-__global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Params P, float p) {
+// CLUSTERED: the unit is split over the P.sel_cluster CTAs of a thread-block cluster (DSMEM exchange); false = one CTA.
+// COHERENT: logits / chunk statistics were written earlier in this same launch (score_select_kernel).
+// pbits: this CTA's slice of the probability row, sh: its scratch, both in shared memory.
+template <int CALIBRATE, int GMAX, int NT, bool CLUSTERED, bool COHERENT>
+__device__ __forceinline__ void select_unit(const Params &P, float p, int unit, uint32_t *pbits, SelShared &sh) {
   constexpr int NW = NT / 32;
-  pdl_wait_then_trigger();
-  extern __shared__ __align__(16) unsigned char sel_smem[];
   cg::cluster_group cluster = cg::this_cluster();
-  const int C = P.sel_cluster;
-  const int rank = (int)cluster.block_rank();
-  const int unit = blockIdx.x / C, b = unit / P.Hkv, h = unit % P.Hkv;
+  const int C = CLUSTERED ? P.sel_cluster : 1;
+  const int rank = CLUSTERED ? (int)cluster.block_rank() : 0;
+  const int b = unit / P.Hkv, h = unit % P.Hkv;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  uint32_t *pbits = reinterpret_cast<uint32_t *>(sel_smem);                       // [P.sel_slice_cap]
-  SelShared &sh = *reinterpret_cast<SelShared *>(sel_smem + (size_t)P.sel_slice_cap * 4);
 
   int n, lo, hi;
   pool_bounds(P, b, n, lo, hi);
@@ -131,10 +138,10 @@ __global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Pa
       if (warp < G) {   // warp g reduces the chunk statistics of query head g (lanes over chunks)
         const int g = warp;
         float m = -INFINITY, sacc = 0.f;
-        for (int c = ch0 + lane; c <= ch1; c += 32) m = fmaxf(m, __ldg(&sp[(size_t)c * 8 + g]).x);
+        for (int c = ch0 + lane; c <= ch1; c += 32) m = fmaxf(m, sel_ld2<COHERENT>(&sp[(size_t)c * 8 + g]).x);
         m = warp_max_f32(m);
         for (int c = ch0 + lane; c <= ch1; c += 32) {
-          const float2 v = __ldg(&sp[(size_t)c * 8 + g]);
+          const float2 v = sel_ld2<COHERENT>(&sp[(size_t)c * 8 + g]);
           sacc += v.y * fast_exp2(v.x - m);
         }
         sacc = warp_sum_f32(sacc);
@@ -158,7 +165,7 @@ __global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Pa
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int pos = s0 + i0 + u * NT;
-            x[u] = (i0 + u * NT < per && pos >= lo && pos < hi) ? __ldg(row + pos) * c2 : -INFINITY;
+            x[u] = (i0 + u * NT < per && pos >= lo && pos < hi) ? sel_ld<COHERENT>(row + pos) * c2 : -INFINITY;
           }
           const float mn = fmaxf(fmaxf(fmaxf(x[0], x[1]), fmaxf(x[2], x[3])), m);
           if (mn != -INFINITY) {
@@ -222,11 +229,11 @@ __global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Pa
             if (live && g < G) {
               const float *src = lg + (size_t)g * P.max_ctx + pos;
               if (vec) {
-                x[u][g] = __ldg(reinterpret_cast<const float4 *>(src));
+                x[u][g] = sel_ld4<COHERENT>(reinterpret_cast<const float4 *>(src));
               } else {
-                if (pos < P.max_ctx) x[u][g].x = __ldg(src);
-                if (pos + 1 < P.max_ctx) x[u][g].y = __ldg(src + 1);
-                if (pos + 2 < P.max_ctx) x[u][g].z = __ldg(src + 2);
+                if (pos < P.max_ctx) x[u][g].x = sel_ld<COHERENT>(src);
+                if (pos + 1 < P.max_ctx) x[u][g].y = sel_ld<COHERENT>(src + 1);
+                if (pos + 2 < P.max_ctx) x[u][g].z = sel_ld<COHERENT>(src + 2);
               }
             }
           }
@@ -275,7 +282,7 @@ __global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Pa
           float pr = 0.f;
 #pragma unroll
           for (int g = 0; g < GMAX; ++g)
-            if (g < G) pr = fmaf(fast_exp2(fmaf(__ldg(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
+            if (g < G) pr = fmaf(fast_exp2(fmaf(sel_ld<COHERENT>(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
           float a = (acc[pos] - ring[pos]) + pr;
           a = fmaxf(a, 0.f);
           acc[pos] = a;
@@ -624,6 +631,16 @@ __global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Pa
     for (int y = y1 + gt_; y < mask_bytes; y += gs_) mask[y] = 0;
   }
   if (C > 1) cluster.sync();  // no CTA may exit while a peer can still read its shared memory
+}
+
+// One thread-block cluster (or one CTA) per (sequence, KV head).
+template <int CALIBRATE, int GMAX, int NT>
+__global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Params P, float p) {
+  pdl_wait_then_trigger();
+  extern __shared__ __align__(16) unsigned char sel_smem[];
+  uint32_t *pbits = reinterpret_cast<uint32_t *>(sel_smem);                       // [P.sel_slice_cap]
+  SelShared &sh = *reinterpret_cast<SelShared *>(sel_smem + (size_t)P.sel_slice_cap * 4);
+  select_unit<CALIBRATE, GMAX, NT, true, false>(P, p, blockIdx.x / P.sel_cluster, pbits, sh);
 }
 
 }  // namespace hardkv

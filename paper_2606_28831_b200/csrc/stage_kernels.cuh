@@ -11,9 +11,12 @@ namespace hardkv {
 // constant-size condensed tier (L76), ranked on Cautious-Update votes (L86).
 // One CTA per sequence, one warp per KV head (ctx_len / c_lo are per sequence: they are read by
 // every warp before the barrier and written by thread 0 after it).
+// do_retire = 0 is the step between two compressions (L274): Step 1 only -- the token joins the dense tier, nothing
+// retires and the dense anchor stays (L78 steps 1-2); do_retire = 1 is the bookkeeping of a compression step.
 // =============================================================================================
 template <typename T, int D>
-__global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void *k_new, const void *v_new, const void *q_) {
+__global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void *k_new, const void *v_new, const void *q_,
+                                                            int do_retire) {
   pdl_wait_then_trigger();
   constexpr int ROWB = D * sizeof(T);
   constexpr int LPR = ROWB / 16;  // 16-byte vectors per row
@@ -53,7 +56,7 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
     const int32_t *votes = P.st.votes + (size_t)unit * P.max_ctx;
     clo = clo0;
     bool qbar_ready = false;
-    while (n1 - P.recent - clo > lup) {
+    while (do_retire && n1 - P.recent - clo > lup) {
       const int t = clo;
       int slot = -1;
       const bool full = cnt >= P.cond_cap && P.cond_cap > 0;   // a full tier produces an evictee (merging, reading C17)
@@ -168,15 +171,19 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
       }
       ++clo;
     }
-    if (lane == 0) P.st.cond_count[unit] = cnt;
+    if (lane == 0) {
+      P.st.cond_count[unit] = cnt;
+      P.att_arrive[unit] = 0;   // re-arm the split-K arrival counter of the attention that follows (a launch that
+    }                           // failed midway must not poison the next step)
   }
   // every warp computed the same final c_lo (or ran no head: recompute it arithmetically)
   __syncthreads();
   if (threadIdx.x == 0) {
     int c = clo0;
-    if (n1 - P.recent - c > lup) c = n1 - P.recent - lup;
+    if (do_retire && n1 - P.recent - c > lup) c = n1 - P.recent - lup;
     P.st.ctx_len[b] = n1;
     P.st.c_lo[b] = c;
+    if (do_retire) P.st.dense_lo[b] = max(min(P.sink, n1), n1 - P.recent);   // re-anchor the dense tier (L71)
   }
 }
 
@@ -307,8 +314,11 @@ __global__ void __launch_bounds__(256) attend_generic_kernel(Params P, const voi
   constexpr int UNR = 4;
   const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
   const int n = P.st.ctx_len[b];
-  const int s_end = min(P.sink, n);
-  const int r_lo = max(n - P.recent, s_end);
+  int s_end, r_lo;
+  if (!dense_bounds(P, b, n, s_end, r_lo)) {   // more reuse steps than cfg.reuse_max: flag, leave the unit untouched
+    if (threadIdx.x == 0 && blockIdx.x == 0) atomicExch(P.st.err_flag, 2);
+    return;
+  }
   const int n_dense = s_end + (n - r_lo);
   const int k = P.st.sel_count[unit];
   const int cc = P.st.cond_count[unit];

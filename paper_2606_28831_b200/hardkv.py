@@ -39,13 +39,14 @@ def build(force: bool = False) -> str:
 class Config(C.Structure):
     _fields_ = [(n, C.c_int32) for n in (
         "batch", "num_q_heads", "num_kv_heads", "head_dim", "page_size", "max_ctx", "sink", "recent", "k_cap",
-        "cond_cap", "accum_window", "kv_dtype")] + [("sm_scale", C.c_float), ("pool_kernel", C.c_int32), ("cond_merge", C.c_int32)]
+        "cond_cap", "accum_window", "kv_dtype")] + [("sm_scale", C.c_float), ("pool_kernel", C.c_int32), ("cond_merge", C.c_int32),
+                                        ("reuse_max", C.c_int32)]
 
 
 _STATE_FIELDS = ["k_pool", "v_pool", "base_table", "sel_k_pool", "sel_v_pool", "sel_pages", "cond_k", "cond_v",
                  "cond_pos", "cond_votes", "cond_count", "ctx_len", "c_lo", "l_lower", "l_upper", "votes",
                  "temperature", "score_mode", "acc", "ring", "ring_slot", "sel_idx", "sel_count", "sel_table",
-                 "sel_mask", "logits", "probs", "err_flag"]
+                 "sel_mask", "logits", "probs", "err_flag", "dense_lo"]
 
 
 class StateStruct(C.Structure):
@@ -138,9 +139,10 @@ class HardKV:
     """One hardkv_ctx.  Every method enqueues kernels on torch's current stream and returns at once."""
 
     def __init__(self, *, batch, num_q_heads, num_kv_heads, head_dim, max_ctx, sink, recent, k_cap, cond_cap,
-                 kv_dtype, accum_window=0, page_size=16, sm_scale=0.0, pool_kernel=0, cond_merge=0, device="cuda:0"):
+                 kv_dtype, accum_window=0, page_size=16, sm_scale=0.0, pool_kernel=0, cond_merge=0, reuse_max=0,
+                 device="cuda:0"):
         self.cfg = Config(batch, num_q_heads, num_kv_heads, head_dim, page_size, max_ctx, sink, recent, k_cap,
-                          cond_cap, accum_window, kv_dtype, sm_scale, pool_kernel, cond_merge)
+                          cond_cap, accum_window, kv_dtype, sm_scale, pool_kernel, cond_merge, reuse_max)
         nbytes = C.c_size_t()
         _check(lib.hardkv_workspace_bytes(C.byref(self.cfg), C.byref(nbytes)))
         self.workspace = torch.zeros(nbytes.value + 256, dtype=torch.uint8, device=device)

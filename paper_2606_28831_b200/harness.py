@@ -5,6 +5,8 @@ method's arithmetic lives here.  Layouts are those of include/hardkv.h.
 """
 from __future__ import annotations
 
+import dataclasses
+
 import numpy as np
 import torch
 
@@ -16,13 +18,13 @@ def torch_dtype(wl: Workload):
     return torch.bfloat16 if wl.dtype == "bf16" else torch.float32
 
 
-def make_engine(wl: Workload, device="cuda:0", want_accum=None) -> hardkv.HardKV:
+def make_engine(wl: Workload, device="cuda:0", want_accum=None, reuse_max: int = 0) -> hardkv.HardKV:
     accum = bool(np.any(wl.score_mode == 1)) if want_accum is None else want_accum
     return hardkv.HardKV(batch=wl.B, num_q_heads=wl.Hq, num_kv_heads=wl.Hkv, head_dim=wl.d, max_ctx=wl.max_ctx,
                          sink=wl.sink, recent=wl.recent, k_cap=wl.k_cap, cond_cap=wl.cond_cap,
                          kv_dtype=hardkv.BF16 if wl.dtype == "bf16" else hardkv.F32,
                          accum_window=wl.accum_window if accum else 0, sm_scale=float(wl.sm_scale),
-                         pool_kernel=wl.pool_kernel, cond_merge=wl.cond_merge, device=device)
+                         pool_kernel=wl.pool_kernel, cond_merge=wl.cond_merge, reuse_max=reuse_max, device=device)
 
 
 def to_dev(x: np.ndarray, wl: Workload, device="cuda:0") -> torch.Tensor:
@@ -30,11 +32,16 @@ def to_dev(x: np.ndarray, wl: Workload, device="cuda:0") -> torch.Tensor:
     return torch.from_numpy(np.ascontiguousarray(x, np.float32)).to(device).to(torch_dtype(wl)).contiguous()
 
 
-def make_state(wl: Workload, device="cuda:0", prefill=None, want_mask=False, layers: int = 1):
+def make_state(wl: Workload, device="cuda:0", prefill=None, want_mask=False, layers: int = 1, retain=None,
+               layer_seeds=None):
     """Allocate and fill the device state of `layers` layers (page tables shared by all layers, L207-209).
 
     prefill: optional dict (b, h) -> (K0, V0) float32; generated from wl when absent.
-    Returns (list of DeviceState, prefill dict or None).  Layers l > 0 reuse layer 0's prefill
+    retain: optional set of (b, h): only these units' host prefill arrays are kept in the returned dict
+    (full-size tests that sample units; the 64k-context configs would otherwise hold GBs of host memory).
+    layer_seeds: optional list of `layers` seeds: layer l is filled from the workload re-seeded with layer_seeds[l]
+    (independent data per layer; the returned dict is then keyed (l, b, h)).
+    Returns (list of DeviceState, prefill dict or None).  Without layer_seeds, layers l > 0 reuse layer 0's prefill
     values rolled by l rows (distinct addresses and data; the same statistics).
     """
     B, Hkv, Hq, d, mc = wl.B, wl.Hkv, wl.Hq, wl.d, wl.max_ctx
@@ -53,10 +60,20 @@ def make_state(wl: Workload, device="cuda:0", prefill=None, want_mask=False, lay
         v_pool = torch.zeros(units * ppu, PAGE, d, dtype=dt, device=device)
         for b in range(B):
             for h in range(Hkv):
-                if layer == 0:
+                if layer_seeds is not None:
+                    wl_l = dataclasses.replace(wl)
+                    wl_l.seed = layer_seeds[layer]
+                    K0, V0 = wl_l.prefill_unit(b, h)
+                    if retain is None or (b, h) in retain:
+                        keep[(layer, b, h)] = (K0, V0)
+                    kd, vd = to_dev(K0, wl, device), to_dev(V0, wl, device)
+                elif layer == 0:
                     if (b, h) not in keep:
-                        keep[(b, h)] = wl.prefill_unit(b, h)
-                    K0, V0 = keep[(b, h)]
+                        K0, V0 = wl.prefill_unit(b, h)
+                        if retain is None or (b, h) in retain:
+                            keep[(b, h)] = (K0, V0)
+                    else:
+                        K0, V0 = keep[(b, h)]
                     kd, vd = to_dev(K0, wl, device), to_dev(V0, wl, device)
                 else:
                     src = states[0]
@@ -96,6 +113,7 @@ def make_state(wl: Workload, device="cuda:0", prefill=None, want_mask=False, lay
             logits=torch.zeros(B * Hq, mc, dtype=torch.float32, device=device),
             probs=torch.zeros(units, mc, dtype=torch.float32, device=device),
             err_flag=torch.zeros(1, dtype=torch.int32, device=device),
+            dense_lo=i32(np.maximum(np.minimum(wl.sink, wl.n0), wl.n0 - wl.recent)),
         )
         states.append(st)
     return states, keep
@@ -107,7 +125,7 @@ def gather_rows(pool: torch.Tensor, table_unit: torch.Tensor, n: int) -> np.ndar
     return pool[table_unit.long()].reshape(-1, d)[:n].float().cpu().numpy()
 
 
-_MUTABLE = ["votes", "cond_k", "cond_v", "cond_pos", "cond_votes", "cond_count", "ctx_len", "c_lo", "sel_idx",
+_MUTABLE = ["votes", "cond_k", "cond_v", "cond_pos", "cond_votes", "cond_count", "ctx_len", "c_lo", "dense_lo", "sel_idx",
             "sel_count", "sel_table", "acc", "ring", "ring_slot"]
 
 

@@ -76,6 +76,7 @@ class Workload:
     temperature: np.ndarray = field(default=None)  # [B][Hkv] calibration T (reading C10: 1)
 
     def __post_init__(self):
+        self._memo = {}
         self.seed = 28831000 + self.index
         if self.l_lower is None:
             self.l_lower = np.zeros(self.B, np.int32)
@@ -94,10 +95,20 @@ class Workload:
     # ---- latent structure per (b, KV head) ---------------------------------------------
     def latent(self, b: int, h: int):
         """(q_bar[d], u_hat[d], tau): persistent query direction and logit temperature."""
-        g = _rng(self.seed, _T_LATENT, b, h)
-        qb = g.standard_normal(self.d).astype(np.float32)
-        tau = np.float32(np.exp(g.uniform(np.log(self.tau_lo), np.log(self.tau_hi))))
-        return qb, qb / np.linalg.norm(qb), tau
+        key = ("latent", self.seed, b, h, self.d, self.tau_lo, self.tau_hi)
+        if key not in self._memo:
+            g = _rng(self.seed, _T_LATENT, b, h)
+            qb = g.standard_normal(self.d).astype(np.float32)
+            tau = np.float32(np.exp(g.uniform(np.log(self.tau_lo), np.log(self.tau_hi))))
+            self._memo[key] = (qb, qb / np.linalg.norm(qb), tau)
+        return self._memo[key]
+
+    def _prefill_heavy_hitters(self, b: int, h: int) -> np.ndarray:
+        """Positions of the planted heavy hitters of the prefill (memoised: a pure function of the seed and shape)."""
+        key = ("hh", self.seed, b, h, int(self.n0[b]), self.planted)
+        if key not in self._memo:
+            self._memo[key] = np.flatnonzero(self.planted_mask(b, h, 0, int(self.n0[b])))
+        return self._memo[key]
 
     def planted_mask(self, b: int, h: int, lo: int, hi: int) -> np.ndarray:
         """Which positions in [lo, hi) carry a planted heavy hitter (data-only rule)."""
@@ -165,7 +176,7 @@ class Workload:
                 pos = int(self.n0[b]) + t
                 for h in range(self.Hkv):
                     if self.mix_new_keys:
-                        hh = np.flatnonzero(self.planted_mask(b, h, 0, int(self.n0[b])))
+                        hh = self._prefill_heavy_hitters(b, h)
                         if len(hh):
                             j = hh[int(mixr[b, h] * len(hh)) % len(hh)]
                             k[b, h] = np.float32(0.7) * k[b, h] + np.float32(0.3) * prefill_K[(b, h)][j]
