@@ -107,13 +107,21 @@ hardkv_status hardkv_workspace_bytes(const hardkv_config *cfg, size_t *bytes);
 hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t bytes, hardkv_ctx **out);
 void          hardkv_destroy(hardkv_ctx *ctx);
 const char   *hardkv_status_string(hardkv_status s);
-/* Kernel variant switch for A/B measurements: 0 = generic FMA kernels, 1 = tuned paths (default),
- * 2 = tuned paths with the TMA-staged (cp.async.bulk + mbarrier ring) persistent score kernel. */
+/* Kernel variant switch for A/B measurements: 0 = generic FMA kernels, 1 = tuned separate kernels,
+ * 2 = the same with the TMA-staged (cp.async.bulk + mbarrier ring) persistent score kernel, 3 = score and selection
+ * fused into one persistent kernel (bf16, no SNAPKV head, a unit's pool must fit one SM's shared memory:
+ * HARDKV_ERR_UNSUPPORTED elsewhere).  Default 1 (3 measured slower on B200: DESIGN.md section 7). */
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant);
 /* Geometry of the select kernel, for A/B measurements and tests: cluster = CTAs per (b, h) in {1, 2, 4, 8}, threads per
  * CTA in {512, 1024}; 0 keeps the automatic choice for that argument.  HARDKV_ERR_UNSUPPORTED when a CTA's slice of the
  * pool would not fit one SM's shared memory.  Host-side only; call it before capturing a graph with this ctx. */
 hardkv_status hardkv_set_select_geometry(hardkv_ctx *ctx, int32_t cluster, int32_t threads);
+/* Measurement hook: while `slots` (DEVICE memory, 2 * capacity u64, the caller presets every pair to (~0, 0)) is set,
+ * the i-th hot-kernel launch made through this ctx (append, score, select, score_select, attend; generic variants
+ * excepted) records the globaltimer ns at which its first CTA started and its last CTA ended in slots[2 i], slots[2 i
+ * + 1] -- also inside a captured graph, which is how bench.py reports per-kernel times of the graph it times.  Calling
+ * it again restarts the slot counter; slots = NULL (the default) turns it off and the kernels pay nothing. */
+hardkv_status hardkv_set_timing(hardkv_ctx *ctx, unsigned long long *slots, int32_t capacity);
 /* 1: launch the hot kernels with the programmatic-dependent-launch attribute (each kernel waits for its predecessor at
  * its top, so ordering is that of a plain stream launch).  Default 0: measured slower inside a captured graph. */
 hardkv_status hardkv_set_pdl(hardkv_ctx *ctx, int32_t on);
@@ -136,6 +144,10 @@ hardkv_status hardkv_score(hardkv_ctx *, const hardkv_state *, const void *q, ha
 /* Logits Calibration (apply-T) -> probs, then hardkv_topp_select.  SNAPKV heads (cfg.pool_kernel > 1)
  * are calibrated on their logits max-pooled along the sequence, window clipped to the pool (L278). */
 hardkv_status hardkv_calibrate_topp(hardkv_ctx *, const hardkv_state *, float p, hardkv_stream);
+/* hardkv_score followed by hardkv_calibrate_topp as ONE call (stages 1 + 2a-2c; same results).  With
+ * kernel variant 3 this is a single persistent launch: CTAs stream K pages, and the CTA that retires the last chunk of
+ * a unit runs that unit's calibration + Top-p + compaction while the others keep streaming. */
+hardkv_status hardkv_score_select(hardkv_ctx *, const hardkv_state *, const void *q, float p, hardkv_stream);
 /* Logits Calibration, solve-T: Algorithm 2 "Binary Search on T" (L625-648) for Problem 1 (L108-110), run at a
  * request's first compression (L607).  Needs state->logits of a preceding hardkv_score.  Per (b, KV head):
  * k = Num_Selected_TopP(S, p) with S the raw attention scores (group mean of softmax(z), T = 1, no k_cap clamp);

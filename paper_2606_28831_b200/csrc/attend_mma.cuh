@@ -36,6 +36,7 @@ __device__ __forceinline__ float bf16_round(float x) { return __bfloat162float(_
 template <int D, int MODE>
 __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void *q_, float *out, float *lse) {
   pdl_wait_then_trigger();
+  KernelClock kclock(P);
   constexpr int NKC = D / 32;   // 64-byte chunks of a key row
   constexpr int NVC = D / 64;   // 128-byte chunks of a value row
   constexpr int ROWB = D * 2;

@@ -29,6 +29,31 @@ struct Params {
   float *pooled;         // [B][Hq][max_ctx] max-pooled logits of SNAPKV heads (NULL when pool_kernel <= 1)
   int pool_kernel;       // SNAPKV max-pool window (odd), <= 1: no SNAPKV head in this config
   int cond_merge;        // 1: evictees of a full condensed tier are merged into a resident (Appendix G)
+  // fused score -> select kernel (score_select.cuh)
+  int ss_slice_cap;      // capacity (tokens) of the probability slice of one unit held by one 1024-thread CTA
+  int32_t *ss_next;      // [1] next work item (zero between launches)
+  int32_t *ss_arrive;    // [units] chunks of a unit scanned so far (zero between launches)
+  // in-graph kernel timing (hardkv_set_timing): NULL in normal runs
+  unsigned long long *timing;   // [2 * slots]: (start of the first CTA, end of the last CTA) in globaltimer ns per launch
+  int timing_slot;
+};
+
+// Records when the first CTA of a launch starts and when its last CTA ends (thread 0 of every CTA: one atomicMin, one
+// atomicMax), so that bench.py can report each kernel's duration INSIDE the captured graph it times.  Costs nothing
+// when P.timing is NULL.  The destructor covers every return path.
+struct KernelClock {
+  unsigned long long *slot;
+  static __device__ __forceinline__ unsigned long long now() {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+  }
+  __device__ __forceinline__ explicit KernelClock(const Params &P) : slot(P.timing ? P.timing + 2 * P.timing_slot : nullptr) {
+    if (slot && threadIdx.x == 0) atomicMin(slot, now());
+  }
+  __device__ __forceinline__ ~KernelClock() {
+    if (slot && threadIdx.x == 0) atomicMax(slot + 1, now());
+  }
 };
 
 // ---- programmatic dependent launch (PDL): every hot kernel waits here for the preceding kernel of the stream to complete

@@ -32,6 +32,7 @@ __device__ __forceinline__ void mma_bf16_16816(float (&c)[4], uint32_t a0, uint3
 template <int D>
 __global__ void __launch_bounds__(256) score_mma_kernel(Params P, const void *q_) {
   pdl_wait_then_trigger();
+  KernelClock kclock(P);
   constexpr int NCH = D / 32;                 // 64-byte chunks per row
   constexpr int ROWB = D * 2;
   const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;

@@ -12,6 +12,7 @@
 #include "stage_kernels.cuh"
 #include "attend_mma.cuh"
 #include "metric_kernels.cuh"
+#include "score_select.cuh"
 
 using namespace hardkv;
 
@@ -19,6 +20,9 @@ struct hardkv_ctx {
   hardkv_config cfg;
   Params base;      // config-derived fields + workspace pointers; `st` is filled per call
   int variant;
+  int fused_ok;                  // the fused score -> select kernel applies to this config (score_select.cuh)
+  unsigned long long *timing;    // hardkv_set_timing: per-launch (first CTA start, last CTA end), or NULL
+  int timing_cap, timing_next;
   int pdl;                       // 1: launches carry the programmatic-stream-serialization attribute (hardkv_set_pdl)
   int num_sms;
   size_t ws_bytes;
@@ -31,7 +35,7 @@ namespace {
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout { size_t part, arrive, stats, stage_q, stage_k, stage_v, stage_out, pooled, total; };
+struct WsLayout { size_t part, arrive, ss, stats, stage_q, stage_k, stage_v, stage_out, pooled, total; };
 
 size_t esize_of(const hardkv_config &c) { return c.kv_dtype == HARDKV_F32 ? 4 : 2; }
 
@@ -49,6 +53,7 @@ WsLayout ws_layout(const hardkv_config &c) {
   WsLayout w;
   size_t off = 0;
   w.arrive = off; off += align256(units * sizeof(int32_t));
+  w.ss = off;     off += align256((units + 1) * sizeof(int32_t));
   w.part = off;   off += align256(units * att_chunks_of(c) * G * (c.head_dim + 2) * sizeof(float));
   w.stats = off;  off += align256(units * score_chunks_of(c) * 8 * sizeof(float2));
   const size_t qb = (size_t)c.batch * c.num_q_heads * c.head_dim, kb = units * c.head_dim;
@@ -59,6 +64,17 @@ WsLayout ws_layout(const hardkv_config &c) {
   w.pooled = off;    off += c.pool_kernel > 1 ? align256((size_t)c.batch * c.num_q_heads * c.max_ctx * sizeof(float)) : 0;
   w.total = off;
   return w;
+}
+
+// The fused score -> select kernel holds a whole unit's probability slice in one 1024-thread CTA.
+int ss_slice_cap_of(const hardkv_config &c) {
+  const int max_pool = c.max_ctx - c.recent > 0 ? c.max_ctx - c.recent : 1;
+  return sel_slice_len(max_pool + 31, 1, SS_THREADS);
+}
+bool fused_eligible(const hardkv_config &c) {
+  const int units = c.batch * c.num_kv_heads;
+  return c.kv_dtype == HARDKV_BF16 && c.pool_kernel <= 1 && units <= SS_MAX_UNITS &&
+         score_select_smem(c.head_dim, ss_slice_cap_of(c), units, c.batch) <= 227u * 1024u;
 }
 
 size_t select_smem_bytes(const Params &P) { return (size_t)P.sel_slice_cap * 4 + sizeof(SelShared); }
@@ -139,6 +155,17 @@ Params params_of(const hardkv_ctx *ctx, const hardkv_state *s) {
   return P;
 }
 
+// Params of ONE launch: takes the next timing slot when hardkv_set_timing is active.
+Params launch_params(hardkv_ctx *ctx, const Params &P0) {
+  Params P = P0;
+  P.timing = nullptr;
+  if (ctx->timing && ctx->timing_next < ctx->timing_cap) {
+    P.timing = ctx->timing;
+    P.timing_slot = ctx->timing_next++;
+  }
+  return P;
+}
+
 // Dispatch on (dtype, head_dim) and on G where the kernel keeps per-head registers.
 #define HK_DISPATCH_TD(cfg, ...)                                                                   \
   do {                                                                                             \
@@ -180,14 +207,16 @@ void launch_pdl(const hardkv_ctx *ctx, void (*kernel)(KArgs...), dim3 grid, dim3
 // bf16 tensor-core paths (variant 1); fp32 K/V and variant 0 run the generic FMA kernels
 bool fast_path(const hardkv_ctx *ctx) { return ctx->variant >= 1 && ctx->cfg.kv_dtype == HARDKV_BF16; }
 
-void launch_append(hardkv_ctx *ctx, const Params &P, const void *k_new, const void *v_new, const void *q,
+void launch_append(hardkv_ctx *ctx, const Params &P0, const void *k_new, const void *v_new, const void *q,
                    int do_retire, cudaStream_t st) {
+  const Params P = launch_params(ctx, P0);
   ctx->launches += 1;
   HK_DISPATCH_TD(ctx->cfg, (launch_pdl(ctx, append_retire_kernel<T, D>, dim3(P.B), dim3(256), 0, st, P, k_new, v_new, q,
                                        do_retire)));
 }
 
-void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
+void launch_score(hardkv_ctx *ctx, const Params &P0, const void *q, cudaStream_t st) {
+  const Params P = launch_params(ctx, P0);
   ctx->launches += 1;
   dim3 grid(P.score_chunks, P.B * P.Hkv);
   if (fast_path(ctx) && ctx->variant == 2) {   // TMA-staged persistent variant (A/B: see DESIGN.md)
@@ -206,7 +235,8 @@ void launch_score(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t 
 
 // calibrate: 0 = select on probs as given, 1 = logits -> probs with in-kernel statistics,
 // 2 = logits -> probs with the chunk statistics the bf16 score kernel left in the workspace
-void launch_select(hardkv_ctx *ctx, const Params &P, float p, int calibrate, cudaStream_t st) {
+void launch_select(hardkv_ctx *ctx, const Params &P0, float p, int calibrate, cudaStream_t st) {
+  const Params P = launch_params(ctx, P0);
   ctx->launches += 1;
   cudaLaunchConfig_t lc = {};
   lc.gridDim = dim3(P.B * P.Hkv * P.sel_cluster);
@@ -237,6 +267,21 @@ void launch_select(hardkv_ctx *ctx, const Params &P, float p, int calibrate, cud
 #undef HK_SEL
 }
 
+// stages 1 + 2a-2c as one persistent kernel, one CTA per SM (variant 3)
+void launch_score_select(hardkv_ctx *ctx, const Params &P0, const void *q, float p, cudaStream_t st) {
+  const Params P = launch_params(ctx, P0);
+  ctx->launches += 1;
+  const size_t smem = score_select_smem(P.d, P.ss_slice_cap, P.B * P.Hkv, P.B);
+  const dim3 grid(ctx->num_sms), block(SS_THREADS);
+  if (P.d == 128) {
+    if (P.G <= 4) launch_pdl(ctx, score_select_kernel<128, 4>, grid, block, smem, st, P, q, p);
+    else launch_pdl(ctx, score_select_kernel<128, 8>, grid, block, smem, st, P, q, p);
+  } else {
+    if (P.G <= 4) launch_pdl(ctx, score_select_kernel<64, 4>, grid, block, smem, st, P, q, p);
+    else launch_pdl(ctx, score_select_kernel<64, 8>, grid, block, smem, st, P, q, p);
+  }
+}
+
 // SNAPKV metric transform (L278): only configs that declare a pooling window pay for the launch
 void launch_pool(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
   if (P.pool_kernel <= 1) return;
@@ -251,19 +296,21 @@ void launch_rewrite(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
   HK_DISPATCH_TD(ctx->cfg, (rewrite_kernel<T, D><<<grid, 256, 0, st>>>(P)));
 }
 
-void launch_attend(hardkv_ctx *ctx, const Params &P, const void *q, float *out, float *lse, int mode,
+void launch_attend(hardkv_ctx *ctx, const Params &P0, const void *q, float *out, float *lse, int mode,
                    cudaStream_t st) {
+  const Params P = launch_params(ctx, P0);
   ctx->launches += 1;
   if (fast_path(ctx)) {
     dim3 gm((P.att_chunks * ATT_CHUNK + ATT_MMA_CHUNK - 1) / ATT_MMA_CHUNK, P.B * P.Hkv);
+    const size_t sm = 0;
     if (P.d == 128) {
-      if (mode == ATT_REWRITE) launch_pdl(ctx, attend_mma_kernel<128, ATT_REWRITE>, gm, dim3(256), 0, st, P, q, out, lse);
-      else if (mode == ATT_SPARSE) launch_pdl(ctx, attend_mma_kernel<128, ATT_SPARSE>, gm, dim3(256), 0, st, P, q, out, lse);
-      else launch_pdl(ctx, attend_mma_kernel<128, ATT_TIER>, gm, dim3(256), 0, st, P, q, out, lse);
+      if (mode == ATT_REWRITE) launch_pdl(ctx, attend_mma_kernel<128, ATT_REWRITE>, gm, dim3(256), sm, st, P, q, out, lse);
+      else if (mode == ATT_SPARSE) launch_pdl(ctx, attend_mma_kernel<128, ATT_SPARSE>, gm, dim3(256), sm, st, P, q, out, lse);
+      else launch_pdl(ctx, attend_mma_kernel<128, ATT_TIER>, gm, dim3(256), sm, st, P, q, out, lse);
     } else {
-      if (mode == ATT_REWRITE) launch_pdl(ctx, attend_mma_kernel<64, ATT_REWRITE>, gm, dim3(256), 0, st, P, q, out, lse);
-      else if (mode == ATT_SPARSE) launch_pdl(ctx, attend_mma_kernel<64, ATT_SPARSE>, gm, dim3(256), 0, st, P, q, out, lse);
-      else launch_pdl(ctx, attend_mma_kernel<64, ATT_TIER>, gm, dim3(256), 0, st, P, q, out, lse);
+      if (mode == ATT_REWRITE) launch_pdl(ctx, attend_mma_kernel<64, ATT_REWRITE>, gm, dim3(256), sm, st, P, q, out, lse);
+      else if (mode == ATT_SPARSE) launch_pdl(ctx, attend_mma_kernel<64, ATT_SPARSE>, gm, dim3(256), sm, st, P, q, out, lse);
+      else launch_pdl(ctx, attend_mma_kernel<64, ATT_TIER>, gm, dim3(256), sm, st, P, q, out, lse);
     }
     return;
   }
@@ -321,6 +368,9 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.sm_scale = cfg->sm_scale > 0.f ? cfg->sm_scale : 1.0f / sqrtf((float)cfg->head_dim);
   char *base = reinterpret_cast<char *>(workspace);
   P.att_arrive = reinterpret_cast<int32_t *>(base + w.arrive);
+  P.ss_arrive = reinterpret_cast<int32_t *>(base + w.ss);
+  P.ss_next = P.ss_arrive + (size_t)cfg->batch * cfg->num_kv_heads;
+  P.ss_slice_cap = ss_slice_cap_of(*cfg);
   P.part = reinterpret_cast<float *>(base + w.part);
   P.score_stats = reinterpret_cast<float2 *>(base + w.stats);
   P.score_chunks = score_chunks_of(*cfg);
@@ -346,6 +396,20 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
     delete ctx;
     return HARDKV_ERR_CUDA;
   }
+  ctx->fused_ok = fused_eligible(*cfg) ? 1 : 0;
+  if (ctx->fused_ok) {
+    static int ss_smem_max = 0;
+    const int need = (int)score_select_smem(cfg->head_dim, P.ss_slice_cap, cfg->batch * cfg->num_kv_heads, cfg->batch);
+    if (need > ss_smem_max) ss_smem_max = need;
+    const cudaFuncAttribute fa = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    if (cudaFuncSetAttribute(score_select_kernel<128, 4>, fa, ss_smem_max) != cudaSuccess ||
+        cudaFuncSetAttribute(score_select_kernel<128, 8>, fa, ss_smem_max) != cudaSuccess ||
+        cudaFuncSetAttribute(score_select_kernel<64, 4>, fa, ss_smem_max) != cudaSuccess ||
+        cudaFuncSetAttribute(score_select_kernel<64, 8>, fa, ss_smem_max) != cudaSuccess) {
+      cudaGetLastError();
+      ctx->fused_ok = 0;
+    }
+  }
   *out = ctx;
   return HARDKV_OK;
 }
@@ -353,7 +417,8 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
 void hardkv_destroy(hardkv_ctx *ctx) { delete ctx; }
 
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant) {
-  if (!ctx || variant < 0 || variant > 2) return HARDKV_ERR_INVALID_ARG;
+  if (!ctx || variant < 0 || variant > 3) return HARDKV_ERR_INVALID_ARG;
+  if (variant == 3 && !ctx->fused_ok) return HARDKV_ERR_UNSUPPORTED;
   ctx->variant = variant;
   return HARDKV_OK;
 }
@@ -367,6 +432,14 @@ hardkv_status hardkv_set_select_geometry(hardkv_ctx *ctx, int32_t cluster, int32
   if ((size_t)cap * 4 + sizeof(SelShared) > 227u * 1024u) return HARDKV_ERR_UNSUPPORTED;
   ctx->base.sel_cluster = cl; ctx->base.sel_slice_cap = cap; ctx->base.sel_nt = nt;
   return raise_select_smem(ctx->base) ? HARDKV_OK : HARDKV_ERR_CUDA;
+}
+
+hardkv_status hardkv_set_timing(hardkv_ctx *ctx, unsigned long long *slots, int32_t capacity) {
+  if (!ctx || capacity < 0 || (slots && capacity == 0)) return HARDKV_ERR_INVALID_ARG;
+  ctx->timing = slots;
+  ctx->timing_cap = slots ? capacity : 0;
+  ctx->timing_next = 0;
+  return HARDKV_OK;
 }
 
 hardkv_status hardkv_set_pdl(hardkv_ctx *ctx, int32_t on) {
@@ -405,6 +478,19 @@ hardkv_status hardkv_calibrate_topp(hardkv_ctx *ctx, const hardkv_state *s, floa
   if (!state_ok(ctx, s) || !(p > 0.f) || !accum_ok(ctx, s)) return HARDKV_ERR_INVALID_ARG;
   launch_pool(ctx, params_of(ctx, s), st);
   launch_select(ctx, params_of(ctx, s), p, 1, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_score_select(hardkv_ctx *ctx, const hardkv_state *s, const void *q, float p, hardkv_stream st) {
+  if (!state_ok(ctx, s) || !q || !(p > 0.f) || !accum_ok(ctx, s)) return HARDKV_ERR_INVALID_ARG;
+  const Params P = params_of(ctx, s);
+  if (ctx->variant == 3) {
+    launch_score_select(ctx, P, q, p, st);
+  } else {
+    launch_score(ctx, P, q, st);
+    launch_pool(ctx, P, st);
+    launch_select(ctx, P, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
+  }
   return launch_status();
 }
 
@@ -463,7 +549,9 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   if (do_select < 0 || do_select > 3) return HARDKV_ERR_INVALID_ARG;
   const bool compress = do_select == HARDKV_STEP_SELECT_REWRITE || do_select == HARDKV_STEP_SELECT_SPARSE;
   launch_append(ctx, P, k_new, v_new, q, compress ? 1 : 0, st);   // between compressions: Step 1 only (L78, L274)
-  if (compress) {
+  if (compress && ctx->variant == 3) {
+    launch_score_select(ctx, P, q, p, st);
+  } else if (compress) {
     launch_score(ctx, P, q, st);
     launch_pool(ctx, P, st);
     // the score kernel's chunk statistics describe the raw logits: configs with pooled heads take them in-kernel

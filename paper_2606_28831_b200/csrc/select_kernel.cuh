@@ -637,6 +637,7 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
 template <int CALIBRATE, int GMAX, int NT>
 __global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Params P, float p) {
   pdl_wait_then_trigger();
+  KernelClock kclock(P);
   extern __shared__ __align__(16) unsigned char sel_smem[];
   uint32_t *pbits = reinterpret_cast<uint32_t *>(sel_smem);                       // [P.sel_slice_cap]
   SelShared &sh = *reinterpret_cast<SelShared *>(sel_smem + (size_t)P.sel_slice_cap * 4);

@@ -18,6 +18,7 @@ template <typename T, int D>
 __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void *k_new, const void *v_new, const void *q_,
                                                             int do_retire) {
   pdl_wait_then_trigger();
+  KernelClock kclock(P);
   constexpr int ROWB = D * sizeof(T);
   constexpr int LPR = ROWB / 16;  // 16-byte vectors per row
   constexpr int EPL = Elem<T>::EPL;
@@ -173,8 +174,10 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
     }
     if (lane == 0) {
       P.st.cond_count[unit] = cnt;
-      P.att_arrive[unit] = 0;   // re-arm the split-K arrival counter of the attention that follows (a launch that
-    }                           // failed midway must not poison the next step)
+      P.att_arrive[unit] = 0;   // re-arm the arrival counters of the kernels that follow (a launch that failed midway
+      P.ss_arrive[unit] = 0;    // must not poison the next step)
+      if (unit == 0) *P.ss_next = 0;
+    }
   }
   // every warp computed the same final c_lo (or ran no head: recompute it arithmetically)
   __syncthreads();

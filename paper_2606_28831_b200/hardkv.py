@@ -56,7 +56,7 @@ class StateStruct(C.Structure):
 F32, BF16 = 0, 1
 STEP_REUSE_TIER, STEP_SELECT_REWRITE, STEP_SELECT_SPARSE, STEP_REUSE_SPARSE = 0, 1, 2, 3   # do_select of decode_step
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
-           "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_calibrate_topp", "hardkv_solve_temperature",
+           "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_timing", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_score_select", "hardkv_calibrate_topp", "hardkv_solve_temperature",
            "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend", "hardkv_sparse_attend",
            "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count"]
 
@@ -76,10 +76,12 @@ def _load():
     lib.hardkv_set_variant.argtypes = [vp, C.c_int32]
     lib.hardkv_set_select_geometry.argtypes = [vp, C.c_int32, C.c_int32]
     lib.hardkv_set_pdl.argtypes = [vp, C.c_int32]
+    lib.hardkv_set_timing.argtypes = [vp, vp, C.c_int32]
     lib.hardkv_append_kv.argtypes = [vp, sp, vp, vp, vp]
     lib.hardkv_append_kv_merge.argtypes = [vp, sp, vp, vp, vp, vp]
     lib.hardkv_score.argtypes = [vp, sp, vp, vp]
     lib.hardkv_calibrate_topp.argtypes = [vp, sp, C.c_float, vp]
+    lib.hardkv_score_select.argtypes = [vp, sp, vp, C.c_float, vp]
     lib.hardkv_solve_temperature.argtypes = [vp, sp, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int32, vp]
     lib.hardkv_topp_select.argtypes = [vp, sp, C.c_float, vp]
     lib.hardkv_rewrite.argtypes = [vp, sp, vp]
@@ -162,6 +164,14 @@ class HardKV:
     def set_select_geometry(self, cluster: int = 0, threads: int = 0):
         _check(lib.hardkv_set_select_geometry(self._ctx, cluster, threads))
 
+    def set_timing(self, slots=None):
+        """slots: int64 CUDA tensor [capacity][2] preset to (max, 0) per row, or None to turn the hook off."""
+        if slots is None:
+            _check(lib.hardkv_set_timing(self._ctx, None, 0))
+        else:
+            assert slots.is_cuda and slots.is_contiguous() and slots.dtype == torch.int64 and slots.shape[1] == 2
+            _check(lib.hardkv_set_timing(self._ctx, _ptr(slots), slots.shape[0]))
+
     def set_pdl(self, on: bool):
         _check(lib.hardkv_set_pdl(self._ctx, int(on)))
 
@@ -173,6 +183,9 @@ class HardKV:
 
     def score(self, st: DeviceState, q):
         _check(lib.hardkv_score(self._ctx, C.byref(st.struct()), _ptr(q), _stream()))
+
+    def score_select(self, st: DeviceState, q, p: float):
+        _check(lib.hardkv_score_select(self._ctx, C.byref(st.struct()), _ptr(q), np.float32(p), _stream()))
 
     def calibrate_topp(self, st: DeviceState, p: float):
         _check(lib.hardkv_calibrate_topp(self._ctx, C.byref(st.struct()), np.float32(p), _stream()))

@@ -153,12 +153,20 @@ def test_fused_decode_step(name, teacher, P):
           f"first divergence step {first_div}, max-abs output error over the run {emax:.2e}")
 
 
-@pytest.mark.parametrize("variant", [0, 2])
+@pytest.mark.parametrize("variant", [0, 2, 3])
 @pytest.mark.parametrize("name", ["c1s", "c2s", "c3s", "c4s", "g1d64", "snap4"])
 def test_kernel_variants(name, variant, P):
-    """Variant 0 (generic fp32-FMA kernels) and variant 2 (TMA-staged persistent score) against the oracle."""
+    """Variant 0 (generic fp32-FMA kernels), 2 (TMA-staged persistent score) and 3 (score and selection fused into one
+    persistent kernel: CTAs stream K pages and the CTA that retires a unit's last chunk runs its selection) against the
+    oracle; the default is variant 1.  Variant 3 does not apply to configs with SNAPKV heads (the pooling pass sits
+    between score and select)."""
+    from paper_2606_28831_b200 import hardkv
     wl = WL[name]
     pr = P(wl, want_mask=False)
+    if variant == 3 and wl.pool_kernel > 1:
+        with pytest.raises(hardkv.HardKVError):
+            pr.eng.set_variant(3)
+        return
     pr.eng.set_variant(variant)
     for t in range(min(wl.steps, 8)):
         q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
@@ -190,6 +198,37 @@ def test_select_every_cluster_size(name, cluster, threads, P):
         pr.st.votes.copy_(votes0)
         np.testing.assert_array_equal(pr.st.sel_idx.cpu().numpy(), pr.ob.sel_idx())
         np.testing.assert_array_equal(pr.st.sel_count.cpu().numpy(), pr.ob.sel_count())
+
+
+@pytest.mark.parametrize("variant", [1, 3])
+@pytest.mark.parametrize("name", ["c2s", "c3s", "c4s", "g8"])
+def test_score_select_entry(name, variant, P):
+    """hardkv_score_select (stages 1 + 2a-2c in one call) against the oracle stages: logits, probabilities and the
+    selection -- as separate kernels (variant 1) and as the fused persistent kernel (variant 3), over several steps so
+    that units of different lengths finish their scan at different times; also a batch of more chunks than SMs."""
+    import dataclasses
+    wl = WL[name]
+    if name == "c2s":    # more (unit, chunk) work items than CTAs: CTAs take several items and switch role mid-kernel
+        wl = make_workload(2, B=12, n0=np.linspace(1400, 5200, 12).astype(np.int32), max_ctx=5376, k_cap=512,
+                           l_upper=np.linspace(1400, 5200, 12).astype(np.int32) - 132, cond_cap=16, steps=4)
+    pr = P(wl)
+    pr.eng.set_variant(variant)
+    for t in range(min(wl.steps, 4)):
+        q, kn, vn, (qd, knd, vnd) = pr.inputs(t)
+        pr.eng.append_kv(pr.st, knd, vnd)
+        pr.eng.score_select(pr.st, qd, wl.p)
+        qu = q.reshape(-1, wl.G, wl.d)
+        for i, u in enumerate(pr.ob.units):
+            u.append(kn.reshape(-1, wl.d)[i], vn.reshape(-1, wl.d)[i])
+            u.retire()
+            u.score(qu[i]); u.calibrate(); u.topp_select(wl.p, True)
+        pr.check_bookkeeping()
+        pr.check_logits()
+        pr.check_probs()
+        if pr.check_selection_band() == 0:
+            pr.check_selection_exact()
+        pr.force_discrete_state()
+    assert int(pr.st.err_flag.item()) == 0
 
 
 def test_select_interval_reuses_selected_tier(P):
