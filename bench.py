@@ -31,8 +31,29 @@ METRIC = "decode_step_kv_bandwidth"      # B_min / time of the fused select+rewr
 UNIT = "GB/s"
 NOMINAL_HBM_GBS = 8000.0                 # the contract's "8 TB/s"
 FALLBACK_HBM_GBS = 6650.0                # B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from `ncu --set full` (profiles/r1_03_final.md), config 2
-NCU_TRAFFIC_BYTES = {2: {"score": 586.4e6, "rewrite_attend": 279.6e6, "calibrate_topp": 41.6e6}}
+TRAFFIC_PROFILE = os.path.join("profiles", "r2_ncu_traffic.json")   # ncu dram bytes per launch + the source hash they belong to
+
+
+def source_hash() -> str:
+    """sha256 over the kernel sources and the ABI header: ties a stored ncu capture to the code it was taken from."""
+    import hashlib
+    h = hashlib.sha256()
+    base = os.path.join(ROOT, "paper_2606_28831_b200", "csrc")
+    for f in sorted(os.listdir(base)) + ["../../include/hardkv.h"]:
+        h.update(open(os.path.join(base, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def profiled_traffic(config: int, variant: int, kernel: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of `kernel` from the committed ncu capture, or None when
+    the capture was taken from other sources, another config or another kernel variant."""
+    try:
+        prof = json.load(open(os.path.join(ROOT, TRAFFIC_PROFILE)))
+    except Exception:
+        return None, None
+    if prof.get("source_hash") != source_hash() or prof.get("config") != config or prof.get("variant") != variant:
+        return None, {"file": TRAFFIC_PROFILE, "stale": True}
+    return prof.get("kernels", {}).get(kernel), {"file": TRAFFIC_PROFILE, "source_hash": prof["source_hash"]}
 
 
 def log(*a):
@@ -168,7 +189,7 @@ def run_cuda(args):
 
     import __graft_entry__
     __graft_entry__.build_cuda()
-    from paper_2606_28831_b200 import accounting, harness, sharding
+    from paper_2606_28831_b200 import accounting, hardkv, harness, sharding
 
     K, W = args.steps, args.warmup
     over = {}
@@ -187,14 +208,17 @@ def run_cuda(args):
     if args.p:
         wl.p = args.p
     L = args.layers or (32 if args.config == 1 else 1)
+    SI = args.select_interval
     t0 = time.time()
-    eng = harness.make_engine(wl, dev)
-    if args.variant != 1:
+    eng = harness.make_engine(wl, dev)                       # the headline engine: every step selects (reuse_max = 0)
+    eng_am = harness.make_engine(wl, dev, reuse_max=SI)      # the paper's periodic regime: the dense tier grows in between
+    default_variant = 1
+    if args.variant != default_variant:
         eng.set_variant(args.variant)
+        eng_am.set_variant(args.variant)
     if K + W > (wl.max_ctx - int(wl.n0.max())) * L:
         raise SystemExit(f"steps + warmup must be <= {(wl.max_ctx - int(wl.n0.max())) * L} for {wl.name} with {L} layer(s)")
     states, prefill = harness.make_state(wl, dev, layers=L)   # step t runs on layer t % L (distinct data, shared tables)
-    st = states[0]
     pk = {u: kv[0] for u, kv in prefill.items()} if wl.mix_new_keys else None
     tdt = harness.torch_dtype(wl)
     qs, ks, vs = [], [], []
@@ -202,10 +226,19 @@ def run_cuda(args):
         qs.append(wl.step_q(t))
         kn, vn = wl.step_kv(t, pk)
         ks.append(kn); vs.append(vn)
-    q_h = torch.from_numpy(np.stack(qs)).to(tdt).pin_memory()      # [W+K][B][Hq][d] pinned host
-    k_h = torch.from_numpy(np.stack(ks)).to(tdt).pin_memory()
-    v_h = torch.from_numpy(np.stack(vs)).to(tdt).pin_memory()
-    q_d, k_d, v_d = q_h.to(dev), k_h.to(dev), v_h.to(dev)          # resident in HBM before the timed region
+    # host inputs of every step packed [q | k_new | v_new] in ONE pinned buffer (the host entry then needs one H2D copy)
+    nq, nk = wl.B * wl.Hq * wl.d, wl.B * wl.Hkv * wl.d
+    qkv_h = torch.empty(W + K, nq + 2 * nk, dtype=tdt).pin_memory()
+    qkv_h[:, :nq] = torch.from_numpy(np.stack(qs)).to(tdt).reshape(W + K, nq)
+    qkv_h[:, nq:nq + nk] = torch.from_numpy(np.stack(ks)).to(tdt).reshape(W + K, nk)
+    qkv_h[:, nq + nk:] = torch.from_numpy(np.stack(vs)).to(tdt).reshape(W + K, nk)
+    q_h = [qkv_h[t, :nq].view(wl.B, wl.Hq, wl.d) for t in range(W + K)]
+    k_h = [qkv_h[t, nq:nq + nk].view(wl.B, wl.Hkv, wl.d) for t in range(W + K)]
+    v_h = [qkv_h[t, nq + nk:].view(wl.B, wl.Hkv, wl.d) for t in range(W + K)]
+    qkv_d = qkv_h.to(dev)                                     # resident in HBM before the device-timed region starts
+    q_d = [qkv_d[t, :nq].view(wl.B, wl.Hq, wl.d) for t in range(W + K)]
+    k_d = [qkv_d[t, nq:nq + nk].view(wl.B, wl.Hkv, wl.d) for t in range(W + K)]
+    v_d = [qkv_d[t, nq + nk:].view(wl.B, wl.Hkv, wl.d) for t in range(W + K)]
     out = torch.zeros(wl.B, wl.Hq, wl.d, dtype=torch.float32, device=dev)
     out_h = torch.zeros(wl.B, wl.Hq, wl.d, dtype=torch.float32).pin_memory()
     if rank == 0:
@@ -219,11 +252,19 @@ def run_cuda(args):
             dist.barrier()
         torch.cuda.synchronize()
 
-    def warm():
+    def warm(e=None):
+        e = e or eng
         for x, sn in zip(states, snaps):
             harness.restore(x, sn)
         for t in range(W):
-            eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
+            e.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
+
+    def capture_steps():
+        g_ = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g_):
+            for t in range(W, W + K):
+                eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
+        return g_
 
     # ---- (1) device-resident timed region: K fused steps --------------------------------------
     warm()
@@ -244,10 +285,7 @@ def run_cuda(args):
     else:
         # the K steps captured into ONE CUDA graph (static shapes, counts on the device: L53, L63) and replayed once:
         # the state advances on the device exactly as in the eager loop
-        graph = torch.cuda.CUDAGraph()
-        with torch.cuda.graph(graph):
-            for t in range(W, W + K):
-                eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out)
+        graph = capture_steps()
         barrier()
         e0.record(stream)
         graph.replay()
@@ -259,7 +297,39 @@ def run_cuda(args):
     assert all(int(x.err_flag.item()) == 0 for x in states), "device err_flag set"
     assert bool(torch.isfinite(out).all()), "non-finite attention output"
 
-    # ---- (2) same steps, stage by stage with events (kernel shares + per-step byte counts) ------
+    # ---- (1b) the same K-step graph once more with the timing hook on: every kernel's duration INSIDE the graph
+    #      (first CTA start -> last CTA end, globaltimer) and the idle gaps between kernels ------------------------------
+    per_launch = launches // K
+    NAMES = {4: ["append_retire", "score", "calibrate_topp", "rewrite_attend"],
+             3: ["append_retire", "score_select", "rewrite_attend"],
+             5: ["append_retire", "score", "maxpool", "calibrate_topp", "rewrite_attend"]}.get(per_launch)
+    in_graph = None
+    if NAMES and not args.eager:
+        slots = torch.empty(launches, 2, dtype=torch.int64, device=dev)
+        slots[:, 0] = torch.iinfo(torch.int64).max
+        slots[:, 1] = 0
+        warm()
+        eng.set_timing(slots)
+        g2 = capture_steps()
+        eng.set_timing(None)
+        slots[:, 0] = torch.iinfo(torch.int64).max       # capture does not execute, but keep the preset explicit
+        slots[:, 1] = 0
+        torch.cuda.synchronize()
+        g2.replay()
+        torch.cuda.synchronize()
+        ts = slots.cpu().numpy().reshape(K, per_launch, 2).astype(np.float64)
+        dur = (ts[:, :, 1] - ts[:, :, 0]) / 1e3                                # [K][kernels] us
+        gaps = (ts[:, 1:, 0] - ts[:, :-1, 1]) / 1e3                            # idle between consecutive kernels of a step
+        step_gap = (ts[1:, 0, 0] - ts[:-1, -1, 1]) / 1e3                       # idle between steps
+        in_graph = {"kernels_us": {n: float(dur[:, i].mean()) for i, n in enumerate(NAMES)},
+                    "gaps_us": {f"{NAMES[i]}->{NAMES[i + 1]}": float(gaps[:, i].mean()) for i in range(per_launch - 1)},
+                    "step_to_step_gap_us": float(step_gap.mean()) if K > 1 else 0.0,
+                    "step_us": float((ts[-1, -1, 1] - ts[0, 0, 0]) / 1e3 / K),
+                    "how": "hardkv_set_timing: globaltimer at the first CTA's start and the last CTA's end of every launch "
+                           "of a second capture of the same K-step graph"}
+        del g2
+
+    # ---- (2) same steps, stage by stage (per-step byte counts; eager stand-alone stage times as context) ------
     warm()
     STAGES = ["append_retire", "score", "calibrate_topp", "rewrite_attend"]
     ev = [[torch.cuda.Event(enable_timing=True) for _ in range(len(STAGES) + 1)] for _ in range(K)]
@@ -284,11 +354,14 @@ def run_cuda(args):
     per_step = [accounting.algorithmic_bytes(wl, cn[i], clo[i], csel[i], ccond[i]) for i in range(K)]
     bytes_total = sum(p["total"] for p in per_step)
     bytes_stage = {"score": float(np.mean([p["score"] for p in per_step])),
-                   "rewrite_attend": float(np.mean([p["attend"] + p["rewrite_write"] for p in per_step]))}
+                   "score_select": float(np.mean([p["score"] for p in per_step])),
+                   "rewrite_attend": float(np.mean([p["attend"] + p["rewrite_write"] for p in per_step])),
+                   "calibrate_topp": float(np.mean([p["select_bytes"] for p in per_step])),
+                   "append_retire": 0.0, "maxpool": 0.0}
 
     # ---- (2b) context lines: the unfused five-call pipeline, and the paper's amortised regime (L274) ------------
-    def timed_loop(body):
-        warm()
+    def timed_loop(body, e=None):
+        warm(e)
         a, b_ = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         a.record(stream)
@@ -303,14 +376,14 @@ def run_cuda(args):
         eng.append_kv(s_, k_d[t], v_d[t]); eng.score(s_, q_d[t]); eng.calibrate_topp(s_, wl.p)
         eng.rewrite(s_); eng.decode_attn(s_, q_d[t], out)
 
-    SI = args.select_interval
     unfused_us = timed_loop(five_calls)
-    amortised_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out,
-                                                        do_select=((t - W) // L) % SI == 0))
+    # between two compressions only Step 1 runs: the token joins the dense tier, nothing retires (L78 steps 1-2, L274)
+    amortised_us = timed_loop(lambda t: eng_am.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out,
+                                                           do_select=((t - W) // L) % SI == 0), eng_am)
     # HA-Sparse (Sparse Loading, L178 / L191): attention gathers through sel_idx, the selected tier is never written
     sparse_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out, do_select=2))
-    sparse_amortised_us = timed_loop(lambda t: eng.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out,
-                                                               do_select=2 if ((t - W) // L) % SI == 0 else 3))
+    sparse_amortised_us = timed_loop(lambda t: eng_am.decode_step(states[t % L], q_d[t], k_d[t], v_d[t], wl.p, out,
+                                                                  do_select=2 if ((t - W) // L) % SI == 0 else 3), eng_am)
     solve_us = None
     if args.snapkv_window:   # Algorithm 2 (L625-648), run once per request (L607): timed on the first step's logits
         warm()
@@ -327,20 +400,37 @@ def run_cuda(args):
     kv_cond = float(2 * row_b * units_ * wl.cond_cap)
     kv_tier = float(2 * row_b * units_ * wl.k_cap)                                # static HA-Max capacity (L191-195)
 
+    # ---- (2c) read-only streaming probe: what a plain 16-byte read loop reaches on this GPU (context for the K scan)
+    probe_buf = states[0].k_pool
+    for _ in range(2):
+        hardkv.probe_read_stream(probe_buf)
+    pa, pb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    pa.record(stream)
+    for _ in range(5):
+        hardkv.probe_read_stream(probe_buf)
+    pb.record(stream)
+    torch.cuda.synchronize()
+    read_probe_gbs = probe_buf.numel() * probe_buf.element_size() * 5 / (pa.elapsed_time(pb) * 1e-3) / 1e9
+
     # ---- (3) end to end through the host-buffer entry point -------------------------------------
-    # (3a) eager: one hardkv_decode_step_host call per step (3 H2D copies, 4 kernels, 1 D2H copy, stream sync)
+    # one hardkv_decode_step_host call per step on that step's PINNED HOST inputs (packed q | k_new | v_new: one H2D
+    # copy), the attention kernel stores the output straight into pinned host memory (no D2H copy), then a stream
+    # synchronise: the caller reads out_h before the next token
     warm()
     torch.cuda.synchronize()
     barrier()
     t_e2e0 = time.perf_counter()
     for t in range(W, W + K):
         eng.decode_step_host(states[t % L], q_h[t], k_h[t], v_h[t], wl.p, out_h)
-        stream.synchronize()                      # the caller reads out_h before the next token
+        stream.synchronize()
     t_e2e_eager = time.perf_counter() - t_e2e0
-    # (3b) the same call captured once per layer into a CUDA graph over fixed pinned buffers (the entry point never
-    # synchronises, so it is capturable): per step the host writes that step's q / k / v into the pinned buffers, replays
-    # (H2D copies + the step + D2H of the output, all inside the graph) and synchronises before reading the output
-    pin_q, pin_k, pin_v = (torch.empty_like(x[0]).pin_memory() for x in (q_h, k_h, v_h))
+    assert bool(torch.isfinite(out_h).all()), "non-finite output through the host entry"
+    # the same call captured once per layer into a CUDA graph over one fixed pinned input buffer: per step the host
+    # writes that step's packed inputs into it, replays (H2D copy + the step), synchronises
+    pin_in = torch.empty_like(qkv_h[0]).pin_memory()
+    pin_q, pin_k, pin_v = (pin_in[:nq].view(wl.B, wl.Hq, wl.d), pin_in[nq:nq + nk].view(wl.B, wl.Hkv, wl.d),
+                           pin_in[nq + nk:].view(wl.B, wl.Hkv, wl.d))
     warm()
     torch.cuda.synchronize()
     host_graphs = []
@@ -352,13 +442,17 @@ def run_cuda(args):
     barrier()
     t_e2e0 = time.perf_counter()
     for t in range(W, W + K):
-        pin_q.copy_(q_h[t]); pin_k.copy_(k_h[t]); pin_v.copy_(v_h[t])
+        pin_in.copy_(qkv_h[t])
         host_graphs[t % L].replay()
-        stream.synchronize()                      # the caller reads out_h before the next token
-    t_e2e = time.perf_counter() - t_e2e0
+        stream.synchronize()
+    t_e2e_graph = time.perf_counter() - t_e2e0
     assert bool(torch.isfinite(out_h).all()), "non-finite output through the host entry"
-    h2d = (q_h[0].numel() + k_h[0].numel() + v_h[0].numel()) * q_h.element_size()
+    t_e2e = min(t_e2e_eager, t_e2e_graph)
+    h2d = qkv_h[0].numel() * qkv_h.element_size()
     d2h = out_h.numel() * 4
+
+    # ---- (4) --cond-merge: LSE drift of the condensed tier, merging vs eviction vs keeping everything ---------------
+    drift = lse_drift(args, dev) if (args.cond_merge and world == 1) else None
 
     # ---- reduce over ranks ------------------------------------------------------------------------
     ms_total, ms_e2e, bytes_all = sharding.reduce_run(ms_total, t_e2e * 1e3, bytes_total, dev)
@@ -368,19 +462,23 @@ def run_cuda(args):
         gbs = sharding.job_throughput_gbs(ms_total, bytes_all)
         e2e_gbs = bytes_all / (ms_e2e * 1e-3) / 1e9
         us_step = ms_total / K * 1e3
-        dom = max(("score", "rewrite_attend", "calibrate_topp"), key=lambda s: stage_us[s])
+        times = in_graph["kernels_us"] if in_graph else stage_us
+        dom = max(times, key=lambda s_: times[s_])
+        plain = not (args.n0 or args.p or args.snapkv_window or args.cond_merge or args.contiguous_pages or args.layers)
+        traffic, traffic_from = profiled_traffic(args.config, args.variant, dom) if plain else (None, None)
         roof = {"kernel": dom, "bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
-                "traffic": NCU_TRAFFIC_BYTES.get(args.config, {}).get(dom)
-                if not (args.n0 or args.p or args.snapkv_window or args.cond_merge or args.contiguous_pages) else None}
-        if dom in bytes_stage:
-            roof["achieved"] = bytes_stage[dom] / (stage_us[dom] * 1e-6) / 1e9
-            roof["algorithmic_bytes_per_launch"] = bytes_stage[dom]
-        else:  # the select kernel moves no algorithmic KV bytes: report its logits+probs traffic
-            lb = float(np.mean([p["select_bytes"] for p in per_step]))
-            roof["achieved"] = lb / (stage_us[dom] * 1e-6) / 1e9
-            roof["algorithmic_bytes_per_launch"] = lb
+                "achieved": bytes_stage[dom] / (times[dom] * 1e-6) / 1e9,
+                "algorithmic_bytes_per_launch": bytes_stage[dom], "avg_launch_us": times[dom],
+                "timed": "inside the timed CUDA graph (hardkv_set_timing)" if in_graph else "eager stand-alone stage calls",
+                "traffic": traffic, "traffic_from": traffic_from,
+                "read_probe_gbs": read_probe_gbs,
+                "read_probe_note": "plain 16-byte grid-stride read of the K pool (hardkv_probe_read_stream), measured in "
+                                   "this run: the read-only ceiling beside the copy peak",
+                "step": {"achieved": gbs / world, "peak": peak, "frac": gbs / world / peak,
+                         "algorithmic_bytes_per_step": bytes_all / K / world, "us": us_step,
+                         "note": "whole layer-step: B_min of all stages / step time of the timed graph"}}
         roof["frac"] = roof["achieved"] / peak
-        roof["avg_launch_us"] = stage_us[dom]
+        roof["frac_of_read_probe"] = roof["achieved"] / read_probe_gbs
         line = {
             "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -393,7 +491,8 @@ def run_cuda(args):
                        "launch": "eager" if args.eager else "one CUDA graph of the K steps",
                        "l2": "inputs larger than L2 (K scan %.0f MB per layer-step x %d layer(s) of distinct data cycled), "
                              "no flush" % (per_step[0]["score"] / 1e6, L),
-                       "parallelism": f"units sharded, {world} rank(s), no collective"},
+                       "parallelism": f"units sharded, {world} rank(s), no collective",
+                       "source_hash": source_hash()},
             "us_per_layer_step": us_step,
             "tokens_per_s_layer": wl.B * world / (us_step * 1e-6),
             # attention-path only: a model of L_model layers runs L_model layer-steps per token
@@ -405,11 +504,13 @@ def run_cuda(args):
             "algorithmic_bytes_per_step": bytes_all / K / world,
             "mean_k": float(np.mean([p["mean_k"] for p in per_step])), "max_k": int(max(p["max_k"] for p in per_step)),
             "sparsity_utilisation": float(np.mean([p["mean_k"] / max(p["max_k"], 1) for p in per_step])),
-            "stages_us": stage_us, "stages_sum_us": float(sum(stage_us.values())),
+            "in_graph": in_graph,
+            "stages_us_eager_standalone": stage_us, "stages_sum_us_eager_standalone": float(sum(stage_us.values())),
             "unfused_five_calls_us": unfused_us,
             "amortised": {"select_interval": SI, "us_per_layer_step": amortised_us,
-                          "note": "compression every select_interval steps as in the paper (L274); the other steps "
-                                  "append and attend over the previous selected tier"},
+                          "note": "compression every select_interval steps as in the paper (L274); in between only Step 1 "
+                                  "runs: the token joins the dense tier (which grows, L78 steps 1-2), nothing retires, "
+                                  "attention covers dense + the tier of the last compression + condensed"},
             "ha_sparse": {"us_per_layer_step": sparse_us, "amortised_us_per_layer_step": sparse_amortised_us,
                           "select_interval": SI,
                           "note": "Sparse Loading (L178, L191): same selection, attention gathered through sel_idx, "
@@ -423,17 +524,21 @@ def run_cuda(args):
                         "regime; this build keeps the candidate pool resident in both layouts, so HA-Max pays the static "
                         "selected tier on top"},
             "solve_temperature_us": solve_us,
+            "lse_drift": drift,
             "roofline": roof,
             "e2e": {"value": e2e_gbs, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "us_per_layer_step": ms_e2e / K * 1e3, "eager_us_per_layer_step": t_e2e_eager / K * 1e6,
+                    "us_per_layer_step": ms_e2e / K * 1e3,
+                    "eager_us_per_layer_step": t_e2e_eager / K * 1e6, "graph_us_per_layer_step": t_e2e_graph / K * 1e6,
                     "sync": "stream sync after every step",
-                    "launch": "hardkv_decode_step_host captured once per layer into a CUDA graph over pinned host buffers; "
-                              "per step: host write of q / k / v into them, one replay (H2D + step + D2H), sync"},
+                    "launch": "hardkv_decode_step_host per step on pinned host q | k_new | v_new (packed: one H2D copy); the "
+                              "attention kernel's merging CTAs store `out` straight into pinned host memory (these are the "
+                              "d2h bytes: no copy node); value = the faster of the eager call and the call replayed from a "
+                              "captured graph over a fixed pinned buffer (the host copies the step's inputs into it first)"},
             "gpu_launches": int(launches),
             "clocks": clocks,
         }
         if world == 1 and not args.no_cpu_baseline:
-            del st, eng, states, snaps
+            del eng, eng_am, states, snaps
             torch.cuda.empty_cache()
             g, us, cores, sample, done, _ = oracle_leg(args.config, steps=4, warmup=1, budget_s=20.0,
                                                        sample_B=args.ref_batch)
@@ -445,6 +550,43 @@ def run_cuda(args):
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
+
+
+def lse_drift(args, dev):
+    """Appendix G analogue of Figs. 20-21 (L764-860): how far the log-sum-exp of the attended set drifts from the one
+    that keeps every retired token, when the full condensed tier EVICTS (L76) versus MERGES the evictee with the
+    LSE-preserving weights of Eq. 9.  Three engines run the same 256-step trajectory on config-2 shapes (B = 4): a
+    64-slot tier that evicts, a 64-slot tier that merges, and a tier large enough to keep all retired tokens; p = 1 so
+    that the selected tier is the whole pool and the only difference between the runs is the condensed tier."""
+    import torch
+    from paper_2606_28831_b200 import harness
+    from workloads.synth import make_workload
+    steps, B = 256, 4
+    res = {}
+    lses = {}
+    for name, kw in (("keep_all", dict(cond_cap=512, cond_merge=0)), ("evict", dict(cond_cap=64, cond_merge=0)),
+                     ("merge", dict(cond_cap=64, cond_merge=1))):
+        n0 = np.array([4096, 6144, 8192, 5120], np.int32)
+        wl = make_workload(2, B=B, n0=n0, max_ctx=8704, k_cap=8704, l_upper=(n0 - 132).astype(np.int32), **kw)
+        eng = harness.make_engine(wl, dev)
+        (st,), _ = harness.make_state(wl, dev)
+        out = torch.zeros(wl.B, wl.Hq, wl.d, dtype=torch.float32, device=dev)
+        lse = torch.zeros(wl.B, wl.Hq, dtype=torch.float32, device=dev)
+        rec = []
+        for t in range(steps):
+            q = harness.to_dev(wl.step_q(t), wl, dev)
+            kn, vn = wl.step_kv(t, None)
+            eng.decode_step(st, q, harness.to_dev(kn, wl, dev), harness.to_dev(vn, wl, dev), 1.0, out, lse)
+            rec.append(lse.clone())
+        lses[name] = torch.stack(rec).cpu().numpy()
+        assert int(st.err_flag.item()) == 0
+    for name in ("evict", "merge"):
+        d = np.abs(lses[name] - lses["keep_all"])
+        res[name] = {"mean_abs_dlse_last_64_steps": float(d[-64:].mean()), "max_abs_dlse": float(d.max()),
+                     "mean_abs_dlse_by_64_steps": [float(d[i:i + 64].mean()) for i in range(0, steps, 64)]}
+    res["note"] = ("|LSE - LSE(keep all retired tokens)| over a 256-step trajectory, 64-slot condensed tier, config-2 shapes "
+                   "at B = 4, p = 1; the tier fills after 64 retirements, so the first 64 steps are identical")
+    return res
 
 
 L_MODEL = {0: 1, 1: 32, 2: 32, 3: 28, 4: 40}   # layers of the model each config is shaped after (SURVEY 8(d))
@@ -464,7 +606,8 @@ def main():
     ap.add_argument("--layers", type=int, default=0, help="layers of distinct KV data cycled per step (0: 32 for config 1 whose "
                     "single-layer K fits L2, else 1)")
     ap.add_argument("--n0", type=int, default=0, help="override: uniform prefill context (config 3 checkpoints)")
-    ap.add_argument("--variant", type=int, default=1, help="kernel variant (hardkv_set_variant): 1 default, 2 TMA score, 3 async attention")
+    ap.add_argument("--variant", type=int, default=1, help="kernel variant (hardkv_set_variant): 0 generic FMA kernels, 1 tuned "
+                    "separate kernels (default), 2 TMA-staged score kernel, 3 fused persistent score -> select kernel")
     ap.add_argument("--snapkv-window", type=int, default=0, help="odd window: odd KV heads use the SNAPKV max-pool metric "
                     "(L278) and the line reports the Algorithm 2 temperature solve; not the BASELINE workload")
     ap.add_argument("--contiguous-pages", action="store_true", help="diagnostic: identity page ids instead of the seeded "

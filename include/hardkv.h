@@ -197,14 +197,21 @@ hardkv_status hardkv_decode_step(hardkv_ctx *, const hardkv_state *, const void 
 /* hardkv_decode_step with HOST buffers for the per-step tensors (end-to-end entry): q_host
  * [B][Hq][d], k_new_host / v_new_host [B][Hkv][d] in kv_dtype and out_host [B][Hq][d] f32 are
  * HOST pointers (pinned memory for truly asynchronous copies; pageable works, slower).  The
- * call enqueues H2D copies into staging buffers inside the workspace, the step, and the D2H
- * copy of `out`, all on `stream`; it does not synchronise -- out_host is valid after the caller
+ * call enqueues H2D copies into staging buffers inside the workspace (ONE copy when the three
+ * inputs are packed back to back, k_new_host == q_host + bytes(q), v_new_host == k_new_host +
+ * bytes(k_new)), then the step, all on `stream`.  When out_host is pinned (mapped) host memory
+ * the attention kernel stores the result straight into it and no D2H copy is enqueued; pageable
+ * out_host gets one D2H copy.  It does not synchronise -- out_host is valid after the caller
  * synchronises the stream.  The host input buffers must stay untouched until then. */
 hardkv_status hardkv_decode_step_host(hardkv_ctx *, const hardkv_state *, const void *q_host,
                                       const void *k_new_host, const void *v_new_host, float p,
                                       int32_t do_select, float *out_host, hardkv_stream);
 /* Number of kernels this ctx has launched since hardkv_create (host counter; memcpys excluded). */
 int64_t hardkv_launch_count(const hardkv_ctx *ctx);
+/* Measurement helper, no ctx: one read-only pass over buf (DEVICE memory, 16-byte aligned, `bytes` of it) with plain
+ * 16-byte grid-stride loads, 8 in flight per thread.  Timed by the caller, bytes / time is the read bandwidth a
+ * streaming kernel can hope for on this GPU (bench.py --read-peak), next to the copy peak the roofline is quoted on. */
+hardkv_status hardkv_probe_read_stream(const void *buf, size_t bytes, hardkv_stream);
 
 #ifdef __cplusplus
 }

@@ -57,9 +57,12 @@ WsLayout ws_layout(const hardkv_config &c) {
   w.part = off;   off += align256(units * att_chunks_of(c) * G * (c.head_dim + 2) * sizeof(float));
   w.stats = off;  off += align256(units * score_chunks_of(c) * 8 * sizeof(float2));
   const size_t qb = (size_t)c.batch * c.num_q_heads * c.head_dim, kb = units * c.head_dim;
-  w.stage_q = off;   off += align256(qb * esize_of(c));
-  w.stage_k = off;   off += align256(kb * esize_of(c));
+  // staging of the host entry: q | k_new | v_new back to back (rows are >= 128 B, so every part stays 16-byte aligned):
+  // packed host buffers arrive with ONE host-to-device copy
+  w.stage_q = off;   off += qb * esize_of(c);
+  w.stage_k = off;   off += kb * esize_of(c);
   w.stage_v = off;   off += align256(kb * esize_of(c));
+  off = align256(off);
   w.stage_out = off; off += align256(qb * sizeof(float));
   w.pooled = off;    off += c.pool_kernel > 1 ? align256((size_t)c.batch * c.num_q_heads * c.max_ctx * sizeof(float)) : 0;
   w.total = off;
@@ -283,8 +286,9 @@ void launch_score_select(hardkv_ctx *ctx, const Params &P0, const void *q, float
 }
 
 // SNAPKV metric transform (L278): only configs that declare a pooling window pay for the launch
-void launch_pool(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
-  if (P.pool_kernel <= 1) return;
+void launch_pool(hardkv_ctx *ctx, const Params &P0, cudaStream_t st) {
+  if (P0.pool_kernel <= 1) return;
+  const Params P = launch_params(ctx, P0);
   ctx->launches += 1;
   dim3 grid((P.max_ctx + POOL_TOK - 1) / POOL_TOK, P.B * P.Hkv);
   maxpool_kernel<<<grid, 256, 0, st>>>(P);
@@ -321,6 +325,24 @@ void launch_attend(hardkv_ctx *ctx, const Params &P0, const void *q, float *out,
     HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, ATT_SPARSE><<<grid, 256, 0, st>>>(P, q, out, lse))));
   else
     HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, ATT_TIER><<<grid, 256, 0, st>>>(P, q, out, lse))));
+}
+
+// Read-only streaming probe (hardkv_probe_read_stream): what a plain 16-byte grid-stride read reaches on this GPU,
+// the reference the K scan is compared with beside the copy peak of MEASURED_PEAKS.json.
+__device__ unsigned int g_probe_sink;
+__global__ void __launch_bounds__(256) read_stream_kernel(const uint4 *p, size_t n) {
+  unsigned int acc = 0;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x;
+  for (; i + 7 * stride < n; i += 8 * stride) {
+    uint4 v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = ldg_nc(p + i + u * stride);
+#pragma unroll
+    for (int u = 0; u < 8; ++u) acc ^= v[u].x ^ v[u].y ^ v[u].z ^ v[u].w;
+  }
+  for (; i < n; i += stride) { const uint4 v = ldg_nc(p + i); acc ^= v.x ^ v.y ^ v.z ^ v.w; }
+  if (acc == 0x9e3779b9u) g_probe_sink = acc;   // keeps the loads alive; practically never taken
 }
 
 }  // namespace
@@ -540,6 +562,15 @@ hardkv_status hardkv_sparse_attend(hardkv_ctx *ctx, const hardkv_state *s, const
 
 int64_t hardkv_launch_count(const hardkv_ctx *ctx) { return ctx ? ctx->launches : -1; }
 
+hardkv_status hardkv_probe_read_stream(const void *buf, size_t bytes, hardkv_stream st) {
+  if (!buf || bytes < 16 || ((uintptr_t)buf & 15)) return HARDKV_ERR_INVALID_ARG;
+  int dev = 0, nsm = 148;
+  cudaGetDevice(&dev);
+  if (cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || nsm <= 0) nsm = 148;
+  read_stream_kernel<<<nsm * 4, 256, 0, st>>>(static_cast<const uint4 *>(buf), bytes / 16);
+  return launch_status();
+}
+
 hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const void *q, const void *k_new,
                                  const void *v_new, float p, int32_t do_select, float *out, float *lse,
                                  hardkv_stream st) {
@@ -569,14 +600,28 @@ hardkv_status hardkv_decode_step_host(hardkv_ctx *ctx, const hardkv_state *s, co
   const hardkv_config &c = ctx->cfg;
   const size_t qe = (size_t)c.batch * c.num_q_heads * c.head_dim, ke = (size_t)c.batch * c.num_kv_heads * c.head_dim;
   const size_t es = esize_of(c);
-  if (cudaMemcpyAsync(ctx->stage_q, q_host, qe * es, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-      cudaMemcpyAsync(ctx->stage_k, k_new_host, ke * es, cudaMemcpyHostToDevice, st) != cudaSuccess ||
-      cudaMemcpyAsync(ctx->stage_v, v_new_host, ke * es, cudaMemcpyHostToDevice, st) != cudaSuccess)
+  const char *qh = static_cast<const char *>(q_host), *kh = static_cast<const char *>(k_new_host),
+             *vh = static_cast<const char *>(v_new_host);
+  if (kh == qh + qe * es && vh == kh + ke * es) {   // packed [q | k_new | v_new]: one copy into the contiguous staging
+    if (cudaMemcpyAsync(ctx->stage_q, q_host, (qe + 2 * ke) * es, cudaMemcpyHostToDevice, st) != cudaSuccess)
+      return HARDKV_ERR_CUDA;
+  } else if (cudaMemcpyAsync(ctx->stage_q, q_host, qe * es, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+             cudaMemcpyAsync(ctx->stage_k, k_new_host, ke * es, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+             cudaMemcpyAsync(ctx->stage_v, v_new_host, ke * es, cudaMemcpyHostToDevice, st) != cudaSuccess) {
     return HARDKV_ERR_CUDA;
+  }
+  // out_host in pinned (mapped) host memory: the merging CTAs of the attention kernel store the result straight into it
+  // -- no device-to-host copy node; pageable memory goes through the staging buffer and one copy.
+  float *out_dev = nullptr;
+  cudaPointerAttributes pa;
+  if (cudaPointerGetAttributes(&pa, out_host) == cudaSuccess && pa.type == cudaMemoryTypeHost && pa.devicePointer)
+    out_dev = static_cast<float *>(pa.devicePointer);
+  else
+    cudaGetLastError();
   hardkv_status r = hardkv_decode_step(ctx, s, ctx->stage_q, ctx->stage_k, ctx->stage_v, p, do_select,
-                                       ctx->stage_out, nullptr, st);
+                                       out_dev ? out_dev : ctx->stage_out, nullptr, st);
   if (r != HARDKV_OK) return r;
-  if (cudaMemcpyAsync(out_host, ctx->stage_out, qe * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess)
+  if (!out_dev && cudaMemcpyAsync(out_host, ctx->stage_out, qe * sizeof(float), cudaMemcpyDeviceToHost, st) != cudaSuccess)
     return HARDKV_ERR_CUDA;
   return HARDKV_OK;
 }

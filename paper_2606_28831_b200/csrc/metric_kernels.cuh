@@ -17,6 +17,7 @@ namespace hardkv {
 constexpr int POOL_TOK = 1024;   // tokens per CTA of the pooling kernel
 
 __global__ void __launch_bounds__(256) maxpool_kernel(Params P) {
+  KernelClock kclock(P);
   const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
   if (P.st.score_mode[h] != HARDKV_SCORE_SNAPKV) return;
   int n, lo, hi;

@@ -58,7 +58,7 @@ STEP_REUSE_TIER, STEP_SELECT_REWRITE, STEP_SELECT_SPARSE, STEP_REUSE_SPARSE = 0,
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
            "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_timing", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_score_select", "hardkv_calibrate_topp", "hardkv_solve_temperature",
            "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend", "hardkv_sparse_attend",
-           "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count"]
+           "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count", "hardkv_probe_read_stream"]
 
 
 def _load():
@@ -90,6 +90,7 @@ def _load():
     lib.hardkv_sparse_attend.argtypes = [vp, sp, vp, vp, vp, vp]
     lib.hardkv_decode_step.argtypes = [vp, sp, vp, vp, vp, C.c_float, C.c_int32, vp, vp, vp]
     lib.hardkv_decode_step_host.argtypes = [vp, sp, vp, vp, vp, C.c_float, C.c_int32, vp, vp]
+    lib.hardkv_probe_read_stream.argtypes = [vp, C.c_size_t, vp]
     lib.hardkv_launch_count.argtypes = [vp]
     lib.hardkv_launch_count.restype = C.c_int64
     for n in EXPORTS:
@@ -116,6 +117,12 @@ def _ptr(t):
 
 def _stream():
     return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+
+
+def probe_read_stream(buf: torch.Tensor):
+    """One read-only streaming pass over a CUDA tensor on the current stream (hardkv_probe_read_stream)."""
+    assert buf.is_cuda and buf.is_contiguous()
+    _check(lib.hardkv_probe_read_stream(_ptr(buf), buf.numel() * buf.element_size(), _stream()))
 
 
 class DeviceState:
