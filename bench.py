@@ -204,7 +204,11 @@ def run_cuda(args):
         over["cond_merge"] = 1
     if args.contiguous_pages:
         over["contiguous_pages"] = True
-    wl = sharding.rank_workload(args.config, rank, **over)   # every rank: its own batch of the same shape
+    if args.shard == "heads" and world > 1:
+        # width (tensor-parallel) sharding, L555-562: ONE batch, every rank takes Hkv / world KV heads of every sequence
+        wl = sharding.head_shard(sharding.rank_workload(args.config, 0, **over), rank, world)
+    else:
+        wl = sharding.rank_workload(args.config, rank, **over)   # every rank: its own batch of the same shape
     if args.p:
         wl.p = args.p
     L = args.layers or (32 if args.config == 1 else 1)
@@ -454,6 +458,11 @@ def run_cuda(args):
     # ---- (4) --cond-merge: LSE drift of the condensed tier, merging vs eviction vs keeping everything ---------------
     drift = lse_drift(args, dev) if (args.cond_merge and world == 1) else None
 
+    # ---- KV-head sharding: the one exchange of the deployment, a gather of the per-head counts (L562) --------------
+    head_counts = None
+    if args.shard == "heads" and world > 1:
+        head_counts = sharding.gather_head_counts(states[(W + K - 1) % L].sel_count.view(wl.B, wl.Hkv), world)
+
     # ---- reduce over ranks ------------------------------------------------------------------------
     ms_total, ms_e2e, bytes_all = sharding.reduce_run(ms_total, t_e2e * 1e3, bytes_total, dev)
 
@@ -481,7 +490,8 @@ def run_cuda(args):
         roof["frac_of_read_probe"] = roof["achieved"] / read_probe_gbs
         line = {
             "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-            "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_total / K, "higher_is_better": True,
+            "scaling": "strong" if (args.shard == "heads" and world > 1) else "weak", "vs_baseline": None,
             "dtype": "bf16" if wl.dtype == "bf16" else "f32", "data": "synthetic",
             "config": {"workload": f"BASELINE.json configs[{args.config}] ({wl.name})", "batch": wl.B,
                        "q_heads": wl.Hq, "kv_heads": wl.Hkv, "head_dim": wl.d, "ctx": [int(wl.n0.min()), int(wl.n0.max())],
@@ -491,7 +501,10 @@ def run_cuda(args):
                        "launch": "eager" if args.eager else "one CUDA graph of the K steps",
                        "l2": "inputs larger than L2 (K scan %.0f MB per layer-step x %d layer(s) of distinct data cycled), "
                              "no flush" % (per_step[0]["score"] / 1e6, L),
-                       "parallelism": f"units sharded, {world} rank(s), no collective",
+                       "parallelism": (f"KV heads sharded over {world} rank(s) (L555-562), one all-gather of the head counts "
+                                       f"after the run, gathered mean k {float(head_counts.float().mean()):.1f}"
+                                       if head_counts is not None else
+                                       f"sequences sharded, {world} rank(s), no collective"),
                        "source_hash": source_hash()},
             "us_per_layer_step": us_step,
             "tokens_per_s_layer": wl.B * world / (us_step * 1e-6),
@@ -614,6 +627,9 @@ def main():
                     "random block ids (L460); not the BASELINE workload")
     ap.add_argument("--cond-merge", action="store_true", help="condensed-tier evictees are merged (Appendix G) instead "
                     "of dropped; not the BASELINE workload")
+    ap.add_argument("--shard", default="sequences", choices=["sequences", "heads"], help="N > 1: every rank its own batch "
+                    "(weak scaling, default) or the KV heads of ONE batch split over the ranks (tensor parallel, L555-562; "
+                    "strong scaling) with the gather of head counts")
     ap.add_argument("--p", type=float, default=0.0, help="override the nucleus mass (config 4 sweep)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup

@@ -510,3 +510,74 @@ def test_cuda_graph_replay_widened_entries(P):
         for f in ("temperature", "sel_count", "sel_idx", "cond_k", "cond_pos", "votes", "ctx_len", "c_lo"):
             assert torch.equal(getattr(a.st, f), getattr(b.st, f)), (t, f)
         assert torch.equal(a.out, b.out) and torch.equal(a.lse, b.lse)
+
+
+def test_depth_one_graph_over_layers_with_shared_block_ids():
+    """Depth (Fig. 6: "head-independent indices ... regularized for all layers", so one block id
+    addresses the same block in every layer and kernel executions can be captured "throughout the model's depth"): four
+    layers of INDEPENDENTLY seeded KV data and inputs share one base_table / sel_pages, the four layer-steps of a decode
+    step are captured into ONE CUDA graph, and every layer is compared with its own oracle after every replay."""
+    import dataclasses
+    from gpu_common import DEV, Pair
+    from oracle.batch import OracleBatch
+    from paper_2606_28831_b200 import harness
+    Lyr = 4
+    wl = make_workload(2, B=3, n0=i32(900, 2300, 1500), max_ctx=2400, k_cap=256, l_upper=i32(900 - 132, 2300 - 132, 1500 - 132),
+                       cond_cap=24, steps=8)
+    seeds = [wl.seed + 7919 * (l + 1) for l in range(Lyr)]
+    wls = []
+    for sd in seeds:
+        w = dataclasses.replace(wl)
+        w.seed = sd
+        w.page_tables = wl.page_tables      # the block ids are the model's, not the layer's (L207-209)
+        wls.append(w)
+    eng = harness.make_engine(wl, DEV)
+    states, prefill = harness.make_state(wl, DEV, layers=Lyr, layer_seeds=seeds)
+    assert all(s.base_table.data_ptr() == states[0].base_table.data_ptr() and
+               s.sel_pages.data_ptr() == states[0].sel_pages.data_ptr() for s in states)      # block ids shared by all layers
+    assert len({s.k_pool.data_ptr() for s in states}) == Lyr                                  # distinct KV data per layer
+    pairs = []
+    for l in range(Lyr):      # a Pair-shaped view per layer: the shared engine, that layer's state and oracle
+        pr = Pair.__new__(Pair)
+        pr.wl, pr.eng, pr.st = wls[l], eng, states[l]
+        pr.prefill = {(b, h): prefill[(l, b, h)] for b in range(wl.B) for h in range(wl.Hkv)}
+        pr.ob = OracleBatch(wls[l], pr.prefill)
+        pr.out = torch.zeros(wl.B, wl.Hq, wl.d, dtype=torch.float32, device=DEV)
+        pr.lse = torch.zeros(wl.B, wl.Hq, dtype=torch.float32, device=DEV)
+        pr.last_p, pr.flips_total = wl.p, 0
+        pairs.append(pr)
+    assert not np.array_equal(pairs[0].prefill[(0, 0)][0], pairs[1].prefill[(0, 0)][0])
+    bufs = [tuple(x.clone() for x in pr.inputs(0)[3]) for pr in pairs]
+
+    def all_layers():
+        for pr, (qd, kd, vd) in zip(pairs, bufs):
+            eng.decode_step(pr.st, qd, kd, vd, wl.p, pr.out, pr.lse)
+
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    snaps = [harness.snapshot(st) for st in states]
+    with torch.cuda.stream(s):
+        all_layers()                                      # warm-up outside capture
+    torch.cuda.current_stream().wait_stream(s)
+    torch.cuda.synchronize()
+    for st, sn in zip(states, snaps):
+        harness.restore(st, sn)
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g):
+        all_layers()                                      # ONE graph over the depth of the model
+    for t in range(6):
+        hosts = []
+        for pr, (qd, kd, vd) in zip(pairs, bufs):
+            q, kn, vn, (q2, k2, v2) = pr.inputs(t)
+            qd.copy_(q2); kd.copy_(k2); vd.copy_(v2)
+            hosts.append((q, kn, vn))
+        g.replay()
+        for l, (pr, (q, kn, vn)) in enumerate(zip(pairs, hosts)):
+            pr.ob.step(q, kn, vn, wl.p)
+            pr.check_out(f"layer {l} step {t}")
+            if pr.check_selection_band() == 0:
+                pr.check_bookkeeping()
+                pr.check_rewrite_exact()
+                pr.check_votes()
+            pr.force_discrete_state()
+    assert not torch.equal(pairs[0].out, pairs[1].out)

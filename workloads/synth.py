@@ -72,6 +72,9 @@ class Workload:
     pool_kernel: int = 0             # SNAPKV max-pool window (odd; 0: no SNAPKV head)
     cond_merge: int = 0              # 1: condensed-tier evictees are merged (Appendix G) instead of dropped
     contiguous_pages: bool = False   # diagnostic: identity page ids instead of the seeded permutations (L460)
+    head_offset: int = 0             # KV-head (tensor-parallel) shard: this workload holds KV heads [head_offset,
+    Hkv_total: int = 0               # head_offset + Hkv) of a batch with Hkv_total heads (0: not a shard) -- same data
+                                     # per (sequence, head) as the unsharded workload
     seed: int = 0
     temperature: np.ndarray = field(default=None)  # [B][Hkv] calibration T (reading C10: 1)
 
@@ -95,9 +98,9 @@ class Workload:
     # ---- latent structure per (b, KV head) ---------------------------------------------
     def latent(self, b: int, h: int):
         """(q_bar[d], u_hat[d], tau): persistent query direction and logit temperature."""
-        key = ("latent", self.seed, b, h, self.d, self.tau_lo, self.tau_hi)
+        key = ("latent", self.seed, b, h, self.d, self.tau_lo, self.tau_hi, self.head_offset)
         if key not in self._memo:
-            g = _rng(self.seed, _T_LATENT, b, h)
+            g = _rng(self.seed, _T_LATENT, b, h + self.head_offset)
             qb = g.standard_normal(self.d).astype(np.float32)
             tau = np.float32(np.exp(g.uniform(np.log(self.tau_lo), np.log(self.tau_hi))))
             self._memo[key] = (qb, qb / np.linalg.norm(qb), tau)
@@ -105,7 +108,7 @@ class Workload:
 
     def _prefill_heavy_hitters(self, b: int, h: int) -> np.ndarray:
         """Positions of the planted heavy hitters of the prefill (memoised: a pure function of the seed and shape)."""
-        key = ("hh", self.seed, b, h, int(self.n0[b]), self.planted)
+        key = ("hh", self.seed, b, h, int(self.n0[b]), self.planted, self.head_offset)
         if key not in self._memo:
             self._memo[key] = np.flatnonzero(self.planted_mask(b, h, 0, int(self.n0[b])))
         return self._memo[key]
@@ -117,7 +120,7 @@ class Workload:
         out = np.empty(hi - lo, bool)
         blk = 4096
         for s in range(lo // blk, (hi + blk - 1) // blk):
-            m = _rng(self.seed, _T_PLANT, b, h, s).random(blk) < self.planted
+            m = _rng(self.seed, _T_PLANT, b, h + self.head_offset, s).random(blk) < self.planted
             a, e = max(lo, s * blk), min(hi, (s + 1) * blk)
             out[a - lo:e - lo] = m[a - s * blk:e - s * blk]
         return out
@@ -137,7 +140,7 @@ class Workload:
     def prefill_unit(self, b: int, h: int):
         """(K0, V0) float32 [n0[b]][d], already rounded to the workload dtype."""
         n = int(self.n0[b])
-        g = _rng(self.seed, _T_KV, b, h)
+        g = _rng(self.seed, _T_KV, b, h + self.head_offset)
         K = g.standard_normal((n, self.d), dtype=np.float32)
         V = g.standard_normal((n, self.d), dtype=np.float32)
         if self.structured:
@@ -150,7 +153,9 @@ class Workload:
     # ---- per-step inputs ---------------------------------------------------------------------
     def step_q(self, t: int) -> np.ndarray:
         """q [B][Hq][d] of decode step t (float32, rounded to the workload dtype)."""
-        eps = _rng(self.seed, _T_QEPS, t).standard_normal((self.B, self.Hq, self.d), dtype=np.float32)
+        ht = self.Hkv_total or self.Hkv          # a head shard draws the whole batch's stream and keeps its heads
+        eps = _rng(self.seed, _T_QEPS, t).standard_normal((self.B, ht * self.G, self.d), dtype=np.float32)
+        eps = np.ascontiguousarray(eps[:, self.head_offset * self.G:(self.head_offset + self.Hkv) * self.G])
         q = np.empty_like(eps)
         if self.structured:
             for b in range(self.B):
@@ -168,10 +173,11 @@ class Workload:
         """(k_new, v_new) [B][Hkv][d] appended at decode step t (position n0[b]+t).
 
         prefill_K: dict (b,h)->K0, needed only when mix_new_keys (config 3)."""
-        k = _rng(self.seed, _T_KNEW, t).standard_normal((self.B, self.Hkv, self.d), dtype=np.float32)
-        v = _rng(self.seed, _T_VNEW, t).standard_normal((self.B, self.Hkv, self.d), dtype=np.float32)
+        ht, h0 = self.Hkv_total or self.Hkv, self.head_offset
+        k = _rng(self.seed, _T_KNEW, t).standard_normal((self.B, ht, self.d), dtype=np.float32)[:, h0:h0 + self.Hkv].copy()
+        v = _rng(self.seed, _T_VNEW, t).standard_normal((self.B, ht, self.d), dtype=np.float32)[:, h0:h0 + self.Hkv].copy()
         if self.structured:
-            mixr = _rng(self.seed, _T_MIX, t).random((self.B, self.Hkv))
+            mixr = _rng(self.seed, _T_MIX, t).random((self.B, ht))[:, h0:h0 + self.Hkv]
             for b in range(self.B):
                 pos = int(self.n0[b]) + t
                 for h in range(self.Hkv):
@@ -193,7 +199,7 @@ class Workload:
         if self.contiguous_pages:
             return (np.arange(nb, dtype=np.int32).reshape(self.B, self.Hkv, self.pages_per_unit),
                     np.arange(ns, dtype=np.int32).reshape(self.B, self.Hkv, self.sel_pages_per_unit))
-        g = _rng(self.seed, _T_PAGES)
+        g = _rng(self.seed, _T_PAGES, self.head_offset) if self.head_offset else _rng(self.seed, _T_PAGES)
         base = g.permutation(nb).astype(np.int32).reshape(self.B, self.Hkv, self.pages_per_unit)
         sel = g.permutation(ns).astype(np.int32).reshape(self.B, self.Hkv, self.sel_pages_per_unit)
         return base, sel
