@@ -176,6 +176,43 @@ static void hko_metric_probs(const hko_config *c, const hko_unit *u, int mode, d
   free(zh);
 }
 
+/* ---- query cache (L448: "for decoding-time KV cache compression, we store the query cache in a sliding
+ * window"): the queries of the last accum_window decode steps of this head's GQA group. */
+void hko_qcache_push(const hko_config *c, hko_unit *u, const float *q) {
+  if (!u->qcache || c->accum_window <= 0) return;
+  memcpy(u->qcache + (size_t)u->qc_slot * c->G * c->d, q, sizeof(float) * (size_t)c->G * c->d);
+  u->qc_slot = (u->qc_slot + 1) % c->accum_window;
+  if (u->qc_count < c->accum_window) u->qc_count += 1;
+}
+
+/* ---- accumulated attention recomputed from the query cache (reading C18; "vanilla attention averaging in
+ * H2O" is an order-preserving g, Solution 1, L122-124): every cached query scores the CURRENT pool,
+ *   A(i) = sum over cached steps tau, heads g of softmax_i(sm_scale q_{tau,g} . k_i / T) / G,   P_hat = A / sum_i A,
+ * plain loops: one logit row per (tau, g), its softmax over the pool, added up in fp64, rounded once. */
+static void hko_calibrate_qcache(const hko_config *c, hko_unit *u) {
+  int32_t lo = u->c_lo, hi = pool_hi(c, u), N = hi - lo;
+  double *A = (double *)calloc((size_t)N, sizeof(double));
+  double *z = (double *)malloc(sizeof(double) * (size_t)N);
+  for (int32_t tau = 0; tau < u->qc_count; ++tau) {
+    for (int32_t g = 0; g < c->G; ++g) {
+      const float *q = u->qcache + ((size_t)tau * c->G + g) * c->d;
+      double m = -INFINITY, s = 0.0;
+      for (int32_t i = 0; i < N; ++i) {
+        double dot = 0.0;
+        for (int32_t e = 0; e < c->d; ++e) dot += (double)q[e] * (double)u->K[(size_t)(lo + i) * c->d + e];
+        z[i] = (double)c->sm_scale * dot / (double)u->T;
+        if (z[i] > m) m = z[i];
+      }
+      for (int32_t i = 0; i < N; ++i) s += exp(z[i] - m);
+      for (int32_t i = 0; i < N; ++i) A[i] += exp(z[i] - m) / s / (double)c->G;
+    }
+  }
+  double tot = 0.0;
+  for (int32_t i = 0; i < N; ++i) tot += A[i];
+  for (int32_t i = 0; i < N; ++i) u->probs[lo + i] = tot > 0.0 ? (float)(A[i] / tot) : 0.0f;
+  free(A); free(z);
+}
+
 /* ---- Logits Calibration, apply-T (L120 "S_hat = S(g(z/T))", g = identity for
  * VANILLA L276, sequence max-pool for SNAPKV L278; H2O-style averaging L124 for
  * ACCUM, reading C4).  One score per KV head = mean over the GQA group of
@@ -184,6 +221,7 @@ static void hko_metric_probs(const hko_config *c, const hko_unit *u, int mode, d
 void hko_calibrate(const hko_config *c, hko_unit *u) {
   int32_t lo = u->c_lo, hi = pool_hi(c, u);
   if (hi <= lo) return;
+  if (u->score_mode == 3) { hko_calibrate_qcache(c, u); return; }
   double *P = (double *)calloc((size_t)(hi - lo), sizeof(double));
   hko_metric_probs(c, u, u->score_mode, (double)u->T, P);
 
@@ -321,7 +359,7 @@ int hko_solve_temperature(const hko_config *c, hko_unit *u, float p, float t_min
                           float eps, int max_iter, double *resid) {
   int32_t lo = u->c_lo, hi = pool_hi(c, u), N = hi - lo;
   if (resid) *resid = 0.0;
-  if (N <= 0 || u->score_mode == 1) return 0;
+  if (N <= 0 || u->score_mode == 1 || u->score_mode == 3) return 0;   /* accumulated metrics keep their T (C4, C18) */
   double *P = (double *)malloc(sizeof(double) * (size_t)N);
   /* line 1: k from the raw attention scores; the k_cap clamp and l_lower do not apply */
   hko_metric_probs(c, u, 0, 1.0, P);
@@ -443,6 +481,7 @@ void hko_attend(const hko_config *c, hko_unit *u, const float *q) {
 void hko_decode_step(const hko_config *c, hko_unit *u, const float *q,
                      const float *k_new, const float *v_new, float p, int do_select) {
   hko_append(c, u, k_new, v_new);
+  hko_qcache_push(c, u, q);     /* the window slides on every decode step, compression or not (L448) */
   if (do_select) {
     hko_retire_q(c, u, q);      /* Step 4 belongs to the compression step; it also re-anchors dense_lo */
     hko_score(c, u, q);

@@ -22,7 +22,8 @@
  * P6 order/temperature invariance, P7 Gaussian budget law, P8 merge algebra,
  * P9 rewrite copies, P10 condensed tier == top-C_cap of the retirement log,
  * P11 bookkeeping invariants, P12 integer mass vs fp64 cumsum, P13 temperature
- * solve (g = id => T* = 1; g = a z => T* = a; M_k decreasing in T), P14 SNAPKV
+ * solve (g = id => T* = 1; g = a z => T* = a; M_k decreasing in T), P17 query-cache
+ * ACCUM (static pool => equals the ring-sum form; library softmax), P14 SNAPKV
  * max-pool == torch.nn.functional.max_pool1d, P15 weighted merging (Eq. 9 weights ==
  * torch.softmax of the pair, SE_evict <= SE_merge <= SE_keep, Thm G.1 limit).
  * Parity unpinned by the paper: readings C2 (GQA group mean), C3 (softmax over
@@ -67,7 +68,8 @@ typedef struct {
   float   *cond_k, *cond_v;    /* [cond_cap][d] condensed tier rows                 */
   int32_t *cond_pos, *cond_votes; /* [cond_cap]                                     */
   int32_t  cond_count;
-  int32_t  score_mode;         /* 0 RAW, 1 ACCUM, 2 SNAPKV (max-pooled logits, L278) */
+  int32_t  score_mode;         /* 0 RAW, 1 ACCUM (ring of per-step rows), 2 SNAPKV (max-pooled logits, L278),
+                                  3 ACCUM recomputed from the query cache (L448, reading C18)            */
   float    T;                  /* calibration temperature of this KV head           */
   float   *acc;                /* [max_ctx] ACCUM running window sum (or NULL)      */
   float   *ring;               /* [accum_window][max_ctx] (or NULL)                 */
@@ -82,6 +84,9 @@ typedef struct {
   float   *sel_k, *sel_v;      /* [k_cap][d] rewritten tier rows                    */
   float   *out;                /* [G][d]                                            */
   float   *lse;                /* [G]                                               */
+  /* --- query cache: "we store the query cache in a sliding window" (L448) -------- */
+  float   *qcache;             /* [accum_window][G][d] queries of the last steps (or NULL) */
+  int32_t  qc_count, qc_slot;  /* valid entries (<= accum_window), next slot to overwrite  */
 } hko_unit;
 
 /* Step 1 of PAPER.md L78: append one (k,v) row at position n; n <- n+1. */
@@ -91,6 +96,8 @@ int  hko_retire(const hko_config *c, hko_unit *u);
 /* The same with the step's queries q [G][d]: when c->cond_merge, the evictee of a full tier is folded into the
  * highest-scoring resident with the LSE-preserving weights of Appendix G (Eq. 9; reading C17). */
 int  hko_retire_q(const hko_config *c, hko_unit *u, const float *q);
+/* Slides the step's queries q [G][d] into the query cache (L448); a no-op when u->qcache is NULL. */
+void hko_qcache_push(const hko_config *c, hko_unit *u, const float *q);
 /* z[g][i] = sm_scale * q_g . k_i over the pool (Eq. 4 exponent, reading C1). */
 void hko_score(const hko_config *c, hko_unit *u, const float *q);
 /* Logits Calibration, apply-T form (L120 Solution 1), group mean (reading C2). */

@@ -53,6 +53,7 @@ class HkoUnit(C.Structure):
         ("logits", _F), ("probs", _F),
         ("sel_idx", _I), ("sel_count", C.c_int32), ("k_topp", C.c_int32), ("tau_bits", C.c_uint32),
         ("sel_k", _F), ("sel_v", _F), ("out", _F), ("lse", _F),
+        ("qcache", _F), ("qc_count", C.c_int32), ("qc_slot", C.c_int32),
     ]
 
 
@@ -70,6 +71,8 @@ def lib():
         _lib.hko_retire_q.argtypes = [cp, up, _F]
         _lib.hko_retire_q.restype = C.c_int
         _lib.hko_score.argtypes = [cp, up, _F]
+        _lib.hko_qcache_push.argtypes = [cp, up, _F]
+        _lib.hko_qcache_push.restype = None
         _lib.hko_calibrate.argtypes = [cp, up]
         _lib.hko_solve_temperature.argtypes = [cp, up, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int,
                                                C.POINTER(C.c_double)]
@@ -165,6 +168,10 @@ class Unit:
         u.logits, u.probs = _fp(self.logits), _fp(self.probs)
         u.sel_idx, u.sel_count, u.k_topp, u.tau_bits = _ip(self.sel_idx), 0, 0, 0
         u.sel_k, u.sel_v, u.out, u.lse = _fp(self.sel_k), _fp(self.sel_v), _fp(self.out), _fp(self.lse)
+        self.qcache = np.zeros((max(cfg.accum_window, 1), cfg.G, d), np.float32) if score_mode == 3 else None
+        if score_mode == 3:
+            u.qcache = _fp(self.qcache)
+        u.qc_count, u.qc_slot = 0, 0
 
     # --- scalars -------------------------------------------------------------------
     n = property(lambda s: s.u.n)
@@ -189,6 +196,9 @@ class Unit:
 
     def retire_q(self, q) -> int:
         return lib().hko_retire_q(C.byref(self.ccfg), C.byref(self.u), _fp(_f32(q)))
+
+    def qcache_push(self, q):
+        lib().hko_qcache_push(C.byref(self.ccfg), C.byref(self.u), _fp(_f32(q)))
 
     def score(self, q):
         lib().hko_score(C.byref(self.ccfg), C.byref(self.u), _fp(_f32(q)))
@@ -243,7 +253,7 @@ def decode_step_batch(units: list[Unit], q: np.ndarray, k_new: np.ndarray, v_new
     nt = lib().hko_decode_step_batch(C.byref(units[0].ccfg), arr, len(units), _fp(q), _fp(k_new), _fp(v_new),
                                      np.float32(p), int(do_select))
     for u, cu in zip(units, arr):   # copy the scalar fields back (arrays are shared by pointer)
-        for f in ("n", "c_lo", "dense_lo", "cond_count", "ring_slot", "sel_count", "k_topp", "tau_bits"):
+        for f in ("n", "c_lo", "dense_lo", "cond_count", "ring_slot", "qc_count", "qc_slot", "sel_count", "k_topp", "tau_bits"):
             setattr(u.u, f, getattr(cu, f))
     return nt
 

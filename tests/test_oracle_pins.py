@@ -638,3 +638,46 @@ def test_p16_reuse_steps_partition_the_live_tokens(interval, p):
         x = (qt @ Kt[0].T) / math.sqrt(d)
         np.testing.assert_allclose(u.lse, torch.logsumexp(x, -1).numpy(), atol=1e-5, rtol=0)
     assert p == 1.0 or u.cond_count > 0     # the deferred retirements did happen at the compression steps
+
+
+# ---- P17: accumulated attention recomputed from the query cache (L448, L122-124; reading C18) ---------------------
+def test_p17_qcache_accum_equals_ring_sum_on_a_static_pool_and_library_softmax():
+    """score_mode 3 scores the CURRENT pool with every query of the sliding window.  (a) While the pool does not change,
+    that is the sum of the window's per-step rows -- the ring-sum ACCUM form already pinned by
+    test_accum_is_sliding_window_sum -- so both modes must give the same normalised row, before and after the window
+    wraps.  (b) Independently: the row equals the mean over (cached step, head) of scipy softmax rows of numpy logits.
+    (c) When the pool does change the two forms differ (old rows were normalised over old pools): the recomputed one is
+    still the library softmax mean over the NEW pool."""
+    w, G, d = 4, 3, 64
+    rng = np.random.default_rng(11)
+    cfg = OracleConfig(G=G, d=d, max_ctx=160, sink=2, recent=8, k_cap=160, cond_cap=4, accum_window=w)
+    K0, V0 = rng.standard_normal((90, d)).astype(np.float32), rng.standard_normal((90, d)).astype(np.float32)
+    ring, qc = Unit(cfg, K0, V0, l_upper=10**6, T=0.7, score_mode=1), Unit(cfg, K0, V0, l_upper=10**6, T=0.7, score_mode=3)
+    lo, hi = qc.pool
+    qs = []
+    for t in range(7):                                    # static pool: no append; the window wraps at t = 4
+        q = (rng.standard_normal((G, d)) * 1.3).astype(np.float32)
+        qs.append(q)
+        ring.score(q); ring.calibrate()
+        qc.qcache_push(q); qc.calibrate()
+        np.testing.assert_allclose(qc.probs[lo:hi], ring.probs[lo:hi], rtol=3e-6, atol=1e-12)
+        win = qs[-w:]
+        z = np.stack([(np.float64(cfg.c().sm_scale) * (qq.astype(np.float64) @ K0[lo:hi].astype(np.float64).T)) / np.float64(np.float32(0.7))
+                      for qq in win])                     # [steps][G][N]
+        ref = scipy.special.softmax(z, axis=2).mean(axis=(0, 1))
+        np.testing.assert_allclose(qc.probs[lo:hi], ref / ref.sum(), rtol=2e-7, atol=0)
+        assert abs(qc.probs[lo:hi].astype(np.float64).sum() - 1) < 1e-5
+    # (c) the pool moves: decode steps append tokens; the recomputed metric follows the library form on the new pool
+    for t in range(3):
+        q = (rng.standard_normal((G, d)) * 1.3).astype(np.float32)
+        qs.append(q)
+        kn, vn = rng.standard_normal(d).astype(np.float32), rng.standard_normal(d).astype(np.float32)
+        qc.decode_step(q, kn, vn, p=0.9)
+        ring.decode_step(q, kn, vn, p=0.9)
+        lo, hi = qc.pool
+        z = np.stack([(np.float64(cfg.c().sm_scale) * (qq.astype(np.float64) @ qc.K[lo:hi].astype(np.float64).T)) / np.float64(np.float32(0.7))
+                      for qq in qs[-w:]])
+        ref = scipy.special.softmax(z, axis=2).mean(axis=(0, 1))
+        np.testing.assert_allclose(qc.probs[lo:hi], ref / ref.sum(), rtol=2e-7, atol=0)
+    assert not np.allclose(qc.probs[lo:hi], ring.probs[lo:hi], rtol=1e-4)
+    assert qc.u.qc_count == w and qc.u.qc_slot == (7 + 3) % w
