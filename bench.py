@@ -202,6 +202,12 @@ def run_cuda(args):
         over["pool_kernel"] = args.snapkv_window
     if args.cond_merge:
         over["cond_merge"] = 1
+    if args.accum_recompute:      # accumulated-attention heads on the query-cache form (L448) instead of the ring of rows
+        sm = sharding.rank_workload(args.config, 0).score_mode.copy()
+        sm[sm == 1] = 3
+        if not (sm == 3).any():
+            sm[len(sm) // 2:] = 3
+        over["score_mode"] = sm
     if args.contiguous_pages:
         over["contiguous_pages"] = True
     if args.shard == "heads" and world > 1:
@@ -306,7 +312,11 @@ def run_cuda(args):
     per_launch = launches // K
     NAMES = {4: ["append_retire", "score", "calibrate_topp", "rewrite_attend"],
              3: ["append_retire", "score_select", "rewrite_attend"],
-             5: ["append_retire", "score", "maxpool", "calibrate_topp", "rewrite_attend"]}.get(per_launch)
+             5: ["append_retire", "score", "maxpool", "calibrate_topp", "rewrite_attend"],
+             8: ["append_retire", "qcache_push", "score", "qcache_stats", "qcache_reduce", "qcache_accum", "calibrate_topp",
+                 "rewrite_attend"]}.get(per_launch)
+    if per_launch == 8:      # qcache_push takes no timing slot
+        NAMES.remove("qcache_push")
     in_graph = None
     if NAMES and not args.eager:
         slots = torch.empty(launches, 2, dtype=torch.int64, device=dev)
@@ -321,7 +331,8 @@ def run_cuda(args):
         torch.cuda.synchronize()
         g2.replay()
         torch.cuda.synchronize()
-        ts = slots.cpu().numpy().reshape(K, per_launch, 2).astype(np.float64)
+        per_launch = len(NAMES)
+        ts = slots.cpu().numpy()[:K * per_launch].reshape(K, per_launch, 2).astype(np.float64)
         dur = (ts[:, :, 1] - ts[:, :, 0]) / 1e3                                # [K][kernels] us
         gaps = (ts[:, 1:, 0] - ts[:, :-1, 1]) / 1e3                            # idle between consecutive kernels of a step
         step_gap = (ts[1:, 0, 0] - ts[:-1, -1, 1]) / 1e3                       # idle between steps
@@ -361,7 +372,10 @@ def run_cuda(args):
                    "score_select": float(np.mean([p["score"] for p in per_step])),
                    "rewrite_attend": float(np.mean([p["attend"] + p["rewrite_write"] for p in per_step])),
                    "calibrate_topp": float(np.mean([p["select_bytes"] for p in per_step])),
-                   "append_retire": 0.0, "maxpool": 0.0}
+                   "append_retire": 0.0, "maxpool": 0.0, "qcache_reduce": 0.0,
+                   # the query-cache passes stream the pool of the QCACHE heads once each
+                   "qcache_stats": float(np.mean([p["score"] for p in per_step])) * float((wl.score_mode == 3).mean()),
+                   "qcache_accum": float(np.mean([p["score"] for p in per_step])) * float((wl.score_mode == 3).mean())}
 
     # ---- (2b) context lines: the unfused five-call pipeline, and the paper's amortised regime (L274) ------------
     def timed_loop(body, e=None):
@@ -473,7 +487,8 @@ def run_cuda(args):
         us_step = ms_total / K * 1e3
         times = in_graph["kernels_us"] if in_graph else stage_us
         dom = max(times, key=lambda s_: times[s_])
-        plain = not (args.n0 or args.p or args.snapkv_window or args.cond_merge or args.contiguous_pages or args.layers)
+        plain = not (args.n0 or args.p or args.snapkv_window or args.cond_merge or args.contiguous_pages or args.layers
+                     or args.accum_recompute)
         traffic, traffic_from = profiled_traffic(args.config, args.variant, dom) if plain else (None, None)
         roof = {"kernel": dom, "bound": "hbm", "unit": "GB/s", "peak": peak, "peak_source": peak_src,
                 "achieved": bytes_stage[dom] / (times[dom] * 1e-6) / 1e9,
@@ -497,6 +512,7 @@ def run_cuda(args):
                        "q_heads": wl.Hq, "kv_heads": wl.Hkv, "head_dim": wl.d, "ctx": [int(wl.n0.min()), int(wl.n0.max())],
                        "p": wl.p, "k_cap": wl.k_cap, "select_interval": 1, "layers": L, "variant": args.variant,
                        "snapkv_window": args.snapkv_window, "cond_merge": bool(args.cond_merge),
+                       "accum_recompute": bool(args.accum_recompute), "score_mode": wl.score_mode.tolist(),
                        "page_ids": "identity (diagnostic)" if args.contiguous_pages else "seeded permutation (random block ids, L460)",
                        "launch": "eager" if args.eager else "one CUDA graph of the K steps",
                        "l2": "inputs larger than L2 (K scan %.0f MB per layer-step x %d layer(s) of distinct data cycled), "
@@ -627,6 +643,9 @@ def main():
                     "random block ids (L460); not the BASELINE workload")
     ap.add_argument("--cond-merge", action="store_true", help="condensed-tier evictees are merged (Appendix G) instead "
                     "of dropped; not the BASELINE workload")
+    ap.add_argument("--accum-recompute", action="store_true", help="accumulated-attention heads recompute their metric from "
+                    "the 32-deep query cache (L448; a contraction with M = 32 G query rows) instead of the ring of rows; "
+                    "configs without such heads put the upper half of the KV heads on it; not the BASELINE workload")
     ap.add_argument("--shard", default="sequences", choices=["sequences", "heads"], help="N > 1: every rank its own batch "
                     "(weak scaling, default) or the KV heads of ONE batch split over the ranks (tensor parallel, L555-562; "
                     "strong scaling) with the gather of head counts")

@@ -60,7 +60,12 @@ typedef enum {
 typedef enum { HARDKV_F32 = 0, HARDKV_BF16 = 1 } hardkv_dtype;
 /* Importance metric of a KV head (L276-278): raw attention logits (VANILLA), accumulated attention over the
  * last accum_window steps (H2O-style, L124), or logits max-pooled along the sequence (SNAPKV, L150 / L278). */
-typedef enum { HARDKV_SCORE_RAW = 0, HARDKV_SCORE_ACCUM = 1, HARDKV_SCORE_SNAPKV = 2 } hardkv_score_mode;
+typedef enum {
+  HARDKV_SCORE_RAW = 0, HARDKV_SCORE_ACCUM = 1, HARDKV_SCORE_SNAPKV = 2,
+  /* accumulated attention RECOMPUTED from the sliding-window query cache (L448): every cached query of the last
+   * accum_window steps scores the current pool; the head's metric is the mean of their softmax rows (L122-124) */
+  HARDKV_SCORE_ACCUM_QCACHE = 3
+} hardkv_score_mode;
 
 /* Static for the lifetime of a ctx (and of any graph captured with it). */
 typedef struct {
@@ -95,6 +100,8 @@ typedef struct {
   uint8_t *sel_mask;                /* (opt) [B][Hkv][max_ctx/8], bit i%8 of byte i/8 (L439)                */
   float *logits, *probs;
   int32_t *err_flag;                /* one device int                                                    */
+  void *qcache;                     /* (opt) [B][Hq][accum_window][d] kv_dtype: the queries of the last steps (L448)         */
+  int32_t *qc_count, *qc_slot;      /* (opt) [B]: valid steps in the window, next slot; needed by SCORE_ACCUM_QCACHE heads    */
   int32_t *dense_lo;                /* [B] first position of the recent part of the dense tier: ctx_len - recent at the
                                        last compression step (written by the append stage of a compression step); the
                                        caller initialises it to max(min(sink, n), n - recent)                     */
@@ -141,7 +148,11 @@ hardkv_status hardkv_append_kv_merge(hardkv_ctx *, const hardkv_state *, const v
                                      const void *q, hardkv_stream);
 /* logits[b][h*G+g][i] = sm_scale * q . K[i] over the pool (exponent of Eq. 4). */
 hardkv_status hardkv_score(hardkv_ctx *, const hardkv_state *, const void *q, hardkv_stream);
-/* Logits Calibration (apply-T) -> probs, then hardkv_topp_select.  SNAPKV heads (cfg.pool_kernel > 1)
+/* Slides the step's queries q [B][Hq][d] into state->qcache (L448).  hardkv_decode_step does this itself on every
+ * step when state->qcache is set; the stage-by-stage caller does it once per decode step before hardkv_calibrate_topp. */
+hardkv_status hardkv_qcache_push(hardkv_ctx *, const hardkv_state *, const void *q, hardkv_stream);
+/* Logits Calibration (apply-T) -> probs, then hardkv_topp_select.  Heads in mode SCORE_ACCUM_QCACHE take their
+ * probabilities from two more passes over the pool with the cached queries (qcache_kernels.cuh) instead of the logits.  SNAPKV heads (cfg.pool_kernel > 1)
  * are calibrated on their logits max-pooled along the sequence, window clipped to the pool (L278). */
 hardkv_status hardkv_calibrate_topp(hardkv_ctx *, const hardkv_state *, float p, hardkv_stream);
 /* hardkv_score followed by hardkv_calibrate_topp as ONE call (stages 1 + 2a-2c; same results).  With

@@ -35,12 +35,16 @@ __device__ __forceinline__ float bf16_round(float x) { return __bfloat162float(_
 
 template <int D, int MODE>
 __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void *q_, float *out, float *lse) {
-  pdl_wait_then_trigger();
+  // wait_select: launched programmatically behind the select kernel; units come in the order their selections finish and
+  // every CTA waits for its own unit only (the stream predecessors of the select kernel are complete: it was launched
+  // with a full dependency on them)
+  if (P.wait_select) pdl_trigger(); else pdl_wait_then_trigger();
   KernelClock kclock(P);
   constexpr int NKC = D / 32;   // 64-byte chunks of a key row
   constexpr int NVC = D / 64;   // 128-byte chunks of a value row
   constexpr int ROWB = D * 2;
-  const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
+  const int unit = P.wait_select ? P.unit_order[blockIdx.y] : (int)blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
+  if (P.wait_select) wait_unit_selected(P, unit);
   const int n = P.st.ctx_len[b];
   int s_end, r_lo;
   if (!dense_bounds(P, b, n, s_end, r_lo)) {   // more reuse steps than cfg.reuse_max: flag, leave the unit untouched

@@ -33,6 +33,15 @@ struct Params {
   int ss_slice_cap;      // capacity (tokens) of the probability slice of one unit held by one 1024-thread CTA
   int32_t *ss_next;      // [1] next work item (zero between launches)
   int32_t *ss_arrive;    // [units] chunks of a unit scanned so far (zero between launches)
+  // select -> attention overlap (hardkv_decode_step with programmatic dependent launch)
+  int32_t *epoch;        // [1] decode steps appended so far: the append kernel bumps it, select publishes it per unit
+  int32_t *sel_flag;     // [units] == *epoch once the unit's selection of this step is complete and visible
+  int32_t *unit_order;   // [units] units by increasing pool length (the order their selections finish in)
+  int wait_select;       // attention launch: 1 = launched programmatically behind the select kernel: wait per unit
+  // query-cache form of the accumulated-attention metric (qcache_kernels.cuh)
+  float2 *qc_stats;      // [units][score_chunks][256] per chunk and query row: (max, sum 2^(x - max)) of x = z log2(e) / T
+  float2 *qc_final;      // [units][256] per query row: (max, 1 / (sum * G * n_c))
+  int st_esize;          // bytes of one q / K / V element
   // in-graph kernel timing (hardkv_set_timing): NULL in normal runs
   unsigned long long *timing;   // [2 * slots]: (start of the first CTA, end of the last CTA) in globaltimer ns per launch
   int timing_slot;
@@ -63,6 +72,25 @@ struct KernelClock {
 __device__ __forceinline__ void pdl_wait_then_trigger() {
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+}
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+// Consumer side of the select -> attention overlap: the attention kernel is launched programmatically behind the select
+// kernel (its CTAs take the SMs that select CTAs leave) and each CTA waits here until its unit's selection of this step is
+// published.  Deadlock-free: every select CTA is resident before the first attention CTA exists.  A watchdog turns a
+// protocol error into err_flag = 120 instead of a hang.
+__device__ __forceinline__ void wait_unit_selected(const Params &P, int unit) {
+  if (threadIdx.x == 0) {
+    const int want = *reinterpret_cast<volatile int32_t *>(P.epoch);
+    volatile int32_t *f = P.sel_flag + unit;
+    unsigned polls = 0;
+    while (*f != want) {
+      __nanosleep(100);
+      if (++polls > (1u << 24)) { atomicCAS(P.st.err_flag, 0, 120); break; }
+    }
+    __threadfence();    // acquire: the unit's sel_idx / sel_count / probs are visible to this CTA after the barrier
+  }
+  __syncthreads();
 }
 
 // ---- 16-byte vector access -------------------------------------------------------------------

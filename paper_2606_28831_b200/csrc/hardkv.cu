@@ -12,6 +12,7 @@
 #include "stage_kernels.cuh"
 #include "attend_mma.cuh"
 #include "metric_kernels.cuh"
+#include "qcache_kernels.cuh"
 #include "score_select.cuh"
 
 using namespace hardkv;
@@ -35,7 +36,7 @@ namespace {
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout { size_t part, arrive, ss, stats, stage_q, stage_k, stage_v, stage_out, pooled, total; };
+struct WsLayout { size_t part, arrive, ss, stats, stage_q, stage_k, stage_v, stage_out, pooled, qc_stats, qc_final, total; };
 
 size_t esize_of(const hardkv_config &c) { return c.kv_dtype == HARDKV_F32 ? 4 : 2; }
 
@@ -65,6 +66,9 @@ WsLayout ws_layout(const hardkv_config &c) {
   off = align256(off);
   w.stage_out = off; off += align256(qb * sizeof(float));
   w.pooled = off;    off += c.pool_kernel > 1 ? align256((size_t)c.batch * c.num_q_heads * c.max_ctx * sizeof(float)) : 0;
+  // query-cache metric: only configs that declare an accumulation window can hold SCORE_ACCUM_QCACHE heads
+  w.qc_stats = off;  off += c.accum_window > 0 ? align256(units * score_chunks_of(c) * QC_ROWS * sizeof(float2)) : 0;
+  w.qc_final = off;  off += c.accum_window > 0 ? align256(units * QC_ROWS * sizeof(float2)) : 0;
   w.total = off;
   return w;
 }
@@ -130,6 +134,7 @@ hardkv_status check_config(const hardkv_config *c) {
     return HARDKV_ERR_INVALID_ARG;
   if (c->page_size != PAGE) return HARDKV_ERR_UNSUPPORTED;
   if (c->max_ctx % PAGE || c->k_cap % PAGE) return HARDKV_ERR_INVALID_ARG;
+  if (c->accum_window > 0 && c->accum_window * (c->num_q_heads / c->num_kv_heads) > QC_ROWS) return HARDKV_ERR_UNSUPPORTED;
   if (c->pool_kernel < 0 || c->pool_kernel > 63 || (c->pool_kernel > 1 && c->pool_kernel % 2 == 0)) return HARDKV_ERR_INVALID_ARG;
   const int G = c->num_q_heads / c->num_kv_heads;
   const bool gok = G == 1 || G == 2 || G == 4 || G == 5 || G == 7 || G == 8;
@@ -285,6 +290,44 @@ void launch_score_select(hardkv_ctx *ctx, const Params &P0, const void *q, float
   }
 }
 
+// accumulated attention from the query cache (L448; reading C18): two passes over the pool + a reduction, launched
+// only when the caller's state holds a query cache (heads in other modes exit at once)
+void launch_qcache_metric(hardkv_ctx *ctx, const Params &P0, cudaStream_t st) {
+  if (!P0.st.qcache || P0.accum_window <= 0 || ctx->cfg.kv_dtype != HARDKV_BF16) return;
+  const dim3 grid(P0.score_chunks, P0.B * P0.Hkv);
+  const size_t rowb = (size_t)P0.d * 2;
+  const size_t sm1 = QC_ROWS * rowb + 8 * QC_ROWS * sizeof(float2), sm2 = QC_ROWS * rowb + QC_ROWS * sizeof(float2);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(qcache_pass_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(QC_ROWS * 256 + 8 * QC_ROWS * 8));
+    cudaFuncSetAttribute(qcache_pass_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(QC_ROWS * 256 + 8 * QC_ROWS * 8));
+    cudaFuncSetAttribute(qcache_pass_kernel<64, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(QC_ROWS * 256 + 8 * QC_ROWS * 8));
+    cudaFuncSetAttribute(qcache_pass_kernel<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(QC_ROWS * 256 + 8 * QC_ROWS * 8));
+    attr_set = true;
+  }
+  ctx->launches += 3;
+  {
+    const Params P = launch_params(ctx, P0);
+    if (P.d == 128) qcache_pass_kernel<128, 1><<<grid, 256, sm1, st>>>(P);
+    else qcache_pass_kernel<64, 1><<<grid, 256, sm1, st>>>(P);
+  }
+  {
+    const Params P = launch_params(ctx, P0);
+    qcache_reduce_kernel<<<P.B * P.Hkv, QC_ROWS, 0, st>>>(P);
+  }
+  {
+    const Params P = launch_params(ctx, P0);
+    if (P.d == 128) qcache_pass_kernel<128, 2><<<grid, 256, sm2, st>>>(P);
+    else qcache_pass_kernel<64, 2><<<grid, 256, sm2, st>>>(P);
+  }
+}
+
+void launch_qcache_push(hardkv_ctx *ctx, const Params &P, const void *q, cudaStream_t st) {
+  if (!P.st.qcache || P.accum_window <= 0) return;
+  ctx->launches += 1;
+  qcache_push_kernel<<<P.B, 256, 0, st>>>(P, q);
+}
+
 // SNAPKV metric transform (L278): only configs that declare a pooling window pay for the launch
 void launch_pool(hardkv_ctx *ctx, const Params &P0, cudaStream_t st) {
   if (P0.pool_kernel <= 1) return;
@@ -399,6 +442,9 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.pool_kernel = cfg->pool_kernel;
   P.cond_merge = cfg->cond_merge != 0;
   P.pooled = cfg->pool_kernel > 1 ? reinterpret_cast<float *>(base + w.pooled) : nullptr;
+  P.qc_stats = cfg->accum_window > 0 ? reinterpret_cast<float2 *>(base + w.qc_stats) : nullptr;
+  P.qc_final = cfg->accum_window > 0 ? reinterpret_cast<float2 *>(base + w.qc_final) : nullptr;
+  P.st_esize = (int)esize_of(*cfg);
   ctx->stage_q = base + w.stage_q; ctx->stage_k = base + w.stage_k; ctx->stage_v = base + w.stage_v;
   ctx->stage_out = reinterpret_cast<float *>(base + w.stage_out);
   select_geometry(*cfg, 0, 0, &P.sel_cluster, &P.sel_slice_cap, &P.sel_nt);
@@ -491,26 +537,35 @@ hardkv_status hardkv_score(hardkv_ctx *ctx, const hardkv_state *s, const void *q
 }
 
 static bool accum_ok(const hardkv_ctx *ctx, const hardkv_state *s) {
-  // ACCUM heads need their state; score_mode lives on the device, so require the buffers
-  // whenever the config declares a window.
-  return ctx->cfg.accum_window <= 0 || (s->acc && s->ring && s->ring_slot);
+  // ACCUM / ACCUM_QCACHE heads need their state; score_mode lives on the device, so require one complete set of
+  // buffers (the ring of rows or the query cache) whenever the config declares a window.
+  return ctx->cfg.accum_window <= 0 || (s->acc && s->ring && s->ring_slot) || (s->qcache && s->qc_count && s->qc_slot);
 }
 
 hardkv_status hardkv_calibrate_topp(hardkv_ctx *ctx, const hardkv_state *s, float p, hardkv_stream st) {
   if (!state_ok(ctx, s) || !(p > 0.f) || !accum_ok(ctx, s)) return HARDKV_ERR_INVALID_ARG;
   launch_pool(ctx, params_of(ctx, s), st);
+  launch_qcache_metric(ctx, params_of(ctx, s), st);
   launch_select(ctx, params_of(ctx, s), p, 1, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_qcache_push(hardkv_ctx *ctx, const hardkv_state *s, const void *q, hardkv_stream st) {
+  if (!state_ok(ctx, s) || !q || !s->qcache || !s->qc_count || !s->qc_slot || ctx->cfg.accum_window <= 0)
+    return HARDKV_ERR_INVALID_ARG;
+  launch_qcache_push(ctx, params_of(ctx, s), q, st);
   return launch_status();
 }
 
 hardkv_status hardkv_score_select(hardkv_ctx *ctx, const hardkv_state *s, const void *q, float p, hardkv_stream st) {
   if (!state_ok(ctx, s) || !q || !(p > 0.f) || !accum_ok(ctx, s)) return HARDKV_ERR_INVALID_ARG;
   const Params P = params_of(ctx, s);
-  if (ctx->variant == 3) {
+  if (ctx->variant == 3 && !P.st.qcache) {
     launch_score_select(ctx, P, q, p, st);
   } else {
     launch_score(ctx, P, q, st);
     launch_pool(ctx, P, st);
+    launch_qcache_metric(ctx, P, st);
     launch_select(ctx, P, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
   }
   return launch_status();
@@ -580,11 +635,13 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   if (do_select < 0 || do_select > 3) return HARDKV_ERR_INVALID_ARG;
   const bool compress = do_select == HARDKV_STEP_SELECT_REWRITE || do_select == HARDKV_STEP_SELECT_SPARSE;
   launch_append(ctx, P, k_new, v_new, q, compress ? 1 : 0, st);   // between compressions: Step 1 only (L78, L274)
-  if (compress && ctx->variant == 3) {
+  launch_qcache_push(ctx, P, q, st);                              // the query window slides on every step (L448)
+  if (compress && ctx->variant == 3 && !P.st.qcache) {
     launch_score_select(ctx, P, q, p, st);
   } else if (compress) {
     launch_score(ctx, P, q, st);
     launch_pool(ctx, P, st);
+    launch_qcache_metric(ctx, P, st);
     // the score kernel's chunk statistics describe the raw logits: configs with pooled heads take them in-kernel
     launch_select(ctx, P, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
   }

@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(SOLVE_NT, 1) solve_temperature_kernel(Params P
   __shared__ SolveShared sh;
   const int unit = blockIdx.x, b = unit / P.Hkv, h = unit % P.Hkv;
   const int mode = P.st.score_mode[h];
-  if (mode == HARDKV_SCORE_ACCUM) return;          // reading C4: T stays inside the per-step softmax
+  if (mode == HARDKV_SCORE_ACCUM || mode == HARDKV_SCORE_ACCUM_QCACHE) return;   // readings C4 / C18: accumulated metrics keep their T
   int n, lo, hi;
   pool_bounds(P, b, n, lo, hi);
   if (hi <= lo) return;

@@ -109,6 +109,12 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
     if (want_mask)
       for (int y = rank * NT + tid; y < mask_bytes; y += C * NT) mask[y] = 0;
     if (rank == 0 && tid == 0) P.st.sel_count[unit] = 0;
+    __syncthreads();
+    if (C > 1) cluster.sync();
+    if (rank == 0 && tid == 0 && P.sel_flag) {
+      __threadfence();
+      *reinterpret_cast<volatile int32_t *>(P.sel_flag + unit) = *reinterpret_cast<volatile int32_t *>(P.epoch);
+    }
     return;
   }
 
@@ -123,7 +129,9 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
   for (int d = tid; d < SEL_NB; d += NT) { sh.h_cnt[d] = 0; sh.h_hi[d] = 0; sh.h_lo[d] = 0; }
 
   // ---------------- 2a: calibration ------------------------------------------------------------
-  if (CALIBRATE) {
+  // heads on the query-cache metric arrive with their probabilities in state->probs (qcache_kernels.cuh): select as given
+  const bool given = CALIBRATE == 0 || P.st.score_mode[h] == HARDKV_SCORE_ACCUM_QCACHE;
+  if (!given) {
     // softmax in the base-2 domain: exp(z/T - m) = 2^(z*c2 - m2), c2 = log2(e)/T (one FFMA + one MUFU.EX2)
     const float c2 = 1.4426950408889634f / P.st.temperature[unit];
     // SNAPKV heads calibrate the max-pooled copy of their logits (L278; metric_kernels.cuh), all others the raw logits
@@ -631,6 +639,13 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
     for (int y = y1 + gt_; y < mask_bytes; y += gs_) mask[y] = 0;
   }
   if (C > 1) cluster.sync();  // no CTA may exit while a peer can still read its shared memory
+  else __syncthreads();
+  // publish: every thread's stores of this unit (sel_idx, sel_count, sel_table, votes) happen before the barrier above,
+  // the fence is cumulative, then the flag -- the attention kernel may already be waiting for it (wait_unit_selected)
+  if (rank == 0 && tid == 0 && P.sel_flag) {
+    __threadfence();
+    *reinterpret_cast<volatile int32_t *>(P.sel_flag + unit) = *reinterpret_cast<volatile int32_t *>(P.epoch);
+  }
 }
 
 // One thread-block cluster (or one CTA) per (sequence, KV head).

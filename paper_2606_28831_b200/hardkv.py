@@ -46,7 +46,7 @@ class Config(C.Structure):
 _STATE_FIELDS = ["k_pool", "v_pool", "base_table", "sel_k_pool", "sel_v_pool", "sel_pages", "cond_k", "cond_v",
                  "cond_pos", "cond_votes", "cond_count", "ctx_len", "c_lo", "l_lower", "l_upper", "votes",
                  "temperature", "score_mode", "acc", "ring", "ring_slot", "sel_idx", "sel_count", "sel_table",
-                 "sel_mask", "logits", "probs", "err_flag", "dense_lo"]
+                 "sel_mask", "logits", "probs", "err_flag", "qcache", "qc_count", "qc_slot", "dense_lo"]
 
 
 class StateStruct(C.Structure):
@@ -56,7 +56,7 @@ class StateStruct(C.Structure):
 F32, BF16 = 0, 1
 STEP_REUSE_TIER, STEP_SELECT_REWRITE, STEP_SELECT_SPARSE, STEP_REUSE_SPARSE = 0, 1, 2, 3   # do_select of decode_step
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
-           "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_timing", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_score_select", "hardkv_calibrate_topp", "hardkv_solve_temperature",
+           "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_timing", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_score_select", "hardkv_qcache_push", "hardkv_calibrate_topp", "hardkv_solve_temperature",
            "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend", "hardkv_sparse_attend",
            "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count", "hardkv_probe_read_stream"]
 
@@ -82,6 +82,7 @@ def _load():
     lib.hardkv_score.argtypes = [vp, sp, vp, vp]
     lib.hardkv_calibrate_topp.argtypes = [vp, sp, C.c_float, vp]
     lib.hardkv_score_select.argtypes = [vp, sp, vp, C.c_float, vp]
+    lib.hardkv_qcache_push.argtypes = [vp, sp, vp, vp]
     lib.hardkv_solve_temperature.argtypes = [vp, sp, C.c_float, C.c_float, C.c_float, C.c_float, C.c_int32, vp]
     lib.hardkv_topp_select.argtypes = [vp, sp, C.c_float, vp]
     lib.hardkv_rewrite.argtypes = [vp, sp, vp]
@@ -193,6 +194,9 @@ class HardKV:
 
     def score_select(self, st: DeviceState, q, p: float):
         _check(lib.hardkv_score_select(self._ctx, C.byref(st.struct()), _ptr(q), np.float32(p), _stream()))
+
+    def qcache_push(self, st: DeviceState, q):
+        _check(lib.hardkv_qcache_push(self._ctx, C.byref(st.struct()), _ptr(q), _stream()))
 
     def calibrate_topp(self, st: DeviceState, p: float):
         _check(lib.hardkv_calibrate_topp(self._ctx, C.byref(st.struct()), np.float32(p), _stream()))

@@ -19,7 +19,7 @@ def torch_dtype(wl: Workload):
 
 
 def make_engine(wl: Workload, device="cuda:0", want_accum=None, reuse_max: int = 0) -> hardkv.HardKV:
-    accum = bool(np.any(wl.score_mode == 1)) if want_accum is None else want_accum
+    accum = bool(np.any((wl.score_mode == 1) | (wl.score_mode == 3))) if want_accum is None else want_accum
     return hardkv.HardKV(batch=wl.B, num_q_heads=wl.Hq, num_kv_heads=wl.Hkv, head_dim=wl.d, max_ctx=wl.max_ctx,
                          sink=wl.sink, recent=wl.recent, k_cap=wl.k_cap, cond_cap=wl.cond_cap,
                          kv_dtype=hardkv.BF16 if wl.dtype == "bf16" else hardkv.F32,
@@ -53,6 +53,7 @@ def make_state(wl: Workload, device="cuda:0", prefill=None, want_mask=False, lay
     sel_pages = torch.from_numpy(sel_np).to(device)
     i32 = lambda a: torch.from_numpy(np.ascontiguousarray(a, np.int32)).to(device)
     accum = bool(np.any(wl.score_mode == 1))
+    qcache = bool(np.any(wl.score_mode == 3))
     keep = {} if prefill is None else prefill
     states = []
     for layer in range(layers):
@@ -114,6 +115,9 @@ def make_state(wl: Workload, device="cuda:0", prefill=None, want_mask=False, lay
             probs=torch.zeros(units, mc, dtype=torch.float32, device=device),
             err_flag=torch.zeros(1, dtype=torch.int32, device=device),
             dense_lo=i32(np.maximum(np.minimum(wl.sink, wl.n0), wl.n0 - wl.recent)),
+            qcache=torch.zeros(B, Hq, wl.accum_window, d, dtype=dt, device=device) if qcache else None,
+            qc_count=torch.zeros(B, dtype=torch.int32, device=device) if qcache else None,
+            qc_slot=torch.zeros(B, dtype=torch.int32, device=device) if qcache else None,
         )
         states.append(st)
     return states, keep
@@ -126,7 +130,7 @@ def gather_rows(pool: torch.Tensor, table_unit: torch.Tensor, n: int) -> np.ndar
 
 
 _MUTABLE = ["votes", "cond_k", "cond_v", "cond_pos", "cond_votes", "cond_count", "ctx_len", "c_lo", "dense_lo", "sel_idx",
-            "sel_count", "sel_table", "acc", "ring", "ring_slot"]
+            "sel_count", "sel_table", "acc", "ring", "ring_slot", "qcache", "qc_count", "qc_slot"]
 
 
 def snapshot(st: hardkv.DeviceState) -> dict:

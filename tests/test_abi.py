@@ -33,7 +33,7 @@ def test_header_symbols_exported(lib):
 
 def test_struct_layout_matches_header(lib):
     assert C.sizeof(lib.Config) == 16 * 4
-    assert C.sizeof(lib.StateStruct) == 29 * C.sizeof(C.c_void_p)
+    assert C.sizeof(lib.StateStruct) == 32 * C.sizeof(C.c_void_p)
 
 
 def test_host_only_validation(lib):

@@ -330,6 +330,19 @@ def test_config4_full_size_sweep_ring_wraps(p, c4_state):
     s.report(f"c4 p={p} {steps} steps")
 
 
+def test_config4_full_size_query_cache_recompute():
+    """SURVEY 8(f)-1 / PAPER.md L448: BASELINE configs[4] with its accumulated-attention heads (4-7) on the query-cache
+    form -- the last 32 queries score the CURRENT 64k pool (M = 160 query rows per unit, a real contraction) instead of
+    summing a ring of per-step rows.  40 steps so the query window fills and wraps; sampled units against the oracle."""
+    wl = make_workload(4, score_mode=np.array([0, 0, 0, 0, 3, 3, 3, 3], np.uint8))
+    s = Sampled(wl, [(0, 1), (3, 6), (7, 4), (5, 7)], graph=True)
+    steps = 36
+    for t in range(steps):
+        s.step(t, 0.9, full_check=(t < 2 or t in (31, 32, 33) or t == steps - 1))
+    assert all(u.u.qc_count == wl.accum_window for (b, h), u in zip(s.sample, s.units) if wl.score_mode[h] == 3)
+    s.report(f"c4 query-cache ACCUM p=0.9 {steps} steps")
+
+
 def test_config2_full_size_snapkv_solve_then_step():
     """Full-size config 2 with half the KV heads on the SNAPKV metric (window 7): Algorithm 2 solves T on the first
     step's logits (sampled units against the oracle's bisection, 1e-3 relative), then fused steps run with the

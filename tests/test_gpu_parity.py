@@ -38,6 +38,11 @@ def small_workloads():
                                score_mode=np.array([0, 2, 2, 0, 2, 0, 2, 2], np.uint8), pool_kernel=7),
         "snap7": make_workload(3, B=2, n0=i32(1300, 1300), max_ctx=1536, k_cap=256, l_upper=i32(1100, 1100),
                                cond_cap=8, steps=6, score_mode=np.array([2, 2, 0, 2], np.uint8), pool_kernel=5),
+        # accumulated attention recomputed from the query cache (L448; score_mode 3), alone and next to ring-sum ACCUM heads
+        "qc4": make_workload(1, n0=i32(2100), max_ctx=2176, k_cap=512, l_upper=i32(1960), cond_cap=32, steps=8,
+                             score_mode=np.array([0, 3, 3, 0, 3, 0, 3, 3], np.uint8), accum_window=4),
+        "qc5": make_workload(4, B=2, n0=i32(1500, 1500), max_ctx=1600, k_cap=384, l_upper=i32(1390, 1390),
+                             cond_cap=16, accum_window=6, steps=9, score_mode=np.array([0, 3, 0, 1, 3, 1, 3, 3], np.uint8)),
         "g8": make_workload(1, Hq=8, Hkv=1, n0=i32(1100), max_ctx=1120, k_cap=1120, l_upper=i32(5000), cond_cap=0,
                             steps=3),
     }
@@ -67,11 +72,14 @@ def test_stages_teacher_forced(name, P):
             u.append(kn.reshape(-1, d)[i], vn.reshape(-1, d)[i])
             u.retire()
         pr.check_bookkeeping()
-        # step 1: score
+        # step 1: score (and, for heads on the query-cache metric, the window slides: L448)
         eng.score(st, qd)
+        if st.qcache is not None:
+            eng.qcache_push(st, qd)
         qu = q.reshape(-1, G, d)
         for i, u in enumerate(ob.units):
             u.score(qu[i])
+            u.qcache_push(qu[i])
         pr.check_logits()
         # step 2a-2c end to end from the CUDA logits (votes restored afterwards)
         votes0 = st.votes.clone()
