@@ -123,6 +123,11 @@ hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant);
  * CTA in {512, 1024}; 0 keeps the automatic choice for that argument.  HARDKV_ERR_UNSUPPORTED when a CTA's slice of the
  * pool would not fit one SM's shared memory.  Host-side only; call it before capturing a graph with this ctx. */
 hardkv_status hardkv_set_select_geometry(hardkv_ctx *ctx, int32_t cluster, int32_t threads);
+/* 1 (default): in hardkv_decode_step's compression steps on the bf16 paths the attention kernel is launched
+ * programmatically behind the select kernel: its CTAs take the SMs that finished selections leave and wait per unit for
+ * that unit's selection (flag published by the select kernel), units in the order their selections finish, so the
+ * latency-bound selection of the long units hides under the attention of the short ones.  0: plain stream order. */
+hardkv_status hardkv_set_overlap(hardkv_ctx *ctx, int32_t on);
 /* Measurement hook: while `slots` (DEVICE memory, 2 * capacity u64, the caller presets every pair to (~0, 0)) is set,
  * the i-th hot-kernel launch made through this ctx (append, score, select, score_select, attend; generic variants
  * excepted) records the globaltimer ns at which its first CTA started and its last CTA ended in slots[2 i], slots[2 i

@@ -29,8 +29,10 @@ __device__ __forceinline__ void mma_bf16_16816(float (&c)[4], uint32_t a0, uint3
 //   k-slots (2 tig, 2 tig + 1, 2 tig + 8, 2 tig + 9) of MMA 2c + s  <-  elements 32c + 8 tig + 4s + (0, 1, 2, 3).
 // Accumulator fragment: c0/c1 = token gid, heads 2 tig / 2 tig + 1; c2/c3 = token gid + 8.
 // =============================================================================================
-template <int D>
-__global__ void __launch_bounds__(256) score_mma_kernel(Params P, const void *q_) {
+// PIF: pages a warp keeps in flight (all of their loads are issued before the first MMA); MINB: CTAs per SM the
+// register allocation is held to.
+template <int D, int PIF = 2, int MINB = 2>
+__global__ void __launch_bounds__(256, MINB) score_mma_kernel(Params P, const void *q_) {
   pdl_wait_then_trigger();
   KernelClock kclock(P);
   constexpr int NCH = D / 32;                 // 64-byte chunks per row
@@ -69,12 +71,12 @@ __global__ void __launch_bounds__(256) score_mma_kernel(Params P, const void *q_
   int my_page = -1;
   if (lane < PPW && wp0 + lane >= first_page && wp0 + lane <= last_page) my_page = __ldg(tab + wp0 + lane);
 #pragma unroll 1
-  for (int j0 = 0; j0 < PPW; j0 += 2) {
-    // two pages (8 KiB) in flight per warp: all 16 loads are issued before the first MMA
-    int phys[2];
-    uint4 ka[2][NCH], kb[2][NCH];
+  for (int j0 = 0; j0 < PPW; j0 += PIF) {
+    // PIF pages (4 KiB each) in flight per warp: all their loads are issued before the first MMA
+    int phys[PIF];
+    uint4 ka[PIF][NCH], kb[PIF][NCH];
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
+    for (int u = 0; u < PIF; ++u) {
       phys[u] = __shfl_sync(0xffffffffu, my_page, j0 + u);
       if (phys[u] >= 0) {   // warp-uniform; one base per page, every load at an immediate offset from it
         const char *src = klane + (size_t)phys[u] * (PAGE * ROWB);
@@ -90,7 +92,7 @@ __global__ void __launch_bounds__(256) score_mma_kernel(Params P, const void *q_
       }
     }
 #pragma unroll
-    for (int u = 0; u < 2; ++u) {
+    for (int u = 0; u < PIF; ++u) {
       if (phys[u] < 0) continue;   // warp-uniform
       const int pg = wp0 + j0 + u;
       float acc[4] = {0.f, 0.f, 0.f, 0.f};

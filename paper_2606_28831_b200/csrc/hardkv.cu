@@ -21,6 +21,7 @@ struct hardkv_ctx {
   hardkv_config cfg;
   Params base;      // config-derived fields + workspace pointers; `st` is filled per call
   int variant;
+  int overlap;                   // 1 (default): the attention of a compression step starts while the select kernel runs
   int fused_ok;                  // the fused score -> select kernel applies to this config (score_select.cuh)
   unsigned long long *timing;    // hardkv_set_timing: per-launch (first CTA start, last CTA end), or NULL
   int timing_cap, timing_next;
@@ -36,7 +37,7 @@ namespace {
 
 size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
 
-struct WsLayout { size_t part, arrive, ss, stats, stage_q, stage_k, stage_v, stage_out, pooled, qc_stats, qc_final, total; };
+struct WsLayout { size_t part, arrive, ss, ovl, stats, stage_q, stage_k, stage_v, stage_out, pooled, qc_stats, qc_final, total; };
 
 size_t esize_of(const hardkv_config &c) { return c.kv_dtype == HARDKV_F32 ? 4 : 2; }
 
@@ -55,6 +56,7 @@ WsLayout ws_layout(const hardkv_config &c) {
   size_t off = 0;
   w.arrive = off; off += align256(units * sizeof(int32_t));
   w.ss = off;     off += align256((units + 1) * sizeof(int32_t));
+  w.ovl = off;    off += align256((2 * units + 1) * sizeof(int32_t));   // sel_flag[units] | unit_order[units] | epoch
   w.part = off;   off += align256(units * att_chunks_of(c) * G * (c.head_dim + 2) * sizeof(float));
   w.stats = off;  off += align256(units * score_chunks_of(c) * 8 * sizeof(float2));
   const size_t qb = (size_t)c.batch * c.num_q_heads * c.head_dim, kb = units * c.head_dim;
@@ -219,7 +221,8 @@ void launch_append(hardkv_ctx *ctx, const Params &P0, const void *k_new, const v
                    int do_retire, cudaStream_t st) {
   const Params P = launch_params(ctx, P0);
   ctx->launches += 1;
-  HK_DISPATCH_TD(ctx->cfg, (launch_pdl(ctx, append_retire_kernel<T, D>, dim3(P.B), dim3(256), 0, st, P, k_new, v_new, q,
+  // one CTA per sequence + one for the step counter and the unit order of the overlapped attention
+  HK_DISPATCH_TD(ctx->cfg, (launch_pdl(ctx, append_retire_kernel<T, D>, dim3(P.B + 1), dim3(256), 0, st, P, k_new, v_new, q,
                                        do_retire)));
 }
 
@@ -234,8 +237,10 @@ void launch_score(hardkv_ctx *ctx, const Params &P0, const void *q, cudaStream_t
     return;
   }
   if (fast_path(ctx)) {
-    if (P.d == 128) launch_pdl(ctx, score_mma_kernel<128>, grid, dim3(256), 0, st, P, q);
-    else launch_pdl(ctx, score_mma_kernel<64>, grid, dim3(256), 0, st, P, q);
+    // d = 128: one page in flight per warp at 64 registers, four CTAs per SM -- the same 128 KiB in flight per SM as two
+    // pages at two CTAs, in 32 warps instead of 16 (98.5 vs 100.7 us on config 2, probe in profiles/r2_probes.md)
+    if (P.d == 128) launch_pdl(ctx, score_mma_kernel<128, 1, 4>, grid, dim3(256), 0, st, P, q);
+    else launch_pdl(ctx, score_mma_kernel<64, 2, 2>, grid, dim3(256), 0, st, P, q);
     return;
   }
   HK_DISPATCH_TD(ctx->cfg, HK_DISPATCH_G(P.G, (score_generic_kernel<T, D, G><<<grid, 256, 0, st>>>(P, q))));
@@ -343,10 +348,30 @@ void launch_rewrite(hardkv_ctx *ctx, const Params &P, cudaStream_t st) {
   HK_DISPATCH_TD(ctx->cfg, (rewrite_kernel<T, D><<<grid, 256, 0, st>>>(P)));
 }
 
+// overlap = 1: the launch directly follows the select kernel in the stream and may start while it runs (programmatic
+// dependent launch): its CTAs take units in the order their selections finish and wait per unit (wait_unit_selected)
 void launch_attend(hardkv_ctx *ctx, const Params &P0, const void *q, float *out, float *lse, int mode,
-                   cudaStream_t st) {
-  const Params P = launch_params(ctx, P0);
+                   cudaStream_t st, int overlap = 0) {
+  Params P = launch_params(ctx, P0);
   ctx->launches += 1;
+  if (fast_path(ctx) && overlap) {
+    P.wait_select = 1;
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3((P.att_chunks * ATT_CHUNK + ATT_MMA_CHUNK - 1) / ATT_MMA_CHUNK, P.B * P.Hkv);
+    lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0; lc.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    lc.attrs = at; lc.numAttrs = 1;
+    if (P.d == 128) {
+      if (mode == ATT_REWRITE) cudaLaunchKernelEx(&lc, attend_mma_kernel<128, ATT_REWRITE>, P, q, out, lse);
+      else cudaLaunchKernelEx(&lc, attend_mma_kernel<128, ATT_SPARSE>, P, q, out, lse);
+    } else {
+      if (mode == ATT_REWRITE) cudaLaunchKernelEx(&lc, attend_mma_kernel<64, ATT_REWRITE>, P, q, out, lse);
+      else cudaLaunchKernelEx(&lc, attend_mma_kernel<64, ATT_SPARSE>, P, q, out, lse);
+    }
+    return;
+  }
   if (fast_path(ctx)) {
     dim3 gm((P.att_chunks * ATT_CHUNK + ATT_MMA_CHUNK - 1) / ATT_MMA_CHUNK, P.B * P.Hkv);
     const size_t sm = 0;
@@ -423,6 +448,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   memset(ctx, 0, sizeof(*ctx));
   ctx->cfg = *cfg;
   ctx->variant = 1;
+  ctx->overlap = 1;
   ctx->ws_bytes = w.total;
   Params &P = ctx->base;
   P.B = cfg->batch; P.Hq = cfg->num_q_heads; P.Hkv = cfg->num_kv_heads; P.G = P.Hq / P.Hkv;
@@ -436,6 +462,10 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.ss_arrive = reinterpret_cast<int32_t *>(base + w.ss);
   P.ss_next = P.ss_arrive + (size_t)cfg->batch * cfg->num_kv_heads;
   P.ss_slice_cap = ss_slice_cap_of(*cfg);
+  P.sel_flag = reinterpret_cast<int32_t *>(base + w.ovl);
+  P.unit_order = P.sel_flag + (size_t)cfg->batch * cfg->num_kv_heads;
+  P.epoch = P.unit_order + (size_t)cfg->batch * cfg->num_kv_heads;
+  P.wait_select = 0;
   P.part = reinterpret_cast<float *>(base + w.part);
   P.score_stats = reinterpret_cast<float2 *>(base + w.stats);
   P.score_chunks = score_chunks_of(*cfg);
@@ -500,6 +530,12 @@ hardkv_status hardkv_set_select_geometry(hardkv_ctx *ctx, int32_t cluster, int32
   if ((size_t)cap * 4 + sizeof(SelShared) > 227u * 1024u) return HARDKV_ERR_UNSUPPORTED;
   ctx->base.sel_cluster = cl; ctx->base.sel_slice_cap = cap; ctx->base.sel_nt = nt;
   return raise_select_smem(ctx->base) ? HARDKV_OK : HARDKV_ERR_CUDA;
+}
+
+hardkv_status hardkv_set_overlap(hardkv_ctx *ctx, int32_t on) {
+  if (!ctx || (on != 0 && on != 1)) return HARDKV_ERR_INVALID_ARG;
+  ctx->overlap = on;
+  return HARDKV_OK;
 }
 
 hardkv_status hardkv_set_timing(hardkv_ctx *ctx, unsigned long long *slots, int32_t capacity) {
@@ -645,8 +681,10 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
     // the score kernel's chunk statistics describe the raw logits: configs with pooled heads take them in-kernel
     launch_select(ctx, P, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
   }
+  // the select kernel (variants 1, 2: the last launch above) is followed by the attention of the same units: overlap them
+  const int overlap = compress && ctx->overlap && fast_path(ctx) && (ctx->variant == 1 || ctx->variant == 2);
   launch_attend(ctx, P, q, out, lse, do_select == HARDKV_STEP_SELECT_REWRITE ? ATT_REWRITE
-                                     : (do_select == HARDKV_STEP_REUSE_TIER ? ATT_TIER : ATT_SPARSE), st);
+                                     : (do_select == HARDKV_STEP_REUSE_TIER ? ATT_TIER : ATT_SPARSE), st, overlap);
   return launch_status();
 }
 

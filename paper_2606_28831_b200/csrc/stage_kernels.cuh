@@ -25,22 +25,28 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
   __shared__ float s_qbar[8][D];  // per warp: group mean of the step's queries (merging only)
   const bool merging = P.cond_merge && q_ != nullptr && P.cond_cap > 0;
   if ((int)blockIdx.x == P.B) {
-    // ---- one extra CTA: the step counter, and the units by increasing pool length AFTER this step's append / retirement
-    //      (arithmetic on the old scalars, so it does not wait for the other CTAs): the order in which the selections of
-    //      this step will finish, which is the order the overlapped attention kernel takes the units in ----
+    // ---- one extra CTA: the step counter, and unit_order = the units by increasing pool length AFTER this step's
+    //      append / retirement (arithmetic on the old scalars, so this CTA does not wait for the others): the order in
+    //      which the selections of this step finish, which is the order the overlapped attention kernel takes them in ----
+    __shared__ int s_len[1024];
     if (threadIdx.x == 0) *P.epoch += 1;
     const int units = P.B * P.Hkv;
+    auto len_of = [&](int v) {
+      const int bb = v / P.Hkv, n1_ = P.st.ctx_len[bb] + 1;
+      int c = P.st.c_lo[bb];
+      if (do_retire && n1_ - P.recent - c > P.st.l_upper[bb]) c = n1_ - P.recent - P.st.l_upper[bb];
+      return max(n1_ - P.recent - c, 0);
+    };
+    const bool cached = units <= 1024;
+    if (cached) {
+      for (int u = threadIdx.x; u < units; u += blockDim.x) s_len[u] = len_of(u);
+      __syncthreads();
+    }
     for (int u = threadIdx.x; u < units; u += blockDim.x) {
-      auto len_of = [&](int v) {
-        const int bb = v / P.Hkv, n1_ = P.st.ctx_len[bb] + 1;
-        int c = P.st.c_lo[bb];
-        if (do_retire && n1_ - P.recent - c > P.st.l_upper[bb]) c = n1_ - P.recent - P.st.l_upper[bb];
-        return max(n1_ - P.recent - c, 0);
-      };
-      const int len = len_of(u);
+      const int len = cached ? s_len[u] : len_of(u);
       int r = 0;
       for (int v = 0; v < units; ++v) {
-        const int lv = len_of(v);
+        const int lv = cached ? s_len[v] : len_of(v);
         r += (lv < len) || (lv == len && v < u);
       }
       P.unit_order[r] = u;

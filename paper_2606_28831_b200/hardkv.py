@@ -56,7 +56,7 @@ class StateStruct(C.Structure):
 F32, BF16 = 0, 1
 STEP_REUSE_TIER, STEP_SELECT_REWRITE, STEP_SELECT_SPARSE, STEP_REUSE_SPARSE = 0, 1, 2, 3   # do_select of decode_step
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
-           "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_timing", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_score_select", "hardkv_qcache_push", "hardkv_calibrate_topp", "hardkv_solve_temperature",
+           "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_overlap", "hardkv_set_timing", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_score_select", "hardkv_qcache_push", "hardkv_calibrate_topp", "hardkv_solve_temperature",
            "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend", "hardkv_sparse_attend",
            "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count", "hardkv_probe_read_stream"]
 
@@ -76,6 +76,7 @@ def _load():
     lib.hardkv_set_variant.argtypes = [vp, C.c_int32]
     lib.hardkv_set_select_geometry.argtypes = [vp, C.c_int32, C.c_int32]
     lib.hardkv_set_pdl.argtypes = [vp, C.c_int32]
+    lib.hardkv_set_overlap.argtypes = [vp, C.c_int32]
     lib.hardkv_set_timing.argtypes = [vp, vp, C.c_int32]
     lib.hardkv_append_kv.argtypes = [vp, sp, vp, vp, vp]
     lib.hardkv_append_kv_merge.argtypes = [vp, sp, vp, vp, vp, vp]
@@ -179,6 +180,9 @@ class HardKV:
         else:
             assert slots.is_cuda and slots.is_contiguous() and slots.dtype == torch.int64 and slots.shape[1] == 2
             _check(lib.hardkv_set_timing(self._ctx, _ptr(slots), slots.shape[0]))
+
+    def set_overlap(self, on: bool):
+        _check(lib.hardkv_set_overlap(self._ctx, int(on)))
 
     def set_pdl(self, on: bool):
         _check(lib.hardkv_set_pdl(self._ctx, int(on)))
