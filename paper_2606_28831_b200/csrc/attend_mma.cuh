@@ -23,7 +23,10 @@
 
 namespace hardkv {
 
-constexpr int ATT_TPW = 4;                    // tiles of 16 rows per warp
+#ifndef HARDKV_ATT_TPW
+#define HARDKV_ATT_TPW 4
+#endif
+constexpr int ATT_TPW = HARDKV_ATT_TPW;       // tiles of 16 rows per warp
 constexpr int ATT_MMA_CHUNK = 8 * ATT_TPW * 16;   // virtual rows per CTA: 8 warps x ATT_TPW tiles
 constexpr uint32_t ROW_INVALID = 0xffffffffu;
 

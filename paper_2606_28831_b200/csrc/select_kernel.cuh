@@ -565,12 +565,16 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
   }
 
   // ---------------- 2c: stream compaction in ascending position order -----------------------------
-  const int w0 = warp * wseg;  // this warp's contiguous segment of the slice
+  // A lane owns 4 consecutive tokens of every 128-token group of its warp's segment (one 16-byte LDS); lane-major order
+  // is position order.  Slice entries outside the pool are SEL_INVALID (> every probability): `valid` masks them.
+  const int w0 = warp * wseg;  // this warp's contiguous segment of the slice (a multiple of 32 tokens)
   {
     int gt = 0, tie = 0;
-    for (int i = w0 + lane; i < w0 + wseg; i += 32) {
-      const uint32_t bits = pbits[i];
-      if (bits != SEL_INVALID) { gt += bits > tau; tie += bits == tau; }
+    for (int i = w0 + 4 * lane; i < w0 + wseg; i += 128) {
+      const uint4 v = *reinterpret_cast<const uint4 *>(pbits + i);
+      gt += (v.x > tau && v.x != SEL_INVALID) + (v.y > tau && v.y != SEL_INVALID) + (v.z > tau && v.z != SEL_INVALID) +
+            (v.w > tau && v.w != SEL_INVALID);
+      tie += (v.x == tau) + (v.y == tau) + (v.z == tau) + (v.w == tau);
     }
     gt = __reduce_add_sync(0xffffffffu, gt);
     tie = __reduce_add_sync(0xffffffffu, tie);
@@ -595,36 +599,79 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
       tie_before += tw;
     }
   }
-  for (int w = 0; w < warp; ++w) {
-    const int tw = sh.w_tie[w];
-    int take = r_ties - tie_before;
+  {
+    // this warp's offsets from the per-warp counts, in parallel: lane l stands for warp l (ties are taken in position
+    // order, r_ties in all: a warp takes what is left when the ties of the warps before it are counted)
+    const int tw = lane < NW ? sh.w_tie[lane] : 0, gw = lane < NW ? sh.w_gt[lane] : 0;
+    int tpre = tw;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t_ = __shfl_up_sync(0xffffffffu, tpre, o);
+      if (lane >= o) tpre += t_;
+    }
+    int take = r_ties - (tie_before + tpre - tw);
     take = take < 0 ? 0 : (take > tw ? tw : take);
-    sel_before += sh.w_gt[w] + take;
-    tie_before += tw;
+    sel_before += __reduce_add_sync(0xffffffffu, lane < warp ? gw + take : 0);
+    tie_before += __reduce_add_sync(0xffffffffu, lane < warp ? tw : 0);
   }
   int32_t *votes = P.st.votes + (size_t)unit * P.max_ctx;
-  const unsigned lt = (1u << lane) - 1u;
-  for (int i0 = w0; i0 < w0 + wseg; i0 += 32) {
-    const int pos0 = s0 + i0;               // multiple of 32: one aligned word of the packed mask
+  for (int g0 = w0; g0 < w0 + wseg; g0 += 128) {
+    const int pos0 = s0 + g0;               // multiple of 32
     if (pos0 >= hi) break;                  // warp-uniform
-    const uint32_t bits = pbits[i0 + lane];
-    const bool valid = bits != SEL_INVALID;
-    const bool g = valid && bits > tau;
-    const bool t = valid && bits == tau;
-    const unsigned tb = __ballot_sync(0xffffffffu, t);
-    const bool s = g || (t && (tie_before + __popc(tb & lt)) < r_ties);
-    const unsigned sb = __ballot_sync(0xffffffffu, s);
-    if (s) {
-      const int pos = pos0 + lane;
-      sel_idx[sel_before + __popc(sb & lt)] = pos;
-      atomicAdd(votes + pos, 1);  // cumulative selection mask = votes (L86); result unused -> RED, no round trip
+    const int i = g0 + 4 * lane;
+    uint4 v = make_uint4(SEL_INVALID, SEL_INVALID, SEL_INVALID, SEL_INVALID);
+    if (i < w0 + wseg) v = *reinterpret_cast<const uint4 *>(pbits + i);
+    const uint32_t bq[4] = {v.x, v.y, v.z, v.w};
+    unsigned m = 0, tq = 0;                 // 4-bit masks of this lane: selected because > tau / equal to tau
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      m |= (unsigned)(bq[e] > tau && bq[e] != SEL_INVALID) << e;
+      tq |= (unsigned)(bq[e] == tau) << e;
     }
-    if (want_mask && lane < 4) {  // bit i%8 of byte i/8 (L439): byte y of the word holds bits 8y..8y+7
-      const int y = (pos0 >> 3) + lane;
-      if (y < mask_bytes) mask[y] = (uint8_t)(sb >> (8 * lane));
+    if (!want_mask && !__any_sync(0xffffffffu, (m | tq) != 0)) continue;   // most groups of a sparse head hold nothing
+    int ntie = 0;
+    if (__any_sync(0xffffffffu, tq != 0)) {
+      // ties (rare: usually the one token that is the threshold): the first r_ties of them in position order are taken
+      ntie = __popc(tq);
+      int tpre = ntie;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t_ = __shfl_up_sync(0xffffffffu, tpre, o);
+        if (lane >= o) tpre += t_;
+      }
+      const int tall = __shfl_sync(0xffffffffu, tpre, 31);
+      int seen = tie_before + tpre - ntie;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        if ((tq >> e) & 1) { m |= (unsigned)(seen < r_ties) << e; ++seen; }
+      }
+      tie_before += tall;
     }
-    tie_before += __popc(tb);
-    sel_before += __popc(sb);
+    const int cnt = __popc(m);
+    int pre = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int t_ = __shfl_up_sync(0xffffffffu, pre, o);
+      if (lane >= o) pre += t_;
+    }
+    const int call = __shfl_sync(0xffffffffu, pre, 31);
+    if (m) {
+      int dst = sel_before + pre - cnt;
+      const int pos = pos0 + 4 * lane;
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        if ((m >> e) & 1) {
+          sel_idx[dst++] = pos + e;
+          atomicAdd(votes + pos + e, 1);  // cumulative selection mask = votes (L86); result unused -> RED, no round trip
+        }
+      }
+    }
+    if (want_mask) {  // bit i%8 of byte i/8 (L439): byte y holds tokens 8y..8y+7 = the nibbles of lanes 2y, 2y + 1
+      const unsigned hi_nib = __shfl_down_sync(0xffffffffu, m, 1);
+      const int y = (pos0 >> 3) + (lane >> 1);
+      if ((lane & 1) == 0 && i < w0 + wseg && y < mask_bytes) mask[y] = (uint8_t)(m | (hi_nib << 4));
+    }
+    sel_before += call;
   }
   // pads, the head-wise block table (reading C9; L207-209) and the mask bytes outside the slices
   const int gt_ = rank * NT + tid, gs_ = C * NT;

@@ -589,3 +589,28 @@ def test_depth_one_graph_over_layers_with_shared_block_ids():
                 pr.check_votes()
             pr.force_discrete_state()
     assert not torch.equal(pairs[0].out, pairs[1].out)
+
+
+@pytest.mark.parametrize("name", ["c1s", "c2s", "c3s", "c4s", "g1d64", "g8", "c2m", "qc4"])
+def test_select_attention_overlap(name, P):
+    """hardkv_decode_step launches the attention kernel programmatically behind the select kernel (it starts on the SMs
+    that finished selections leave, takes the units in the order their selections finish and waits per unit on a flag).
+    Bit for bit the same as plain stream order (hardkv_set_overlap(0)) on a second engine, step after step; c2m has more
+    units than one wave of select CTAs leaves SMs for."""
+    if name == "c2m":
+        n0 = np.linspace(500, 2600, 12).astype(np.int32)
+        wl = make_workload(2, B=12, n0=n0, max_ctx=2816, k_cap=384, l_upper=(n0 - 132).astype(np.int32), cond_cap=16, steps=6)
+    else:
+        wl = WL[name]
+    a, b = P(wl, want_mask=False), P(wl, want_mask=False)
+    b.eng.set_overlap(0)
+    for t in range(min(wl.steps, 6)):
+        q, kn, vn, (qd, knd, vnd) = a.inputs(t)
+        a.eng.decode_step(a.st, qd, knd, vnd, wl.p, a.out, a.lse)
+        b.eng.decode_step(b.st, qd, knd, vnd, wl.p, b.out, b.lse)
+        a.ob.step(q, kn, vn, wl.p)
+        a.check_out(f"{name} step {t}")
+        for f in ("sel_count", "sel_idx", "sel_table", "votes", "probs", "sel_k_pool", "sel_v_pool", "cond_pos", "cond_k"):
+            assert torch.equal(getattr(a.st, f), getattr(b.st, f)), (t, f)
+        assert torch.equal(a.out, b.out) and torch.equal(a.lse, b.lse)
+    assert int(a.st.err_flag.item()) == 0 and int(b.st.err_flag.item()) == 0
