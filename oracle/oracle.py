@@ -14,7 +14,10 @@ from dataclasses import dataclass
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SO = os.path.join(_HERE, "libhardkv_oracle.so")
+# HARDKV_ORACLE_SANITIZE=1 (tests/test_oracle_sanitized.py): the same source built with AddressSanitizer + UBSan into a
+# second library; the process must run with libasan preloaded.
+_SANITIZE = os.environ.get("HARDKV_ORACLE_SANITIZE") == "1"
+_SO = os.path.join(_HERE, "libhardkv_oracle_asan.so" if _SANITIZE else "libhardkv_oracle.so")
 _SRC = os.path.join(_HERE, "hardkv_oracle.c")
 
 
@@ -23,8 +26,9 @@ def build(force: bool = False) -> str:
     if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < max(
         os.path.getmtime(_SRC), os.path.getmtime(os.path.join(_HERE, "hardkv_oracle.h"))
     ):
+        flags = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined"] if _SANITIZE else ["-O2"]
         subprocess.check_call(
-            ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-o", _SO, _SRC, "-lm"]
+            ["gcc", *flags, "-std=c11", "-fopenmp", "-fPIC", "-shared", "-Wall", "-o", _SO, _SRC, "-lm"]
         )
     return _SO
 
