@@ -644,7 +644,8 @@ def main():
                     "single-layer K fits L2, else 1)")
     ap.add_argument("--n0", type=int, default=0, help="override: uniform prefill context (config 3 checkpoints)")
     ap.add_argument("--variant", type=int, default=1, help="kernel variant (hardkv_set_variant): 0 generic FMA kernels, 1 tuned "
-                    "separate kernels (default), 2 TMA-staged score kernel, 3 fused persistent score -> select kernel")
+                    "separate kernels (default), 2 TMA-staged score kernel, 3 fused persistent score -> select kernel, 4 persistent score kernel with the select "
+                    "kernel co-resident behind it")
     ap.add_argument("--snapkv-window", type=int, default=0, help="odd window: odd KV heads use the SNAPKV max-pool metric "
                     "(L278) and the line reports the Algorithm 2 temperature solve; not the BASELINE workload")
     ap.add_argument("--contiguous-pages", action="store_true", help="diagnostic: identity page ids instead of the seeded "

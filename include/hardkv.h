@@ -117,7 +117,11 @@ const char   *hardkv_status_string(hardkv_status s);
 /* Kernel variant switch for A/B measurements: 0 = generic FMA kernels, 1 = tuned separate kernels,
  * 2 = the same with the TMA-staged (cp.async.bulk + mbarrier ring) persistent score kernel, 3 = score and selection
  * fused into one persistent kernel (bf16, no SNAPKV head, a unit's pool must fit one SM's shared memory:
- * HARDKV_ERR_UNSUPPORTED elsewhere).  Default 1 (3 measured slower on B200: DESIGN.md section 7). */
+ * HARDKV_ERR_UNSUPPORTED elsewhere), 4 = score || select: in hardkv_decode_step the persistent score kernel of variant 2
+ * streams the units longest pool first and publishes each one when its last chunk is scanned, and the select kernel,
+ * launched programmatically behind it and co-resident on the same SMs, selects a unit while later ones are still being
+ * scanned (bf16, no SNAPKV head, state without a query cache; elsewhere its stages run back to back as in variant 1).
+ * Default 1 (3 measured slower on B200: DESIGN.md section 7). */
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant);
 /* Geometry of the select kernel, for A/B measurements and tests: cluster = CTAs per (b, h) in {1, 2, 4, 8}, threads per
  * CTA in {512, 1024}; 0 keeps the automatic choice for that argument.  HARDKV_ERR_UNSUPPORTED when a CTA's slice of the

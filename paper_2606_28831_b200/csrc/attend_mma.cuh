@@ -46,7 +46,8 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   constexpr int NKC = D / 32;   // 64-byte chunks of a key row
   constexpr int NVC = D / 64;   // 128-byte chunks of a value row
   constexpr int ROWB = D * 2;
-  const int unit = P.wait_select ? P.unit_order[blockIdx.y] : (int)blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
+  const int unit = P.wait_select == 1 ? P.unit_order[blockIdx.y]
+                   : (P.wait_select == 2 ? P.unit_order[gridDim.y - 1 - blockIdx.y] : (int)blockIdx.y), b = unit / P.Hkv, h = unit % P.Hkv;
   if (P.wait_select) wait_unit_selected(P, unit);
   const int n = P.st.ctx_len[b];
   int s_end, r_lo;

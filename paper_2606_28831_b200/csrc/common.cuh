@@ -37,7 +37,9 @@ struct Params {
   int32_t *epoch;        // [1] decode steps appended so far: the append kernel bumps it, select publishes it per unit
   int32_t *sel_flag;     // [units] == *epoch once the unit's selection of this step is complete and visible
   int32_t *unit_order;   // [units] units by increasing pool length (the order their selections finish in)
-  int wait_select;       // attention launch: 1 = launched programmatically behind the select kernel: wait per unit
+  int wait_select;       // attention launch: 1 = launched programmatically behind the select kernel: wait per unit, units by
+                         // increasing pool length; 2 = the same behind the score || select pair: longest pool first
+  int32_t *score_flag;   // [units] == *epoch once every logit / chunk statistic of the unit is stored (score || select overlap)
   // query-cache form of the accumulated-attention metric (qcache_kernels.cuh)
   float2 *qc_stats;      // [units][score_chunks][256] per chunk and query row: (max, sum 2^(x - max)) of x = z log2(e) / T
   float2 *qc_final;      // [units][256] per query row: (max, 1 / (sum * G * n_c))
@@ -89,6 +91,23 @@ __device__ __forceinline__ void wait_unit_selected(const Params &P, int unit) {
       if (++polls > (1u << 24)) { atomicCAS(P.st.err_flag, 0, 120); break; }
     }
     __threadfence();    // acquire: the unit's sel_idx / sel_count / probs are visible to this CTA after the barrier
+  }
+  __syncthreads();
+}
+
+// Consumer side of the score || select overlap: the select kernel is launched programmatically behind the persistent
+// score kernel (every score CTA is resident before the first select CTA exists, and no score CTA ever waits for
+// anything, so the wait is deadlock-free) and takes a unit as soon as the score kernel has published it.
+__device__ __forceinline__ void wait_unit_scored(const Params &P, int unit) {
+  if (threadIdx.x == 0) {
+    const int want = *reinterpret_cast<volatile int32_t *>(P.epoch);
+    volatile int32_t *f = P.score_flag + unit;
+    unsigned polls = 0;
+    while (*f != want) {
+      __nanosleep(200);
+      if (++polls > (1u << 24)) { atomicCAS(P.st.err_flag, 0, 121); break; }
+    }
+    __threadfence();
   }
   __syncthreads();
 }

@@ -23,6 +23,7 @@ struct hardkv_ctx {
   int variant;
   int overlap;                   // 1 (default): the attention of a compression step starts while the select kernel runs
   int fused_ok;                  // the fused score -> select kernel applies to this config (score_select.cuh)
+  int overlap_ok;                // the co-resident score || select pair (variant 4) applies to this config
   unsigned long long *timing;    // hardkv_set_timing: per-launch (first CTA start, last CTA end), or NULL
   int timing_cap, timing_next;
   int pdl;                       // 1: launches carry the programmatic-stream-serialization attribute (hardkv_set_pdl)
@@ -56,7 +57,7 @@ WsLayout ws_layout(const hardkv_config &c) {
   size_t off = 0;
   w.arrive = off; off += align256(units * sizeof(int32_t));
   w.ss = off;     off += align256((units + 1) * sizeof(int32_t));
-  w.ovl = off;    off += align256((2 * units + 1) * sizeof(int32_t));   // sel_flag[units] | unit_order[units] | epoch
+  w.ovl = off;    off += align256((3 * units + 1) * sizeof(int32_t));   // sel_flag[units] | unit_order[units] | epoch | score_flag[units]
   w.part = off;   off += align256(units * att_chunks_of(c) * G * (c.head_dim + 2) * sizeof(float));
   w.stats = off;  off += align256(units * score_chunks_of(c) * 8 * sizeof(float2));
   const size_t qb = (size_t)c.batch * c.num_q_heads * c.head_dim, kb = units * c.head_dim;
@@ -232,8 +233,8 @@ void launch_score(hardkv_ctx *ctx, const Params &P0, const void *q, cudaStream_t
   dim3 grid(P.score_chunks, P.B * P.Hkv);
   if (fast_path(ctx) && ctx->variant == 2) {   // TMA-staged persistent variant (A/B: see DESIGN.md)
     const size_t smem = score_tma_smem(P.d, P.B * P.Hkv, P.B);
-    if (P.d == 128) score_tma_kernel<128><<<ctx->num_sms, SCORE_TMA_THREADS, smem, st>>>(P, q);
-    else score_tma_kernel<64><<<ctx->num_sms, SCORE_TMA_THREADS, smem, st>>>(P, q);
+    if (P.d == 128) score_tma_kernel<128, false><<<ctx->num_sms, SCORE_TMA_THREADS, smem, st>>>(P, q);
+    else score_tma_kernel<64, false><<<ctx->num_sms, SCORE_TMA_THREADS, smem, st>>>(P, q);
     return;
   }
   if (fast_path(ctx)) {
@@ -278,6 +279,54 @@ void launch_select(hardkv_ctx *ctx, const Params &P0, float p, int calibrate, cu
     else HK_SEL(0, 8);
   }
 #undef HK_SEL
+}
+
+// Geometry of the select kernel when it runs beside the publishing score kernel (variant 4): 512-thread CTAs, the
+// smallest cluster whose slice + scratch fit in the shared memory a score CTA leaves free on its SM.
+bool overlap_geometry(const hardkv_config &c, int *cluster, int *slice_cap) {
+  const int units = c.batch * c.num_kv_heads;
+  const int max_pool = c.max_ctx - c.recent > 0 ? c.max_ctx - c.recent : 1;
+  const size_t room = 227u * 1024u - score_tma_smem(c.head_dim, units, c.batch) - 2048 - 1024;  // static smem, per-CTA reserve
+  for (int C = 1; C <= SEL_MAXC; C <<= 1) {
+    const int cap = sel_slice_len(max_pool + 31, C, SEL_NT);
+    if ((size_t)cap * 4 + sizeof(SelShared) <= room) { *cluster = C; *slice_cap = cap; return true; }
+  }
+  return false;
+}
+bool overlap_eligible(const hardkv_config &c) {
+  int cl, cap;
+  return c.kv_dtype == HARDKV_BF16 && c.pool_kernel <= 1 && score_tma_smem(c.head_dim, c.batch * c.num_kv_heads, c.batch) < 200u * 1024u &&
+         overlap_geometry(c, &cl, &cap);
+}
+
+// stages 1 and 2a-2c as two co-resident kernels (variant 4): the persistent, publishing score kernel and, launched
+// programmatically behind it, the select kernel that takes every unit as soon as its last chunk is scanned
+void launch_score_select_overlapped(hardkv_ctx *ctx, const Params &P0, const void *q, float p, cudaStream_t st) {
+  {
+    const Params P = launch_params(ctx, P0);
+    ctx->launches += 1;
+    const size_t smem = score_tma_smem(P.d, P.B * P.Hkv, P.B);
+    if (P.d == 128) score_tma_kernel<128, true><<<ctx->num_sms, SCORE_TMA_THREADS, smem, st>>>(P, q);
+    else score_tma_kernel<64, true><<<ctx->num_sms, SCORE_TMA_THREADS, smem, st>>>(P, q);
+  }
+  Params P = launch_params(ctx, P0);
+  ctx->launches += 1;
+  overlap_geometry(ctx->cfg, &P.sel_cluster, &P.sel_slice_cap);
+  P.sel_nt = SEL_NT;
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3(P.B * P.Hkv * P.sel_cluster);
+  lc.blockDim = dim3(SEL_NT);
+  lc.dynamicSmemBytes = select_smem_bytes(P);
+  lc.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = P.sel_cluster; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  at[1].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[1].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at;
+  lc.numAttrs = 2;
+  if (P.G <= 4) cudaLaunchKernelEx(&lc, select_overlap_kernel<4>, P, p);
+  else cudaLaunchKernelEx(&lc, select_overlap_kernel<8>, P, p);
 }
 
 // stages 1 + 2a-2c as one persistent kernel, one CTA per SM (variant 3)
@@ -355,7 +404,7 @@ void launch_attend(hardkv_ctx *ctx, const Params &P0, const void *q, float *out,
   Params P = launch_params(ctx, P0);
   ctx->launches += 1;
   if (fast_path(ctx) && overlap) {
-    P.wait_select = 1;
+    P.wait_select = overlap;
     cudaLaunchConfig_t lc = {};
     lc.gridDim = dim3((P.att_chunks * ATT_CHUNK + ATT_MMA_CHUNK - 1) / ATT_MMA_CHUNK, P.B * P.Hkv);
     lc.blockDim = dim3(256); lc.dynamicSmemBytes = 0; lc.stream = st;
@@ -465,6 +514,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.sel_flag = reinterpret_cast<int32_t *>(base + w.ovl);
   P.unit_order = P.sel_flag + (size_t)cfg->batch * cfg->num_kv_heads;
   P.epoch = P.unit_order + (size_t)cfg->batch * cfg->num_kv_heads;
+  P.score_flag = P.epoch + 1;
   P.wait_select = 0;
   P.part = reinterpret_cast<float *>(base + w.part);
   P.score_stats = reinterpret_cast<float2 *>(base + w.stats);
@@ -486,8 +536,29 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
     const int ssm = (int)score_tma_smem(cfg->head_dim, cfg->batch * cfg->num_kv_heads, cfg->batch);
     static int score_smem_max = 0;
     if (ssm > score_smem_max) score_smem_max = ssm;
-    cudaFuncSetAttribute(score_tma_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
-    cudaFuncSetAttribute(score_tma_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
+    cudaFuncSetAttribute(score_tma_kernel<128, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
+    cudaFuncSetAttribute(score_tma_kernel<64, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
+    cudaFuncSetAttribute(score_tma_kernel<128, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
+    cudaFuncSetAttribute(score_tma_kernel<64, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, score_smem_max);
+    // the publishing kernel shares its SM with a select CTA: all of the SM's on-chip memory as shared memory
+    cudaFuncSetAttribute(score_tma_kernel<128, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+    cudaFuncSetAttribute(score_tma_kernel<64, true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  }
+  ctx->overlap_ok = overlap_eligible(*cfg) ? 1 : 0;
+  if (ctx->overlap_ok) {
+    static int so_smem_max = 0;
+    int cl, cap;
+    overlap_geometry(*cfg, &cl, &cap);
+    const int need = (int)((size_t)cap * 4 + sizeof(SelShared));
+    if (need > so_smem_max) so_smem_max = need;
+    const cudaFuncAttribute fa = cudaFuncAttributeMaxDynamicSharedMemorySize;
+    if (cudaFuncSetAttribute(select_overlap_kernel<4>, fa, so_smem_max) != cudaSuccess ||
+        cudaFuncSetAttribute(select_overlap_kernel<8>, fa, so_smem_max) != cudaSuccess ||
+        cudaFuncSetAttribute(select_overlap_kernel<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess ||
+        cudaFuncSetAttribute(select_overlap_kernel<8>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared) != cudaSuccess) {
+      cudaGetLastError();
+      ctx->overlap_ok = 0;
+    }
   }
   if (!raise_select_smem(P)) {
     cudaGetLastError();
@@ -515,8 +586,9 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
 void hardkv_destroy(hardkv_ctx *ctx) { delete ctx; }
 
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant) {
-  if (!ctx || variant < 0 || variant > 3) return HARDKV_ERR_INVALID_ARG;
+  if (!ctx || variant < 0 || variant > 4) return HARDKV_ERR_INVALID_ARG;
   if (variant == 3 && !ctx->fused_ok) return HARDKV_ERR_UNSUPPORTED;
+  if (variant == 4 && !ctx->overlap_ok) return HARDKV_ERR_UNSUPPORTED;
   ctx->variant = variant;
   return HARDKV_OK;
 }
@@ -598,7 +670,7 @@ hardkv_status hardkv_score_select(hardkv_ctx *ctx, const hardkv_state *s, const 
   const Params P = params_of(ctx, s);
   if (ctx->variant == 3 && !P.st.qcache) {
     launch_score_select(ctx, P, q, p, st);
-  } else {
+  } else {   // variant 4 needs the unit order of a preceding append in the same call: here its two kernels run back to back
     launch_score(ctx, P, q, st);
     launch_pool(ctx, P, st);
     launch_qcache_metric(ctx, P, st);
@@ -672,8 +744,12 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   const bool compress = do_select == HARDKV_STEP_SELECT_REWRITE || do_select == HARDKV_STEP_SELECT_SPARSE;
   launch_append(ctx, P, k_new, v_new, q, compress ? 1 : 0, st);   // between compressions: Step 1 only (L78, L274)
   launch_qcache_push(ctx, P, q, st);                              // the query window slides on every step (L448)
+  // variant 4 overlaps the two kernels through the unit order the append kernel of THIS call has just written
+  const bool ss_overlap = compress && ctx->variant == 4 && !P.st.qcache;
   if (compress && ctx->variant == 3 && !P.st.qcache) {
     launch_score_select(ctx, P, q, p, st);
+  } else if (ss_overlap) {
+    launch_score_select_overlapped(ctx, P, q, p, st);
   } else if (compress) {
     launch_score(ctx, P, q, st);
     launch_pool(ctx, P, st);
@@ -682,7 +758,7 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
     launch_select(ctx, P, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
   }
   // the select kernel (variants 1, 2: the last launch above) is followed by the attention of the same units: overlap them
-  const int overlap = compress && ctx->overlap && fast_path(ctx) && (ctx->variant == 1 || ctx->variant == 2);
+  const int overlap = ss_overlap ? 2 : (compress && ctx->overlap && fast_path(ctx) && ctx->variant != 3);
   launch_attend(ctx, P, q, out, lse, do_select == HARDKV_STEP_SELECT_REWRITE ? ATT_REWRITE
                                      : (do_select == HARDKV_STEP_REUSE_TIER ? ATT_TIER : ATT_SPARSE), st, overlap);
   return launch_status();

@@ -17,9 +17,10 @@
 namespace hardkv {
 
 #ifndef HARDKV_SCORE_STAGES
-#define HARDKV_SCORE_STAGES 40
+#define HARDKV_SCORE_STAGES 32
 #endif
-constexpr int SCORE_STAGES = HARDKV_SCORE_STAGES;   // pages in flight per SM (multiple of 8): 160 KiB at d = 128
+constexpr int SCORE_STAGES = HARDKV_SCORE_STAGES;   // pages in flight per SM (multiple of 8): 128 KiB at d = 128 (measured
+                                                    // flat from 24 stages up); leaves room for a co-resident select CTA
 constexpr int SCORE_CONSUMERS = 8;          // consumer warps
 constexpr int SCORE_PRODUCERS = 4;          // producer warps (one issuing lane each): a copy costs ~150 issue cycles
 constexpr int SCORE_TMA_THREADS = (SCORE_CONSUMERS + SCORE_PRODUCERS) * 32;
@@ -61,8 +62,14 @@ __host__ __device__ inline size_t score_tma_smem(int d, int units, int B) {
   return (size_t)SCORE_STAGES * PAGE * d * 2 + 2 * SCORE_STAGES * 8 + (size_t)(units + 1 + 2 * B) * 4 + 1024;
 }
 
-template <int D>
-__global__ void __launch_bounds__(SCORE_TMA_THREADS, 1) score_tma_kernel(Params P, const void *q_) {
+// PUBLISH (the score || select overlap of hardkv_decode_step, variant 4): the units are streamed longest pool first
+// (the reverse of unit_order), the kernel lets its dependent launch start at once, and the CTA that retires a unit's
+// last chunk publishes score_flag[unit] = *epoch -- the select kernel, co-resident on the same SMs (the register and
+// shared-memory budget of this kernel is held to half an SM for that), takes the unit while the stream goes on.
+template <int D, bool PUBLISH>
+__global__ void __launch_bounds__(SCORE_TMA_THREADS, 2) score_tma_kernel(Params P, const void *q_) {
+  if (PUBLISH) pdl_trigger();
+  KernelClock kclock(P);
   constexpr int NCH = D / 32;                 // 64-byte chunks per row
   constexpr int ROWB = D * 2, PAGEB = PAGE * ROWB;
   constexpr int SPC = SCORE_PAGES_PER_CTA;
@@ -89,10 +96,11 @@ __global__ void __launch_bounds__(SCORE_TMA_THREADS, 1) score_tma_kernel(Params 
   if (warp == 0) {   // exclusive prefix sum of the chunk counts of the units
     int run = 0;
     for (int u0 = 0; u0 < units; u0 += 32) {
-      const int u = u0 + lane;
+      const int u = u0 + lane;     // rank in the streaming order
       int cnt = 0;
       if (u < units) {
-        const int lo = s_lo[u / P.Hkv], hi = s_hi[u / P.Hkv];
+        const int uu = PUBLISH ? P.unit_order[units - 1 - u] : u;
+        const int lo = s_lo[uu / P.Hkv], hi = s_hi[uu / P.Hkv];
         if (hi > lo) cnt = ((hi - 1) >> 4) / SPC - (lo >> 4) / SPC + 1;
       }
       int inc = cnt;
@@ -118,10 +126,10 @@ __global__ void __launch_bounds__(SCORE_TMA_THREADS, 1) score_tma_kernel(Params 
       const int mid = (ul + uh + 1) >> 1;
       if (unit_first[mid] <= it) ul = mid; else uh = mid - 1;
     }
-    const int unit = ul, b = unit / P.Hkv, h = unit % P.Hkv;
+    const int unit = PUBLISH ? P.unit_order[units - 1 - ul] : ul, b = unit / P.Hkv, h = unit % P.Hkv;
     const int lo = s_lo[b], hi = s_hi[b];
     const int first_page = lo >> 4, last_page = (hi - 1) >> 4;
-    const int chunk = first_page / SPC + (it - unit_first[unit]);
+    const int chunk = first_page / SPC + (it - unit_first[ul]);
     const int pa = max(first_page, chunk * SPC), pb = min(last_page, chunk * SPC + SPC - 1);
     const int np = pb - pa + 1;
     const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
@@ -223,6 +231,22 @@ __global__ void __launch_bounds__(SCORE_TMA_THREADS, 1) score_tma_kernel(Params 
           }
         }
         P.score_stats[((size_t)unit * P.score_chunks + chunk) * 8 + g] = make_float2(m, sacc);
+      }
+      if (PUBLISH) {
+        // every logit of the item was stored before the consumer barrier above; the statistics by the 8 threads of
+        // warp 0, which lane 0 orders behind itself with the warp barrier; the fence is cumulative; then the ticket
+        if (warp == 0) {
+          __syncwarp();
+          if (lane == 0) {
+            __threadfence();
+            const int nch = last_page / SPC - first_page / SPC + 1;
+            if (atomicAdd(P.ss_arrive + unit, 1) == nch - 1) {
+              P.ss_arrive[unit] = 0;                 // re-arm for the next launch / graph replay
+              __threadfence();
+              *reinterpret_cast<volatile int32_t *>(P.score_flag + unit) = *reinterpret_cast<volatile int32_t *>(P.epoch);
+            }
+          }
+        }
       }
     }
     nbase += np;

@@ -706,4 +706,23 @@ __global__ void __launch_bounds__(NT, NT == SEL_NT_BIG ? 1 : 2) select_kernel(Pa
   select_unit<CALIBRATE, GMAX, NT, true, false>(P, p, blockIdx.x / P.sel_cluster, pbits, sh);
 }
 
+// The select half of the score || select overlap (hardkv_decode_step, variant 4): launched programmatically behind the
+// publishing score_tma_kernel; cluster j takes the unit the score kernel finishes j-th (longest pool first), waits for
+// its flag and reads the logits / chunk statistics with L2-coherent loads.  512-thread CTAs whose shared memory and
+// registers fit beside a score CTA on the same SM.
+template <int GMAX>
+__global__ void __launch_bounds__(SEL_NT, 2) select_overlap_kernel(Params P, float p) {
+  pdl_trigger();
+  KernelClock kclock(P);
+  extern __shared__ __align__(16) unsigned char sel_smem[];
+  uint32_t *pbits = reinterpret_cast<uint32_t *>(sel_smem);
+  SelShared &sh = *reinterpret_cast<SelShared *>(sel_smem + (size_t)P.sel_slice_cap * 4);
+  const int units = P.B * P.Hkv;
+  const int unit = P.unit_order[units - 1 - (int)blockIdx.x / P.sel_cluster];
+  int n, lo, hi;
+  pool_bounds(P, unit / P.Hkv, n, lo, hi);
+  if (hi > lo) wait_unit_scored(P, unit);     // an empty pool has no chunk: nothing is published for it
+  select_unit<2, GMAX, SEL_NT, true, true>(P, p, unit, pbits, sh);
+}
+
 }  // namespace hardkv

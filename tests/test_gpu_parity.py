@@ -161,19 +161,20 @@ def test_fused_decode_step(name, teacher, P):
           f"first divergence step {first_div}, max-abs output error over the run {emax:.2e}")
 
 
-@pytest.mark.parametrize("variant", [0, 2, 3])
+@pytest.mark.parametrize("variant", [0, 2, 3, 4])
 @pytest.mark.parametrize("name", ["c1s", "c2s", "c3s", "c4s", "g1d64", "snap4"])
 def test_kernel_variants(name, variant, P):
-    """Variant 0 (generic fp32-FMA kernels), 2 (TMA-staged persistent score) and 3 (score and selection fused into one
-    persistent kernel: CTAs stream K pages and the CTA that retires a unit's last chunk runs its selection) against the
-    oracle; the default is variant 1.  Variant 3 does not apply to configs with SNAPKV heads (the pooling pass sits
+    """Variant 0 (generic fp32-FMA kernels), 2 (TMA-staged persistent score), 3 (score and selection fused into one
+    persistent kernel: CTAs stream K pages and the CTA that retires a unit's last chunk runs its selection) and 4 (the
+    publishing persistent score kernel with the select kernel co-resident behind it, longest unit first) against the
+    oracle; the default is variant 1.  Variants 3 and 4 do not apply to configs with SNAPKV heads (the pooling pass sits
     between score and select)."""
     from paper_2606_28831_b200 import hardkv
     wl = WL[name]
     pr = P(wl, want_mask=False)
-    if variant == 3 and wl.pool_kernel > 1:
+    if variant in (3, 4) and wl.pool_kernel > 1:
         with pytest.raises(hardkv.HardKVError):
-            pr.eng.set_variant(3)
+            pr.eng.set_variant(variant)
         return
     pr.eng.set_variant(variant)
     for t in range(min(wl.steps, 8)):
