@@ -13,6 +13,7 @@
 #include "attend_mma.cuh"
 #include "metric_kernels.cuh"
 #include "qcache_kernels.cuh"
+#include "qcache_umma.cuh"
 #include "score_select.cuh"
 
 using namespace hardkv;
@@ -360,9 +361,25 @@ void launch_qcache_metric(hardkv_ctx *ctx, const Params &P0, cudaStream_t st) {
     attr_set = true;
   }
   ctx->launches += 3;
+  // tcgen05 / TMEM kernels (qcache_umma.cuh); variant 0 keeps the mma.sync kernels for A/B
+  const bool umma = ctx->variant != 0;
+  const dim3 grid_u((P0.score_chunks + QU_CPC - 1) / QU_CPC, P0.B * P0.Hkv);
+  const size_t smu = qcache_umma_smem(P0.d);
+  static bool attr_u = false;
+  if (umma && !attr_u) {
+    const int mx = (int)qcache_umma_smem(128);
+    cudaFuncSetAttribute(qcache_umma_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+    cudaFuncSetAttribute(qcache_umma_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+    cudaFuncSetAttribute(qcache_umma_kernel<64, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+    cudaFuncSetAttribute(qcache_umma_kernel<64, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
+    attr_u = true;
+  }
   {
     const Params P = launch_params(ctx, P0);
-    if (P.d == 128) qcache_pass_kernel<128, 1><<<grid, 256, sm1, st>>>(P);
+    if (umma) {
+      if (P.d == 128) qcache_umma_kernel<128, 1><<<grid_u, QU_THREADS, smu, st>>>(P);
+      else qcache_umma_kernel<64, 1><<<grid_u, QU_THREADS, smu, st>>>(P);
+    } else if (P.d == 128) qcache_pass_kernel<128, 1><<<grid, 256, sm1, st>>>(P);
     else qcache_pass_kernel<64, 1><<<grid, 256, sm1, st>>>(P);
   }
   {
@@ -371,7 +388,10 @@ void launch_qcache_metric(hardkv_ctx *ctx, const Params &P0, cudaStream_t st) {
   }
   {
     const Params P = launch_params(ctx, P0);
-    if (P.d == 128) qcache_pass_kernel<128, 2><<<grid, 256, sm2, st>>>(P);
+    if (umma) {
+      if (P.d == 128) qcache_umma_kernel<128, 2><<<grid_u, QU_THREADS, smu, st>>>(P);
+      else qcache_umma_kernel<64, 2><<<grid_u, QU_THREADS, smu, st>>>(P);
+    } else if (P.d == 128) qcache_pass_kernel<128, 2><<<grid, 256, sm2, st>>>(P);
     else qcache_pass_kernel<64, 2><<<grid, 256, sm2, st>>>(P);
   }
 }

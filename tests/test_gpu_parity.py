@@ -43,6 +43,12 @@ def small_workloads():
                              score_mode=np.array([0, 3, 3, 0, 3, 0, 3, 3], np.uint8), accum_window=4),
         "qc5": make_workload(4, B=2, n0=i32(1500, 1500), max_ctx=1600, k_cap=384, l_upper=i32(1390, 1390),
                              cond_cap=16, accum_window=6, steps=9, score_mode=np.array([0, 3, 0, 1, 3, 1, 3, 3], np.uint8)),
+        # the tensor-core (tcgen05) form of the same metric at its other shapes: more than 128 query rows (20 cached steps
+        # x G = 8 = 160 -> the 256-row block) over a pool of several 128-token tiles and both chunk slots of a CTA; d = 64
+        "qc8w": make_workload(1, Hq=16, Hkv=2, n0=i32(3300), max_ctx=3408, k_cap=512, l_upper=i32(3100), cond_cap=16,
+                              steps=24, score_mode=np.array([3, 3], np.uint8), accum_window=20),
+        "qc64": make_workload(1, Hq=8, Hkv=2, d=64, n0=i32(1900), max_ctx=1936, k_cap=256, l_upper=i32(1700), cond_cap=8,
+                              steps=10, score_mode=np.array([3, 0], np.uint8), accum_window=8),
         "g8": make_workload(1, Hq=8, Hkv=1, n0=i32(1100), max_ctx=1120, k_cap=1120, l_upper=i32(5000), cond_cap=0,
                             steps=3),
     }
