@@ -362,12 +362,12 @@ void launch_qcache_metric(hardkv_ctx *ctx, const Params &P0, cudaStream_t st) {
   }
   ctx->launches += 3;
   // tcgen05 / TMEM kernels (qcache_umma.cuh); variant 0 keeps the mma.sync kernels for A/B
-  const bool umma = ctx->variant != 0;
-  const dim3 grid_u((P0.score_chunks + QU_CPC - 1) / QU_CPC, P0.B * P0.Hkv);
-  const size_t smu = qcache_umma_smem(P0.d);
+  const bool umma = ctx->variant != 0 && P0.B * P0.Hkv <= QU_MAX_UNITS;
+  const dim3 grid_u(ctx->num_sms);
+  const size_t smu = qcache_umma_smem(P0.d, qcache_umma_rows(P0.accum_window, P0.G));
   static bool attr_u = false;
   if (umma && !attr_u) {
-    const int mx = (int)qcache_umma_smem(128);
+    const int mx = (int)(qcache_umma_smem(128, 256) < 216u * 1024u ? qcache_umma_smem(128, 256) : 216u * 1024u);
     cudaFuncSetAttribute(qcache_umma_kernel<128, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
     cudaFuncSetAttribute(qcache_umma_kernel<128, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);
     cudaFuncSetAttribute(qcache_umma_kernel<64, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, mx);

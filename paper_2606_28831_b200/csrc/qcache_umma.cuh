@@ -29,14 +29,28 @@
 namespace hardkv {
 
 constexpr int QU_TILE = 128;            // pool tokens per tile (8 pages)
-constexpr int QU_STAGES = 4;            // K tiles in shared memory
-constexpr int QU_LAG = 2;               // a producer signals tile t - QU_LAG after issuing tile t: 3 tiles in flight
-constexpr int QU_CPC = 2;               // score chunks (of 64 pages) per CTA
-constexpr int QU_EPI_THREADS = 256, QU_MMA_WARP = 8, QU_PROD_THREADS = 128;
+#ifndef HARDKV_QU_STAGES
+#define HARDKV_QU_STAGES 4
+#endif
+#ifndef HARDKV_QU_LAG
+#define HARDKV_QU_LAG 2
+#endif
+#ifndef HARDKV_QU_CPC
+#define HARDKV_QU_CPC 4
+#endif
+constexpr int QU_STAGES = HARDKV_QU_STAGES;   // K tiles in shared memory
+constexpr int QU_LAG = HARDKV_QU_LAG;         // a producer signals tile t - QU_LAG after issuing tile t: QU_LAG + 1 tiles in flight
+constexpr int QU_CPC = HARDKV_QU_CPC;         // score chunks (of 64 pages) per CTA
+#ifndef HARDKV_QU_PROD
+#define HARDKV_QU_PROD 128
+#endif
+constexpr int QU_EPI_THREADS = 256, QU_MMA_WARP = 8, QU_PROD_THREADS = HARDKV_QU_PROD;
 constexpr int QU_THREADS = QU_EPI_THREADS + 32 + QU_PROD_THREADS;
 
-__host__ __device__ inline size_t qcache_umma_smem(int d) {
-  return (size_t)QU_STAGES * QU_TILE * d * 2 + (size_t)QC_ROWS * d * 2 + 2 * QC_ROWS * sizeof(float2) + 256 + 1024;
+// rows = the query block's capacity for this config: 128 or 256 (accum_window * G rounded up to the MMA shape)
+__host__ __device__ inline int qcache_umma_rows(int accum_window, int G) { return accum_window * G <= 128 ? 128 : 256; }
+__host__ __device__ inline size_t qcache_umma_smem(int d, int rows) {
+  return (size_t)QU_STAGES * QU_TILE * d * 2 + (size_t)rows * d * 2 + 1024;   // + 4.2 KB static (statistics, barriers)
 }
 
 // UMMA shared-memory descriptor: K-major, SWIZZLE_128B, 8-row groups 1024 B apart (version 1 = sm_100)
@@ -81,43 +95,64 @@ __device__ __forceinline__ uint32_t umma_sw128_off(int r, int g, int rows) {
   return (uint32_t)((g >> 3) * (rows * 128) + (r >> 3) * 1024 + (r & 7) * 128 + (((g & 7) ^ (r & 7)) << 4));
 }
 
-// PASS 1: per-(CTA, query row) softmax statistics -> qc_stats; PASS 2: probabilities summed over the query rows -> probs.
+
+constexpr int QU_MAX_UNITS = 1024;      // capacity of the per-CTA item index (units beyond it: the mma.sync kernels run instead)
+
+// One work item = one score chunk (64 pages = up to 8 tiles) of one query-cache unit.
+struct QuItem {
+  int unit, b, h, chunk, lo, hi, pgA, pgB, tile_pg0, T, M, RB;
+};
+
+// PASS 1: per-(chunk, query row) softmax statistics -> qc_stats; PASS 2: probabilities summed over the query rows -> probs.
+// Persistent: one CTA per SM walks the items blockIdx.x, blockIdx.x + gridDim.x, ...; the K-tile ring and the TMEM
+// accumulator stages run on across items (a global tile counter gives stage and parity), only the query block of the
+// unit is reloaded per item, by the epilogue warps, while the producers already fetch the item's first tiles.
 template <int D, int PASS>
 __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
   KernelClock kclock(P);
   constexpr int ROWB = D * 2, CPR = D / 8, KSTEPS = D / 16;
   constexpr int TILEB = QU_TILE * ROWB;
+  constexpr int SPC = SCORE_PAGES_PER_CTA;
   extern __shared__ __align__(1024) unsigned char qu_raw[];
-  const int unit = blockIdx.y, b = unit / P.Hkv, h = unit % P.Hkv;
-  if (P.st.score_mode[h] != HARDKV_SCORE_ACCUM_QCACHE) return;
-  int n, lo, hi;
-  pool_bounds(P, b, n, lo, hi);
-  if (hi <= lo) return;
-  const int first_page = lo >> 4, last_page = (hi - 1) >> 4;
-  const int cpg0 = blockIdx.x * (QU_CPC * SCORE_PAGES_PER_CTA);                 // first page of this CTA's range
-  const int pgA = max(first_page, cpg0), pgB = min(last_page, cpg0 + QU_CPC * SCORE_PAGES_PER_CTA - 1);
-  if (pgA > pgB) return;
-  const int tile_pg0 = cpg0 + ((pgA - cpg0) & ~7);                              // tiles are 8-page aligned
-  const int T = (pgB - tile_pg0) / 8 + 1;
-
   unsigned char *smem = reinterpret_cast<unsigned char *>((reinterpret_cast<uintptr_t>(qu_raw) + 1023) & ~(uintptr_t)1023);
   unsigned char *ktile = smem;                                                  // [QU_STAGES][TILEB]
-  unsigned char *qblk = smem + (size_t)QU_STAGES * TILEB;                       // [RB rows], swizzled
-  float2 *s_aux = reinterpret_cast<float2 *>(qblk + (size_t)QC_ROWS * ROWB);    // PASS 1: [2][QC_ROWS] statistics of the two
-                                                                                // warpgroups; PASS 2: [QC_ROWS] (max, weight)
-  uint64_t *full = reinterpret_cast<uint64_t *>(s_aux + 2 * QC_ROWS);
-  uint64_t *empty = full + QU_STAGES, *tfull = empty + QU_STAGES, *tempty = tfull + 2;
-  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
+  unsigned char *qblk = smem + (size_t)QU_STAGES * TILEB;                       // [RBmax rows], swizzled
+  __shared__ __align__(16) float2 s_aux[2 * QC_ROWS];   // PASS 1: [2][QC_ROWS] statistics of the two warpgroups; PASS 2: (max, weight)
+  __shared__ uint64_t full[QU_STAGES], empty[QU_STAGES], tfull[4], tempty[4];
+  __shared__ uint32_t tmem_slot[1];
+  __shared__ int s_first[QU_MAX_UNITS + 1];             // first item of every unit (exclusive prefix sum of the chunk counts)
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int G = P.G, nc = P.st.qc_count[b];
-  const int M = nc * G, RB = M <= 128 ? 128 : 256;                              // query rows, padded to the MMA shape
-  const uint32_t tmem_cols = 2 * RB;                                            // two accumulator stages
+  const int units = P.B * P.Hkv, G = P.G;
+  const int RBmax = qcache_umma_rows(P.accum_window, G);
+  const int NACC = 512 / RBmax;                                                 // accumulator stages in TMEM: 4 or 2
+  const uint32_t tmem_cols = 512;
 
   if (tid == 0) {
     for (int s = 0; s < QU_STAGES; ++s) { mbar_init(&full[s], QU_PROD_THREADS); mbar_init(&empty[s], 1); }
-    for (int a = 0; a < 2; ++a) { mbar_init(&tfull[a], 1); mbar_init(&tempty[a], 128); }
+    for (int a = 0; a < 4; ++a) { mbar_init(&tfull[a], 1); mbar_init(&tempty[a], 128); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  if (warp == 0) {   // chunk counts of the units -> exclusive prefix sum
+    int run = 0;
+    for (int u0 = 0; u0 < units; u0 += 32) {
+      const int u = u0 + lane;
+      int cnt = 0;
+      if (u < units && P.st.score_mode[u % P.Hkv] == HARDKV_SCORE_ACCUM_QCACHE) {
+        int n, lo, hi;
+        pool_bounds(P, u / P.Hkv, n, lo, hi);
+        if (hi > lo) cnt = ((hi - 1) >> 4) / SPC - (lo >> 4) / SPC + 1;
+      }
+      int inc = cnt;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const int t_ = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t_;
+      }
+      if (u < units) s_first[u] = run + inc - cnt;
+      run += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane == 0) s_first[units] = run;
   }
   if (warp == QU_MMA_WARP) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(tmem_slot)), "r"(tmem_cols));
@@ -127,75 +162,103 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
-  const float c2 = P.sm_scale * 1.4426950408889634f / P.st.temperature[unit];   // logit -> base-2 exponent of z / T
+  const int nitems = s_first[units];
+  // a CTA takes a contiguous block of items: consecutive chunks of (mostly) one unit, so the query block is reloaded once
+  // or twice per CTA, not per item; items are equal-sized up to the units' partial first / last chunks
+  const int it_begin = (int)(((long long)blockIdx.x * nitems) / gridDim.x);
+  const int it_end = (int)(((long long)(blockIdx.x + 1) * nitems) / gridDim.x);
+
+  auto decode = [&](int it, QuItem &I) {
+    int ul = 0, uh = units - 1;
+    while (ul < uh) {
+      const int mid = (ul + uh + 1) >> 1;
+      if (s_first[mid] <= it) ul = mid; else uh = mid - 1;
+    }
+    I.unit = ul; I.b = ul / P.Hkv; I.h = ul % P.Hkv;
+    int n;
+    pool_bounds(P, I.b, n, I.lo, I.hi);
+    const int first_page = I.lo >> 4, last_page = (I.hi - 1) >> 4;
+    I.chunk = first_page / SPC + (it - s_first[ul]);
+    const int cpg0 = I.chunk * SPC;
+    I.pgA = max(first_page, cpg0); I.pgB = min(last_page, cpg0 + SPC - 1);
+    I.tile_pg0 = cpg0 + ((I.pgA - cpg0) & ~7);                                  // tiles are 8-page aligned
+    I.T = (I.pgB - I.tile_pg0) / 8 + 1;
+    I.M = P.st.qc_count[I.b] * G;
+    I.RB = I.M <= 128 ? 128 : 256;                                              // query rows, padded to the MMA shape
+  };
 
   if (warp > QU_MMA_WARP) {
-    // ================= producers: gather the pages of tile t into stage t % QU_STAGES =================
+    // ================= producers: gather the pages of every tile into the ring, LAG + 1 tiles in flight =================
     const int p = tid - (QU_EPI_THREADS + 32);
     const int g = p % CPR, rsub = p / CPR;
     constexpr int RPI = QU_PROD_THREADS / CPR;                                  // rows per iteration (8 at d = 128)
-    const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
     const char *kpool = reinterpret_cast<const char *>(P.st.k_pool);
-    for (int t = 0; t < T; ++t) {
-      const int s = t % QU_STAGES;
-      mbar_wait(&empty[s], ((t / QU_STAGES) & 1) ^ 1);                          // the MMAs that read the stage have completed
-      const int pg = tile_pg0 + 8 * t + (lane & 7);
-      const int pid = (pg >= pgA && pg <= pgB) ? __ldg(tab + pg) : -1;           // pages outside the pool are not fetched: their
-      const uint32_t dst0 = smem_u32(ktile + (size_t)s * TILEB);                //  rows hold stale data, masked in the epilogue
+    // the physical ids of an item's (<= 64) pages with one coalesced load per 32 pages, fetched one item ahead; pages
+    // outside the pool are not fetched (their rows hold stale data, masked in the epilogue)
+    auto page_ids = [&](const QuItem &I, int &p0, int &p1) {
+      const int32_t *tab = P.st.base_table + (size_t)I.unit * P.ppu;
+      const int pg = I.tile_pg0 + lane;
+      p0 = (pg >= I.pgA && pg <= I.pgB) ? __ldg(tab + pg) : -1;
+      p1 = (pg + 32 >= I.pgA && pg + 32 <= I.pgB) ? __ldg(tab + pg + 32) : -1;
+    };
+    QuItem I, In;
+    int pid0 = -1, pid1 = -1, np0 = -1, np1 = -1;
+    int it = it_begin, gi = 0;
+    if (it < it_end) { decode(it, I); page_ids(I, pid0, pid1); }
+    while (it < it_end) {
+      const int itn = it + 1;
+      if (itn < it_end) { decode(itn, In); page_ids(In, np0, np1); }
+      for (int t = 0; t < I.T; ++t, ++gi) {
+        const int s = gi % QU_STAGES;
+        mbar_wait(&empty[s], ((gi / QU_STAGES) & 1) ^ 1);                       // the MMAs that read the stage have completed
+        const int pidw = (t >> 2) ? pid1 : pid0;
+        const uint32_t dst0 = smem_u32(ktile + (size_t)s * TILEB);
 #pragma unroll
-      for (int i = 0; i < QU_TILE / RPI; ++i) {
-        const int row = i * RPI + rsub;
-        const int page = __shfl_sync(0xffffffffu, pid, row >> 4);
-        if (page >= 0)
-          cp_async16(dst0 + umma_sw128_off(row, g, QU_TILE), kpool + ((size_t)page * PAGE + (row & 15)) * ROWB + g * 16);
-      }
-      asm volatile("cp.async.commit_group;" ::: "memory");
-      if (t >= QU_LAG) {
-        cp_async_wait<QU_LAG>();
-        proxy_fence_async();
-        mbar_arrive(&full[(t - QU_LAG) % QU_STAGES]);
-      }
-    }
-    // drain: the last min(T, QU_LAG) tiles
-    if (T >= 2) { cp_async_wait<1>(); proxy_fence_async(); mbar_arrive(&full[(T - 2) % QU_STAGES]); }
-    cp_async_wait<0>(); proxy_fence_async(); mbar_arrive(&full[(T - 1) % QU_STAGES]);
-  } else {
-    // ================= the query block -> shared memory (epilogue warps), rows beyond M are zero =================
-    if (warp < QU_MMA_WARP) {
-      const char *qc = reinterpret_cast<const char *>(P.st.qcache);
-      for (int i = tid; i < RB * CPR; i += QU_EPI_THREADS) {
-        const int r = i / CPR, gq = i % CPR;
-        uint4 val = make_uint4(0, 0, 0, 0);
-        if (r < M) {
-          const int tau = r / G, gh = r % G;
-          val = ldg_ca(qc + (((size_t)(b * P.Hq + h * G + gh) * P.accum_window + tau) * D) * 2 + gq * 16);
+        for (int i = 0; i < QU_TILE / RPI; ++i) {
+          const int row = i * RPI + rsub;
+          const int page = __shfl_sync(0xffffffffu, pidw, (t & 3) * 8 + (row >> 4));
+          if (page >= 0)
+            cp_async16(dst0 + umma_sw128_off(row, g, QU_TILE), kpool + ((size_t)page * PAGE + (row & 15)) * ROWB + g * 16);
         }
-        *reinterpret_cast<uint4 *>(qblk + umma_sw128_off(r, gq, RB)) = val;
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        if (gi >= QU_LAG) {
+          cp_async_wait<QU_LAG>();
+          proxy_fence_async();
+          mbar_arrive(&full[(gi - QU_LAG) % QU_STAGES]);
+        }
       }
-      if (PASS == 2) {
-        const float2 *fin = P.qc_final + (size_t)unit * QC_ROWS;
-        for (int i = tid; i < QC_ROWS; i += QU_EPI_THREADS) s_aux[i] = fin[i];
-      }
-      proxy_fence_async();
+      I = In; pid0 = np0; pid1 = np1; it = itn;
     }
-    asm volatile("bar.sync 1, %0;" ::"n"(QU_EPI_THREADS + 32) : "memory");      // epilogue warps + the MMA warp
-    if (warp == QU_MMA_WARP) {
-      // ================= MMA issue: one thread =================
-      const uint32_t qaddr = smem_u32(qblk);
-      for (int t = 0; t < T; ++t) {
-        const int s = t % QU_STAGES, a = t & 1;
-        mbar_wait(&full[s], (t / QU_STAGES) & 1);                               // the tile has landed
-        mbar_wait(&tempty[a], ((t >> 1) & 1) ^ 1);                              // the epilogue has drained the accumulator stage
+    // drain: the last min(gi, QU_LAG) tiles
+    if (QU_LAG >= 3 && gi >= 3) { cp_async_wait<2>(); proxy_fence_async(); mbar_arrive(&full[(gi - 3) % QU_STAGES]); }
+    if (QU_LAG >= 2 && gi >= 2) { cp_async_wait<1>(); proxy_fence_async(); mbar_arrive(&full[(gi - 2) % QU_STAGES]); }
+    if (gi >= 1) { cp_async_wait<0>(); proxy_fence_async(); mbar_arrive(&full[(gi - 1) % QU_STAGES]); }
+  } else if (warp == QU_MMA_WARP) {
+    // ================= MMA issue: one thread =================
+    const uint32_t qaddr = smem_u32(qblk);
+    QuItem I;
+    int gi = 0, prev_unit = -1;
+    for (int it = it_begin; it < it_end; ++it) {
+      decode(it, I);
+      if (I.unit != prev_unit)
+        asm volatile("bar.sync 1, %0;" ::"n"(QU_EPI_THREADS + 32) : "memory");  // the unit's query block is in shared memory
+      prev_unit = I.unit;
+      const int RB = I.RB;
+      for (int t = 0; t < I.T; ++t, ++gi) {
+        const int s = gi % QU_STAGES, a = gi % NACC;
+        mbar_wait(&full[s], (gi / QU_STAGES) & 1);                              // the tile has landed
+        mbar_wait(&tempty[a], ((gi / NACC) & 1) ^ 1);                           // the epilogue has drained the accumulator stage
         tc_fence_after();
         proxy_fence_async();
         if (lane == 0) {
           const uint32_t kaddr = smem_u32(ktile + (size_t)s * TILEB);
+          const uint32_t dcol = tmem + a * RBmax;
           if (PASS == 1) {
             for (int rh = 0; rh < RB / 128; ++rh) {
 #pragma unroll
               for (int kk = 0; kk < KSTEPS; ++kk) {
                 const uint32_t o = (uint32_t)((kk & 3) * 32);
-                umma_bf16(tmem + a * RB + rh * 128, umma_desc(qaddr + (kk >> 2) * (RB * 128) + rh * 16384 + o),
+                umma_bf16(dcol + rh * 128, umma_desc(qaddr + (kk >> 2) * (RB * 128) + rh * 16384 + o),
                           umma_desc(kaddr + (kk >> 2) * (QU_TILE * 128) + o), umma_idesc_bf16(QU_TILE), kk > 0);
               }
             }
@@ -203,7 +266,7 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
 #pragma unroll
             for (int kk = 0; kk < KSTEPS; ++kk) {
               const uint32_t o = (uint32_t)((kk & 3) * 32);
-              umma_bf16(tmem + a * RB, umma_desc(kaddr + (kk >> 2) * (QU_TILE * 128) + o),
+              umma_bf16(dcol, umma_desc(kaddr + (kk >> 2) * (QU_TILE * 128) + o),
                         umma_desc(qaddr + (kk >> 2) * (RB * 128) + o), umma_idesc_bf16(RB), kk > 0);
             }
           }
@@ -212,35 +275,75 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
         }
         __syncwarp();
       }
-    } else {
-      // ================= epilogue: warpgroup a drains accumulator stage a (tiles a, a + 2, ...) =================
-      const int a = warp >> 2, quad = warp & 3;
-      const uint32_t tlane = (uint32_t)(quad * 32) << 16;
+    }
+  } else {
+    // ================= epilogue: warpgroup wg drains the tiles of its parity =================
+    const int wg = warp >> 2, quad = warp & 3;
+    const uint32_t tlane = (uint32_t)(quad * 32) << 16;
+    const char *qc = reinterpret_cast<const char *>(P.st.qcache);
+    QuItem I;
+    int gi = 0, prev_unit = -1;
+    for (int it = it_begin; it < it_end; ++it) {
+      decode(it, I);
+      const int M = I.M, RB = I.RB, lo = I.lo, hi = I.hi;
+      if (I.unit != prev_unit) {
+        // both warpgroups are through with the previous unit: all of its MMAs have completed, the query block and (pass 2)
+        // s_aux are free
+        asm volatile("bar.sync 2, %0;" ::"n"(QU_EPI_THREADS) : "memory");
+        for (int i = tid; i < RB * CPR; i += QU_EPI_THREADS) {                  // the unit's query block; rows beyond M are zero
+          const int r = i / CPR, gq = i % CPR;
+          uint4 val = make_uint4(0, 0, 0, 0);
+          if (r < M) {
+            const int tau = r / G, gh = r % G;
+            val = ldg_ca(qc + (((size_t)(I.b * P.Hq + I.h * G + gh) * P.accum_window + tau) * D) * 2 + gq * 16);
+          }
+          *reinterpret_cast<uint4 *>(qblk + umma_sw128_off(r, gq, RB)) = val;
+        }
+        if (PASS == 2) {
+          const float2 *fin = P.qc_final + (size_t)I.unit * QC_ROWS;
+          for (int i = tid; i < QC_ROWS; i += QU_EPI_THREADS) s_aux[i] = fin[i];
+        }
+        proxy_fence_async();
+        asm volatile("bar.sync 1, %0;" ::"n"(QU_EPI_THREADS + 32) : "memory");  // with the MMA warp
+      }
+      prev_unit = I.unit;
+      const float c2 = P.sm_scale * 1.4426950408889634f / P.st.temperature[I.unit];   // logit -> base-2 exponent of z / T
       if (PASS == 1) {
-        float m0 = -INFINITY, s0 = 0.f, m1 = -INFINITY, s1 = 0.f;              // rows quad * 32 + lane and + 128
-        for (int t = a; t < T; t += 2) {
-          mbar_wait(&tfull[a], (t >> 1) & 1);
+        float m0 = -INFINITY, s0 = 0.f, m1 = -INFINITY, s1 = 0.f;              // rows quad * 32 + lane and + 128 (logit units)
+        for (int t = 0; t < I.T; ++t) {
+          const int gt = gi + t;
+          if ((gt & 1) != wg) continue;
+          const int a = gt % NACC;
+          mbar_wait(&tfull[a], (gt / NACC) & 1);
           tc_fence_after();
-          const int tok0 = (tile_pg0 + 8 * t) * PAGE;
+          const int tok0 = (I.tile_pg0 + 8 * t) * PAGE;
           for (int rh = 0; rh < RB / 128; ++rh) {
             float m = rh ? m1 : m0, sacc = rh ? s1 : s0;
 #pragma unroll 1
             for (int c0 = 0; c0 < QU_TILE; c0 += 32) {
               float v[32];
-              tmem_ld32(tmem + tlane + a * RB + rh * 128 + c0, v);
+              tmem_ld32(tmem + tlane + a * RBmax + rh * 128 + c0, v);
               const int tk = tok0 + c0;
-              const bool inside = tk >= lo && tk + 32 <= hi;
-              float mx = m;
+              if (!(tk >= lo && tk + 32 <= hi)) {                               // warp-uniform: only the pool's first / last tile
 #pragma unroll
-              for (int j = 0; j < 32; ++j) {
-                v[j] = (inside || (tk + j >= lo && tk + j < hi)) ? v[j] * c2 : -INFINITY;
-                mx = fmaxf(mx, v[j]);
+                for (int j = 0; j < 32; ++j) v[j] = (tk + j >= lo && tk + j < hi) ? v[j] : -INFINITY;
               }
-              if (mx != -INFINITY) {
-                float acc = 0.f;
+              // m is kept in logit units (c2 > 0: the maximum commutes with the scale); four independent chains
+              float x0 = fmaxf(v[0], v[1]), x1 = fmaxf(v[2], v[3]), x2 = fmaxf(v[4], v[5]), x3 = fmaxf(v[6], v[7]);
 #pragma unroll
-                for (int j = 0; j < 32; ++j) acc += fast_exp2(v[j] - mx);
-                sacc = sacc * fast_exp2(m - mx) + acc;
+              for (int j = 8; j < 32; j += 4) {
+                x0 = fmaxf(x0, v[j]); x1 = fmaxf(x1, v[j + 1]); x2 = fmaxf(x2, v[j + 2]); x3 = fmaxf(x3, v[j + 3]);
+              }
+              const float mx = fmaxf(fmaxf(fmaxf(x0, x1), fmaxf(x2, x3)), m);
+              if (mx != -INFINITY) {
+                const float nb = -mx * c2;
+                float a0 = 0.f, a1 = 0.f, a2 = 0.f, a3 = 0.f;
+#pragma unroll
+                for (int j = 0; j < 32; j += 4) {
+                  a0 += fast_exp2(fmaf(v[j], c2, nb)); a1 += fast_exp2(fmaf(v[j + 1], c2, nb));
+                  a2 += fast_exp2(fmaf(v[j + 2], c2, nb)); a3 += fast_exp2(fmaf(v[j + 3], c2, nb));
+                }
+                sacc = sacc * fast_exp2(fmaf(m, c2, nb)) + ((a0 + a1) + (a2 + a3));
                 m = mx;
               }
             }
@@ -249,47 +352,58 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
           tc_fence_before();
           mbar_arrive(&tempty[a]);
         }
-        // the two warpgroups' statistics -> one (max, sum) per row -> this CTA's first chunk slot; its other slots stay neutral
+        // the two warpgroups' statistics -> one (max, sum) per row -> the chunk's slot
         const int r0 = quad * 32 + lane;
-        s_aux[a * QC_ROWS + r0] = make_float2(m0, s0);
-        s_aux[a * QC_ROWS + r0 + 128] = make_float2(m1, s1);
+        s_aux[wg * QC_ROWS + r0] = make_float2(m0 * c2, s0);                    // logit units -> base-2 exponent units
+        s_aux[wg * QC_ROWS + r0 + 128] = make_float2(m1 * c2, s1);
         asm volatile("bar.sync 2, %0;" ::"n"(QU_EPI_THREADS) : "memory");
-        const int ch0 = max(first_page / SCORE_PAGES_PER_CTA, (int)blockIdx.x * QU_CPC);
-        const int ch1 = min(last_page / SCORE_PAGES_PER_CTA, (int)blockIdx.x * QU_CPC + QU_CPC - 1);
-        float2 *outp = P.qc_stats + ((size_t)unit * P.score_chunks + ch0) * QC_ROWS;
-        for (int col = tid; col < QC_ROWS; col += QU_EPI_THREADS) {
+        float2 *outp = P.qc_stats + ((size_t)I.unit * P.score_chunks + I.chunk) * QC_ROWS;
+        {
+          const int col = tid;                                                  // QU_EPI_THREADS == QC_ROWS
           const float2 x = s_aux[col], y = s_aux[QC_ROWS + col];
           const float mm = fmaxf(x.x, y.x);
           float ss = 0.f;
           if (x.x != -INFINITY) ss += x.y * fast_exp2(x.x - mm);
           if (y.x != -INFINITY) ss += y.y * fast_exp2(y.x - mm);
-          const bool live = col < RB;
-          outp[col] = live ? make_float2(mm, ss) : make_float2(-INFINITY, 0.f);
-          for (int c = ch0 + 1; c <= ch1; ++c) outp[(size_t)(c - ch0) * QC_ROWS + col] = make_float2(-INFINITY, 0.f);
+          outp[col] = col < RB ? make_float2(mm, ss) : make_float2(-INFINITY, 0.f);
         }
+        asm volatile("bar.sync 2, %0;" ::"n"(QU_EPI_THREADS) : "memory");       // s_aux is free for the next item's statistics
       } else {
-        float *probs = P.st.probs + (size_t)unit * P.max_ctx;
+        float *probs = P.st.probs + (size_t)I.unit * P.max_ctx;
         const int ncol = (M + 31) & ~31;                                        // rows beyond M carry weight 0: skip whole groups
-        for (int t = a; t < T; t += 2) {
-          mbar_wait(&tfull[a], (t >> 1) & 1);
+        for (int t = 0; t < I.T; ++t) {
+          const int gt = gi + t;
+          if ((gt & 1) != wg) continue;
+          const int a = gt % NACC;
+          mbar_wait(&tfull[a], (gt / NACC) & 1);
           tc_fence_after();
-          const int tok = (tile_pg0 + 8 * t) * PAGE + quad * 32 + lane;
-          float sum = 0.f;
+          const int tok = (I.tile_pg0 + 8 * t) * PAGE + quad * 32 + lane;
+          float sum = 0.f, sum1 = 0.f, sum2 = 0.f, sum3 = 0.f;
+#ifdef QU_PROBE_NOEPI
+          for (int c0 = 0; c0 < 0; c0 += 32) {
+#else
 #pragma unroll 1
           for (int c0 = 0; c0 < ncol; c0 += 32) {
+#endif
             float v[32];
-            tmem_ld32(tmem + tlane + a * RB + c0, v);
+            tmem_ld32(tmem + tlane + a * RBmax + c0, v);
 #pragma unroll
-            for (int j = 0; j < 32; ++j) {
-              const float2 f = s_aux[c0 + j];                                   // (row max in base-2 units, 1 / (row sum * G * n_c))
-              sum = fmaf(fast_exp2(fmaf(v[j], c2, -f.x)), f.y, sum);
+            for (int j = 0; j < 32; j += 4) {
+              const float4 f01 = *reinterpret_cast<const float4 *>(&s_aux[c0 + j]);      // (row max in base-2 units,
+              const float4 f23 = *reinterpret_cast<const float4 *>(&s_aux[c0 + j + 2]);  //  1 / (row sum * G * n_c)) x 2
+              sum = fmaf(fast_exp2(fmaf(v[j], c2, -f01.x)), f01.y, sum);
+              sum1 = fmaf(fast_exp2(fmaf(v[j + 1], c2, -f01.z)), f01.w, sum1);
+              sum2 = fmaf(fast_exp2(fmaf(v[j + 2], c2, -f23.x)), f23.y, sum2);
+              sum3 = fmaf(fast_exp2(fmaf(v[j + 3], c2, -f23.z)), f23.w, sum3);
             }
           }
+          sum = (sum + sum1) + (sum2 + sum3);
           tc_fence_before();
           mbar_arrive(&tempty[a]);
           if (tok >= lo && tok < hi) probs[tok] = sum;
         }
       }
+      gi += I.T;
     }
   }
   tc_fence_before();
