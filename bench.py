@@ -511,6 +511,26 @@ def run_cuda(args):
                          "note": "whole layer-step: B_min of all stages / step time of the timed graph"}}
         roof["frac"] = roof["achieved"] / peak
         roof["frac_of_read_probe"] = roof["achieved"] / read_probe_gbs
+        if args.accum_recompute and in_graph:
+            # the query-cache passes are the path's one contraction (tcgen05, qcache_umma.cuh): beside the HBM bound of
+            # their K bytes, the tensor bound of their flops = 2 x pool tokens x query rows (n_c G) x d per pass
+            try:
+                tf_peak = float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["bf16_tflops"])
+                tf_src = "measured (MEASURED_PEAKS.json bf16_tflops, cuBLAS burst)"
+            except Exception:
+                tf_peak, tf_src = 2250.0, "nominal dense bf16 (B200_PROFILING.md)"
+            G_ = wl.Hq // wl.Hkv
+            rows = float(np.mean([min(wl.accum_window, t_ + 1) for t_ in range(W, W + K)])) * G_   # the window fills up
+            toks = float(np.mean([p["score"] for p in per_step])) / (2.0 * wl.d) * float((wl.score_mode == 3).mean())
+            flops = 2.0 * toks * rows * wl.d
+            roof["qcache_tensor"] = {
+                "bound": "tensor", "unit": "TFLOP/s", "peak": tf_peak, "peak_source": tf_src, "query_rows": rows,
+                "flops_per_pass": flops,
+                **{k_: {"us": times[k_], "achieved": flops / (times[k_] * 1e-6) / 1e12,
+                        "frac": flops / (times[k_] * 1e-6) / 1e12 / tf_peak,
+                        "hbm_gbs": bytes_stage[k_] / (times[k_] * 1e-6) / 1e9,
+                        "hbm_frac": bytes_stage[k_] / (times[k_] * 1e-6) / 1e9 / peak}
+                   for k_ in ("qcache_stats", "qcache_accum") if k_ in times}}
         line = {
             "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_total / K, "higher_is_better": True,

@@ -135,14 +135,23 @@ class DeviceState:
             setattr(self, n, tensors.get(n))
         self._struct = None
 
+    def __setattr__(self, name, value):
+        object.__setattr__(self, name, value)
+        if name != "_struct":
+            object.__setattr__(self, "_struct", None)   # a field was rebound: the marshalled struct is stale
+
     def struct(self) -> StateStruct:
-        s = StateStruct()
-        for n in _STATE_FIELDS:
-            t = getattr(self, n)
-            if t is not None:
-                assert t.is_cuda and t.is_contiguous(), n
-            setattr(s, n, None if t is None else t.data_ptr())
-        self._struct = s
+        """The marshalled hardkv_state (pointers only), built once and kept until a field is rebound: the per-call
+        cost of the binding is then a few ctypes conversions, not 32 attribute walks."""
+        s = self._struct
+        if s is None:
+            s = StateStruct()
+            for n in _STATE_FIELDS:
+                t = getattr(self, n)
+                if t is not None:
+                    assert t.is_cuda and t.is_contiguous(), n
+                setattr(s, n, None if t is None else t.data_ptr())
+            object.__setattr__(self, "_struct", s)
         return s
 
 
