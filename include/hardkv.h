@@ -19,8 +19,11 @@
  *  - Return value: HARDKV_OK or an error detectable on the host (bad config,
  *    unsupported (dtype, head_dim, G), NULL required pointer, workspace too small,
  *    a failed launch).  Nothing throws across the ABI.  Inconsistencies only the
- *    device can see (ctx_len >= max_ctx on append) set *err_flag != 0 and leave the
- *    unit untouched; the caller reads the flag after synchronising.
+ *    device can see set *err_flag != 0 (first error wins; the caller reads the flag after
+ *    synchronising): 1 = ctx_len >= max_ctx on append (the sequence is left untouched),
+ *    2 = more reuse steps than cfg.reuse_max, 3 = hardkv_topp_select was given a row that is
+ *    not a probability row (it sums to more than 4: the integer mass would not be exact),
+ *    >= 100 = a device-side wait gave up (a launch-order protocol error, never expected).
  *  - Layouts (row = head_dim elements of kv_dtype; page = page_size rows):
  *      k_pool, v_pool         [n_pages][page][d]
  *      base_table             [B][Hkv][max_ctx/page]   physical page of logical page j

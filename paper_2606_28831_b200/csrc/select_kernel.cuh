@@ -326,15 +326,22 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
   } else {
     __syncthreads();  // histogram zeroed
     if (C > 1) cluster.barrier_wait();
+    float psum = 0.f;
     for (int i = tid; i < per; i += NT) {
       const int pos = s0 + i;
       uint32_t bits = SEL_INVALID;
       if (pos >= lo && pos < hi) {
         bits = min(__float_as_uint(probs[pos]) & 0x7fffffffu, SEL_ONE);
         hist_add(sh, bits >> 20, bits);
+        psum += __uint_as_float(bits);
       }
       pbits[i] = bits;
     }
+    // probabilities given by the caller: the split mass counters of a bin are exact while the row sums to < 4096.  A row
+    // in which any warp's share sums to more than 4 is not a probability row (a normalised row sums to 1): flag it
+    // (err_flag 3); below that bound the whole row stays under 4 * 32 warps * 8 CTAs = 1024, far from the overflow.
+    psum = warp_sum_f32(psum);
+    if (lane == 0 && psum > 4.0f) atomicCAS(P.st.err_flag, 0, 3);
   }
 
   // ---------------- 2b: Top-p threshold --------------------------------------------------------

@@ -294,6 +294,25 @@ def test_select_degenerate(case, P):
     assert u.sel_count > 0
 
 
+def test_topp_select_flags_a_row_that_is_not_a_probability_row(P):
+    """hardkv_topp_select takes the caller's probabilities as given; its integer-mass histogram is exact for rows that
+    sum to far less than 4096, so a row that sums to more than 4 in any warp's share is flagged (err_flag 3) instead of
+    being selected from silently; a normalised row leaves the flag alone."""
+    wl = make_workload(1, Hq=4, Hkv=1, n0=i32(1200), max_ctx=1216, k_cap=1216, l_upper=i32(5000), cond_cap=0)
+    pr = P(wl)
+    u = pr.ob.units[0]
+    lo, hi = u.pool
+    u.probs[lo:hi] = np.float32(1.0 / (hi - lo))
+    pr.upload_oracle_probs()
+    pr.eng.topp_select(pr.st, 0.9)
+    assert int(pr.st.err_flag.item()) == 0
+    u.probs[lo:hi] = np.float32(0.5)
+    pr.upload_oracle_probs()
+    pr.eng.topp_select(pr.st, 0.9)
+    assert int(pr.st.err_flag.item()) == 3
+    pr.st.err_flag.zero_()
+
+
 def test_empty_pool_and_growth(P):
     """Context shorter than sink + recent: empty pool, dense tier only; then the pool opens."""
     wl = make_workload(1, Hq=8, Hkv=2, n0=i32(3), max_ctx=256, k_cap=64, l_upper=i32(30), cond_cap=4, recent=16)
