@@ -71,9 +71,9 @@ __device__ __forceinline__ void umma_commit(uint64_t *bar) {   // arrives on bar
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void proxy_fence_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-// 32 consecutive fp32 columns of this thread's TMEM lane
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
-  uint32_t r[32];
+// 32 consecutive fp32 columns of this thread's TMEM lane: the load is asynchronous, the registers are valid after
+// tmem_ld_wait() -- issue the next group's load before working on the current one
+__device__ __forceinline__ void tmem_ld32_issue(uint32_t taddr, uint32_t (&r)[32]) {
   asm volatile("tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,"
                "%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
                : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
@@ -81,10 +81,8 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
                  "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
                  "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
                : "r"(taddr));
-  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-  for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
 }
+__device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void *src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
@@ -283,13 +281,36 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
     const char *qc = reinterpret_cast<const char *>(P.st.qcache);
     QuItem I;
     int gi = 0, prev_unit = -1;
+    // PASS 1: the statistics of a thread's rows run on over all of this CTA's chunks of a unit (the reduction over the
+    // chunk slots only needs SOME partition of the pool): one flush per unit into the slot of the first chunk, the CTA's
+    // other slots of the unit are written neutral
+    float m0 = -INFINITY, s0 = 0.f, m1 = -INFINITY, s1 = 0.f;                  // rows quad * 32 + lane and + 128 (logit units)
+    int run_chunk0 = 0, run_chunk1 = -1, run_rb = 128;
+    float run_c2 = 1.f;
+    auto flush = [&]() {   // after a bar.sync 2 has NOT yet been passed: every thread publishes, then combines
+      const int r0 = quad * 32 + lane;
+      s_aux[wg * QC_ROWS + r0] = make_float2(m0 * run_c2, s0);                  // logit units -> base-2 exponent units
+      s_aux[wg * QC_ROWS + r0 + 128] = make_float2(m1 * run_c2, s1);
+      asm volatile("bar.sync 2, %0;" ::"n"(QU_EPI_THREADS) : "memory");
+      float2 *outp = P.qc_stats + ((size_t)prev_unit * P.score_chunks + run_chunk0) * QC_ROWS;
+      const int col = tid;                                                      // QU_EPI_THREADS == QC_ROWS
+      const float2 x = s_aux[col], y = s_aux[QC_ROWS + col];
+      const float mm = fmaxf(x.x, y.x);
+      float ss = 0.f;
+      if (x.x != -INFINITY) ss += x.y * fast_exp2(x.x - mm);
+      if (y.x != -INFINITY) ss += y.y * fast_exp2(y.x - mm);
+      outp[col] = col < run_rb ? make_float2(mm, ss) : make_float2(-INFINITY, 0.f);
+      for (int c = run_chunk0 + 1; c <= run_chunk1; ++c) outp[(size_t)(c - run_chunk0) * QC_ROWS + col] = make_float2(-INFINITY, 0.f);
+      m0 = m1 = -INFINITY; s0 = s1 = 0.f;
+    };
     for (int it = it_begin; it < it_end; ++it) {
       decode(it, I);
       const int M = I.M, RB = I.RB, lo = I.lo, hi = I.hi;
       if (I.unit != prev_unit) {
-        // both warpgroups are through with the previous unit: all of its MMAs have completed, the query block and (pass 2)
-        // s_aux are free
+        if (PASS == 1 && prev_unit >= 0) flush();
+        // both warpgroups are through with the previous unit: all of its MMAs have completed, the query block and s_aux are free
         asm volatile("bar.sync 2, %0;" ::"n"(QU_EPI_THREADS) : "memory");
+        run_chunk0 = I.chunk;
         for (int i = tid; i < RB * CPR; i += QU_EPI_THREADS) {                  // the unit's query block; rows beyond M are zero
           const int r = i / CPR, gq = i % CPR;
           uint4 val = make_uint4(0, 0, 0, 0);
@@ -309,7 +330,7 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
       prev_unit = I.unit;
       const float c2 = P.sm_scale * 1.4426950408889634f / P.st.temperature[I.unit];   // logit -> base-2 exponent of z / T
       if (PASS == 1) {
-        float m0 = -INFINITY, s0 = 0.f, m1 = -INFINITY, s1 = 0.f;              // rows quad * 32 + lane and + 128 (logit units)
+        run_chunk1 = I.chunk; run_rb = RB; run_c2 = c2;
         for (int t = 0; t < I.T; ++t) {
           const int gt = gi + t;
           if ((gt & 1) != wg) continue;
@@ -319,11 +340,17 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
           const int tok0 = (I.tile_pg0 + 8 * t) * PAGE;
           for (int rh = 0; rh < RB / 128; ++rh) {
             float m = rh ? m1 : m0, sacc = rh ? s1 : s0;
-#pragma unroll 1
-            for (int c0 = 0; c0 < QU_TILE; c0 += 32) {
+            const uint32_t tbase = tmem + tlane + a * RBmax + rh * 128;
+            uint32_t rb[2][32];                                                 // two groups of 32 columns: one in flight
+            tmem_ld32_issue(tbase, rb[0]);
+            tmem_ld_wait();
+#pragma unroll
+            for (int cg = 0; cg < QU_TILE / 32; ++cg) {
+              if (cg + 1 < QU_TILE / 32) tmem_ld32_issue(tbase + (cg + 1) * 32, rb[(cg + 1) & 1]);
               float v[32];
-              tmem_ld32(tmem + tlane + a * RBmax + rh * 128 + c0, v);
-              const int tk = tok0 + c0;
+#pragma unroll
+              for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(rb[cg & 1][j]);
+              const int tk = tok0 + cg * 32;
               if (!(tk >= lo && tk + 32 <= hi)) {                               // warp-uniform: only the pool's first / last tile
 #pragma unroll
                 for (int j = 0; j < 32; ++j) v[j] = (tk + j >= lo && tk + j < hi) ? v[j] : -INFINITY;
@@ -346,28 +373,13 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
                 sacc = sacc * fast_exp2(fmaf(m, c2, nb)) + ((a0 + a1) + (a2 + a3));
                 m = mx;
               }
+              tmem_ld_wait();                                                   // the next group has landed
             }
             if (rh) { m1 = m; s1 = sacc; } else { m0 = m; s0 = sacc; }
           }
           tc_fence_before();
           mbar_arrive(&tempty[a]);
         }
-        // the two warpgroups' statistics -> one (max, sum) per row -> the chunk's slot
-        const int r0 = quad * 32 + lane;
-        s_aux[wg * QC_ROWS + r0] = make_float2(m0 * c2, s0);                    // logit units -> base-2 exponent units
-        s_aux[wg * QC_ROWS + r0 + 128] = make_float2(m1 * c2, s1);
-        asm volatile("bar.sync 2, %0;" ::"n"(QU_EPI_THREADS) : "memory");
-        float2 *outp = P.qc_stats + ((size_t)I.unit * P.score_chunks + I.chunk) * QC_ROWS;
-        {
-          const int col = tid;                                                  // QU_EPI_THREADS == QC_ROWS
-          const float2 x = s_aux[col], y = s_aux[QC_ROWS + col];
-          const float mm = fmaxf(x.x, y.x);
-          float ss = 0.f;
-          if (x.x != -INFINITY) ss += x.y * fast_exp2(x.x - mm);
-          if (y.x != -INFINITY) ss += y.y * fast_exp2(y.x - mm);
-          outp[col] = col < RB ? make_float2(mm, ss) : make_float2(-INFINITY, 0.f);
-        }
-        asm volatile("bar.sync 2, %0;" ::"n"(QU_EPI_THREADS) : "memory");       // s_aux is free for the next item's statistics
       } else {
         float *probs = P.st.probs + (size_t)I.unit * P.max_ctx;
         const int ncol = (M + 31) & ~31;                                        // rows beyond M carry weight 0: skip whole groups
@@ -386,7 +398,13 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
           for (int c0 = 0; c0 < ncol; c0 += 32) {
 #endif
             float v[32];
-            tmem_ld32(tmem + tlane + a * RBmax + c0, v);
+            {
+              uint32_t r[32];
+              tmem_ld32_issue(tmem + tlane + a * RBmax + c0, r);
+              tmem_ld_wait();
+#pragma unroll
+              for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+            }
 #pragma unroll
             for (int j = 0; j < 32; j += 4) {
               const float4 f01 = *reinterpret_cast<const float4 *>(&s_aux[c0 + j]);      // (row max in base-2 units,
@@ -405,6 +423,7 @@ __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
       }
       gi += I.T;
     }
+    if (PASS == 1 && prev_unit >= 0) flush();
   }
   tc_fence_before();
   __syncthreads();
