@@ -17,10 +17,10 @@
 // reaches the MMA warp through an mbarrier after a proxy fence (the copies are generic-proxy writes, the tensor core
 // reads through the async proxy).
 //
-// Warp roles (13 warps): 0-3 and 4-7 = two epilogue warpgroups, one per accumulator stage in TMEM (even / odd tiles);
-// 8 = TMEM allocation and the single MMA-issuing thread; 9-12 = producers.  Pipelines: full / empty mbarriers over
-// the K-tile stages (producers <-> MMA, released by tcgen05.commit), tfull / tempty over the two accumulator stages
-// (MMA <-> epilogue).
+// Warp roles (13 warps): 0-3 and 4-7 = two epilogue warpgroups (even / odd tiles); 8 = TMEM allocation and the single
+// MMA-issuing thread; 9-12 = producers.  Pipelines: full / empty mbarriers over the K-tile stages (producers <-> MMA,
+// released by tcgen05.commit), tfull / tempty over the accumulator stages in TMEM (MMA <-> epilogue; 512 columns = four
+// stages of 128 or two of 256).
 #pragma once
 #include "common.cuh"
 #include "qcache_kernels.cuh"
@@ -35,12 +35,8 @@ constexpr int QU_TILE = 128;            // pool tokens per tile (8 pages)
 #ifndef HARDKV_QU_LAG
 #define HARDKV_QU_LAG 2
 #endif
-#ifndef HARDKV_QU_CPC
-#define HARDKV_QU_CPC 4
-#endif
 constexpr int QU_STAGES = HARDKV_QU_STAGES;   // K tiles in shared memory
 constexpr int QU_LAG = HARDKV_QU_LAG;         // a producer signals tile t - QU_LAG after issuing tile t: QU_LAG + 1 tiles in flight
-constexpr int QU_CPC = HARDKV_QU_CPC;         // score chunks (of 64 pages) per CTA
 #ifndef HARDKV_QU_PROD
 #define HARDKV_QU_PROD 128
 #endif
@@ -102,9 +98,9 @@ struct QuItem {
 };
 
 // PASS 1: per-(chunk, query row) softmax statistics -> qc_stats; PASS 2: probabilities summed over the query rows -> probs.
-// Persistent: one CTA per SM walks the items blockIdx.x, blockIdx.x + gridDim.x, ...; the K-tile ring and the TMEM
-// accumulator stages run on across items (a global tile counter gives stage and parity), only the query block of the
-// unit is reloaded per item, by the epilogue warps, while the producers already fetch the item's first tiles.
+// Persistent: one CTA per SM takes a contiguous block of the item list; the K-tile ring and the TMEM accumulator stages
+// run on across items (a global tile counter gives stage and parity), the query block is reloaded only when the unit
+// changes, by the epilogue warps, while the producers already fetch the next tiles.
 template <int D, int PASS>
 __global__ void __launch_bounds__(QU_THREADS, 1) qcache_umma_kernel(Params P) {
   KernelClock kclock(P);
