@@ -57,7 +57,8 @@ typedef enum {
   HARDKV_ERR_INVALID_ARG = 1,
   HARDKV_ERR_UNSUPPORTED = 2,   /* (kv_dtype, head_dim, G, page_size) not built */
   HARDKV_ERR_WORKSPACE = 3,
-  HARDKV_ERR_CUDA = 4
+  HARDKV_ERR_CUDA = 4,
+  HARDKV_ERR_NOALLOC_LIMIT = 5  /* hardkv_decode_attn_noalloc: the problem needs more than HARDKV_NOALLOC_SCRATCH_BYTES */
 } hardkv_status;
 
 typedef enum { HARDKV_F32 = 0, HARDKV_BF16 = 1 } hardkv_dtype;
@@ -190,6 +191,25 @@ hardkv_status hardkv_rewrite(hardkv_ctx *, const hardkv_state *, hardkv_stream);
 /* Split-K decode attention over dense + selected + condensed tiers merged by Eq. 6 (L748-762). */
 hardkv_status hardkv_decode_attn(hardkv_ctx *, const hardkv_state *, const void *q, float *out,
                                  float *lse /* nullable */, hardkv_stream);
+/* hardkv_decode_attn for callers that cannot allocate device memory at all (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): no hardkv_ctx and no workspace.  The split-K partial states and the
+ * arrival counters of the attention kernel live in ONE file-scope static __device__ array of the library,
+ * HARDKV_NOALLOC_SCRATCH_BYTES (4 MiB) large, which every GPU that loads the library holds until the process exits.
+ * Same kernel, same arithmetic and same results as hardkv_decode_attn on the same state.  Calls no cudaMalloc / cudaFree
+ * or any allocating routine; the only other stream work is one memset of the arrival counters.
+ *  - cfg is validated like hardkv_create's; a problem whose scratch
+ *        4096 + batch * num_kv_heads * ceil((sink + recent + reuse_max + k_cap + cond_cap) / 128) * G * (head_dim + 2) * 4
+ *    bytes exceeds the array, or with more than 1024 (sequence, KV head) units, is refused with
+ *    HARDKV_ERR_NOALLOC_LIMIT before anything is launched.
+ *  - All calls on a device share the array and it keeps the previous call's contents (the counters are cleared on the
+ *    stream at every call; the partial states are rewritten before they are read).  Calls that can overlap on the GPU
+ *    (different streams, or graphs replayed concurrently) RACE on it: serialise them, or use hardkv_decode_attn with
+ *    one workspace per ctx.
+ *  - The array's device address is looked up once per device (cudaGetSymbolAddress, with that device current) at the
+ *    first call on that device. */
+#define HARDKV_NOALLOC_SCRATCH_BYTES (4u << 20)
+hardkv_status hardkv_decode_attn_noalloc(const hardkv_config *cfg, const hardkv_state *, const void *q, float *out,
+                                         float *lse /* nullable */, hardkv_stream);
 /* Steps 3 + 4 fused: the selected rows are gathered from the base pool through sel_idx, written
  * through to the selected tier (L172) and attended while they are in flight, so each selected
  * row is read once; same results as hardkv_rewrite followed by hardkv_decode_attn. */

@@ -5,6 +5,8 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
+
 #include "common.cuh"
 #include "fast_kernels.cuh"
 #include "score_tma.cuh"
@@ -484,6 +486,35 @@ __global__ void __launch_bounds__(256) read_stream_kernel(const uint4 *p, size_t
 
 }  // namespace
 
+// ---- scratch of hardkv_decode_attn_noalloc: [0, 4096) arrival counters of up to 1024 units | split-K partial states.
+// In HOST code this name is only a stand-in for the symbol, not a device address: the address a kernel may be given
+// comes from cudaGetSymbolAddress (noalloc_scratch below), once per device.
+static __device__ __align__(256) unsigned char g_noalloc_scratch[HARDKV_NOALLOC_SCRATCH_BYTES];
+
+namespace {
+constexpr size_t NOALLOC_COUNTER_BYTES = 4096;
+constexpr int NOALLOC_MAX_UNITS = (int)(NOALLOC_COUNTER_BYTES / sizeof(int32_t));
+constexpr int NOALLOC_MAX_DEVICES = 64;
+
+// Device address of g_noalloc_scratch on the CURRENT device, looked up once per device.
+unsigned char *noalloc_scratch(cudaError_t *err) {
+  static std::mutex mu;
+  static unsigned char *ptr[NOALLOC_MAX_DEVICES] = {};
+  int dev = -1;
+  *err = cudaGetDevice(&dev);
+  if (*err != cudaSuccess) return nullptr;
+  if (dev < 0 || dev >= NOALLOC_MAX_DEVICES) { *err = cudaErrorInvalidDevice; return nullptr; }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!ptr[dev]) {
+    void *p = nullptr;
+    *err = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+    if (*err != cudaSuccess || !p) { if (*err == cudaSuccess) *err = cudaErrorInvalidSymbol; return nullptr; }
+    ptr[dev] = static_cast<unsigned char *>(p);
+  }
+  return ptr[dev];
+}
+}  // namespace
+
 extern "C" {
 
 const char *hardkv_status_string(hardkv_status s) {
@@ -493,6 +524,7 @@ const char *hardkv_status_string(hardkv_status s) {
     case HARDKV_ERR_UNSUPPORTED: return "unsupported (kv_dtype, head_dim, G, page_size)";
     case HARDKV_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
     case HARDKV_ERR_CUDA: return "CUDA launch error";
+    case HARDKV_ERR_NOALLOC_LIMIT: return "problem exceeds the static scratch of the no-allocation entry point (HARDKV_NOALLOC_SCRATCH_BYTES)";
   }
   return "unknown status";
 }
@@ -740,6 +772,49 @@ hardkv_status hardkv_sparse_attend(hardkv_ctx *ctx, const hardkv_state *s, const
                                    hardkv_stream st) {
   if (!state_ok(ctx, s) || !q || !out) return HARDKV_ERR_INVALID_ARG;
   launch_attend(ctx, params_of(ctx, s), q, out, lse, ATT_SPARSE, st);
+  return launch_status();
+}
+
+hardkv_status hardkv_decode_attn_noalloc(const hardkv_config *cfg, const hardkv_state *s, const void *q, float *out,
+                                         float *lse, hardkv_stream st) {
+  const hardkv_status cs = check_config(cfg);
+  if (cs != HARDKV_OK) return cs;
+  // size limit first: nothing is touched or launched for a problem that does not fit the static array
+  const size_t units = (size_t)cfg->batch * cfg->num_kv_heads;
+  const int G = cfg->num_q_heads / cfg->num_kv_heads;
+  const size_t part_bytes = units * att_chunks_of(*cfg) * G * (cfg->head_dim + 2) * sizeof(float);
+  if (units > (size_t)NOALLOC_MAX_UNITS || NOALLOC_COUNTER_BYTES + part_bytes > (size_t)HARDKV_NOALLOC_SCRATCH_BYTES)
+    return HARDKV_ERR_NOALLOC_LIMIT;
+  if (!s || !q || !out) return HARDKV_ERR_INVALID_ARG;
+  if (!(s->k_pool && s->v_pool && s->base_table && s->sel_k_pool && s->sel_v_pool && s->sel_pages && s->sel_count &&
+        s->cond_count && s->ctx_len && s->dense_lo && s->err_flag &&
+        (cfg->cond_cap == 0 || (s->cond_k && s->cond_v))))
+    return HARDKV_ERR_INVALID_ARG;
+  cudaError_t ce;
+  unsigned char *scratch = noalloc_scratch(&ce);
+  if (!scratch) { cudaGetLastError(); return HARDKV_ERR_CUDA; }
+  Params P;
+  memset(&P, 0, sizeof(P));
+  P.B = cfg->batch; P.Hq = cfg->num_q_heads; P.Hkv = cfg->num_kv_heads; P.G = G;
+  P.d = cfg->head_dim; P.max_ctx = cfg->max_ctx; P.sink = cfg->sink; P.recent = cfg->recent;
+  P.k_cap = cfg->k_cap; P.cond_cap = cfg->cond_cap; P.accum_window = cfg->accum_window; P.reuse_max = cfg->reuse_max;
+  P.ppu = cfg->max_ctx / PAGE; P.spu = cfg->k_cap / PAGE;
+  P.att_chunks = att_chunks_of(*cfg);
+  P.sm_scale = cfg->sm_scale > 0.f ? cfg->sm_scale : 1.0f / sqrtf((float)cfg->head_dim);
+  P.st = *s;
+  P.st_esize = (int)esize_of(*cfg);
+  P.att_arrive = reinterpret_cast<int32_t *>(scratch);
+  P.part = reinterpret_cast<float *>(scratch + NOALLOC_COUNTER_BYTES);
+  // the array keeps whatever the last call (or a launch that failed midway) left: the counters must start at zero
+  if (cudaMemsetAsync(P.att_arrive, 0, units * sizeof(int32_t), st) != cudaSuccess) { cudaGetLastError(); return HARDKV_ERR_CUDA; }
+  if (cfg->kv_dtype == HARDKV_BF16) {
+    const dim3 gm((P.att_chunks * ATT_CHUNK + ATT_MMA_CHUNK - 1) / ATT_MMA_CHUNK, P.B * P.Hkv);
+    if (P.d == 128) attend_mma_kernel<128, ATT_TIER><<<gm, 256, 0, st>>>(P, q, out, lse);
+    else attend_mma_kernel<64, ATT_TIER><<<gm, 256, 0, st>>>(P, q, out, lse);
+  } else {
+    const dim3 grid(P.att_chunks, P.B * P.Hkv);
+    HK_DISPATCH_TD(*cfg, HK_DISPATCH_G(P.G, (attend_generic_kernel<T, D, G, ATT_TIER><<<grid, 256, 0, st>>>(P, q, out, lse))));
+  }
   return launch_status();
 }
 

@@ -58,7 +58,8 @@ STEP_REUSE_TIER, STEP_SELECT_REWRITE, STEP_SELECT_SPARSE, STEP_REUSE_SPARSE = 0,
 EXPORTS = ["hardkv_workspace_bytes", "hardkv_create", "hardkv_destroy", "hardkv_status_string",
            "hardkv_set_variant", "hardkv_set_select_geometry", "hardkv_set_overlap", "hardkv_set_timing", "hardkv_set_pdl", "hardkv_append_kv", "hardkv_append_kv_merge", "hardkv_score", "hardkv_score_select", "hardkv_qcache_push", "hardkv_calibrate_topp", "hardkv_solve_temperature",
            "hardkv_topp_select", "hardkv_rewrite", "hardkv_decode_attn", "hardkv_rewrite_attend", "hardkv_sparse_attend",
-           "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count", "hardkv_probe_read_stream"]
+           "hardkv_decode_step", "hardkv_decode_step_host", "hardkv_launch_count", "hardkv_probe_read_stream",
+           "hardkv_decode_attn_noalloc"]
 
 
 def _load():
@@ -93,6 +94,7 @@ def _load():
     lib.hardkv_decode_step.argtypes = [vp, sp, vp, vp, vp, C.c_float, C.c_int32, vp, vp, vp]
     lib.hardkv_decode_step_host.argtypes = [vp, sp, vp, vp, vp, C.c_float, C.c_int32, vp, vp]
     lib.hardkv_probe_read_stream.argtypes = [vp, C.c_size_t, vp]
+    lib.hardkv_decode_attn_noalloc.argtypes = [cp, sp, vp, vp, vp, vp]
     lib.hardkv_launch_count.argtypes = [vp]
     lib.hardkv_launch_count.restype = C.c_int64
     for n in EXPORTS:
@@ -125,6 +127,15 @@ def probe_read_stream(buf: torch.Tensor):
     """One read-only streaming pass over a CUDA tensor on the current stream (hardkv_probe_read_stream)."""
     assert buf.is_cuda and buf.is_contiguous()
     _check(lib.hardkv_probe_read_stream(_ptr(buf), buf.numel() * buf.element_size(), _stream()))
+
+
+NOALLOC_SCRATCH_BYTES = 4 << 20   # HARDKV_NOALLOC_SCRATCH_BYTES
+
+
+def decode_attn_noalloc(cfg: "Config", st: "DeviceState", q, out, lse=None):
+    """hardkv_decode_attn_noalloc: decode attention over the tiers of `st` with no ctx and no workspace -- the kernel's
+    scratch is the library's static device array (4 MiB; calls that overlap on the GPU race on it, see hardkv.h)."""
+    _check(lib.hardkv_decode_attn_noalloc(C.byref(cfg), C.byref(st.struct()), _ptr(q), _ptr(out), _ptr(lse), _stream()))
 
 
 class DeviceState:
