@@ -339,7 +339,8 @@ def run_cuda(args):
         dur = (ts[:, :, 1] - ts[:, :, 0]) / 1e3                                # [K][kernels] us
         gaps = (ts[:, 1:, 0] - ts[:, :-1, 1]) / 1e3                            # idle between consecutive kernels of a step
         step_gap = (ts[1:, 0, 0] - ts[:-1, -1, 1]) / 1e3                       # idle between steps
-        in_graph = {"kernels_us": {n: float(dur[:, i].mean()) for i, n in enumerate(NAMES)},
+        stamped = bool((ts[:, :, 0] < 9e18).all() and (ts[:, :, 1] > 0).all())   # kernels without the hook (variant 0)
+        in_graph = None if not stamped else {"kernels_us": {n: float(dur[:, i].mean()) for i, n in enumerate(NAMES)},
                     "gaps_us": {f"{NAMES[i]}->{NAMES[i + 1]}": float(gaps[:, i].mean()) for i in range(per_launch - 1)},
                     # the attention kernel is launched programmatically behind the select kernel (hardkv_set_overlap): its
                     # window starts while the selections run (negative gap); what it adds to the step is the part after them

@@ -283,22 +283,61 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
       float *acc = P.st.acc + (size_t)unit * P.max_ctx;
       float *ring = P.st.ring + ((size_t)unit * P.accum_window + slot) * P.max_ctx;
       double tot = 0.0;
-      for (int i = tid; i < per; i += NT) {
-        const int pos = s0 + i;
-        uint32_t bits = SEL_INVALID;
-        if (pos >= lo && pos < hi) {
-          float pr = 0.f;
+      // a thread owns quads of 4 consecutive tokens (s0 and max_ctx are multiples of 4: every row is 16-byte aligned at
+      // a quad): one 16-byte load per query head, of acc and of the ring row, 16-byte stores; quads that straddle the
+      // pool's ends or the row's end take the scalar path.  Per-token arithmetic is unchanged.
+      const int nq = per >> 2;
+      for (int qd = tid; qd < nq; qd += NT) {
+        const int pos = s0 + 4 * qd;
+        uint32_t bits[4] = {SEL_INVALID, SEL_INVALID, SEL_INVALID, SEL_INVALID};
+        if (pos >= lo && pos + 3 < hi && pos + 3 < P.max_ctx) {
+          const float4 a4 = *reinterpret_cast<const float4 *>(acc + pos), r4 = *reinterpret_cast<const float4 *>(ring + pos);
+          float pr[4] = {0.f, 0.f, 0.f, 0.f};
 #pragma unroll
-          for (int g = 0; g < GMAX; ++g)
-            if (g < G) pr = fmaf(fast_exp2(fmaf(sel_ld<COHERENT>(lg + (size_t)g * P.max_ctx + pos), c2, -mg[g])), rs[g], pr);
-          float a = (acc[pos] - ring[pos]) + pr;
-          a = fmaxf(a, 0.f);
-          acc[pos] = a;
-          ring[pos] = pr;
-          tot += (double)a;
-          bits = __float_as_uint(a);  // acc for now; normalised below
+          for (int g0 = 0; g0 < GMAX; g0 += 4) {     // four heads' loads in flight at a time (registers), heads in order
+            float4 x[4];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+              if (g0 + u < G) x[u] = sel_ld4<COHERENT>(reinterpret_cast<const float4 *>(lg + (size_t)(g0 + u) * P.max_ctx + pos));
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+              if (g0 + u < G) {
+                pr[0] = fmaf(fast_exp2(fmaf(x[u].x, c2, -mg[g0 + u])), rs[g0 + u], pr[0]);
+                pr[1] = fmaf(fast_exp2(fmaf(x[u].y, c2, -mg[g0 + u])), rs[g0 + u], pr[1]);
+                pr[2] = fmaf(fast_exp2(fmaf(x[u].z, c2, -mg[g0 + u])), rs[g0 + u], pr[2]);
+                pr[3] = fmaf(fast_exp2(fmaf(x[u].w, c2, -mg[g0 + u])), rs[g0 + u], pr[3]);
+              }
+            }
+          }
+          const float ao[4] = {a4.x, a4.y, a4.z, a4.w}, ro[4] = {r4.x, r4.y, r4.z, r4.w};
+          float an[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            an[e] = fmaxf((ao[e] - ro[e]) + pr[e], 0.f);
+            tot += (double)an[e];
+            bits[e] = __float_as_uint(an[e]);     // acc for now; normalised below
+          }
+          *reinterpret_cast<float4 *>(acc + pos) = make_float4(an[0], an[1], an[2], an[3]);
+          *reinterpret_cast<float4 *>(ring + pos) = make_float4(pr[0], pr[1], pr[2], pr[3]);
+        } else {
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int pe = pos + e;
+            if (pe >= lo && pe < hi) {
+              float pr = 0.f;
+#pragma unroll
+              for (int g = 0; g < GMAX; ++g)
+                if (g < G) pr = fmaf(fast_exp2(fmaf(sel_ld<COHERENT>(lg + (size_t)g * P.max_ctx + pe), c2, -mg[g])), rs[g], pr);
+              float a = (acc[pe] - ring[pe]) + pr;
+              a = fmaxf(a, 0.f);
+              acc[pe] = a;
+              ring[pe] = pr;
+              tot += (double)a;
+              bits[e] = __float_as_uint(a);
+            }
+          }
         }
-        pbits[i] = bits;
+        *reinterpret_cast<uint4 *>(pbits + 4 * qd) = make_uint4(bits[0], bits[1], bits[2], bits[3]);
       }
 #pragma unroll
       for (int o = 16; o; o >>= 1) tot += __shfl_xor_sync(0xffffffffu, tot, o);
@@ -312,14 +351,29 @@ __device__ __forceinline__ void select_unit(const Params &P, float p, int unit, 
       cluster.sync();
       tot = 0.0;
       for (int c = 0; c < C; ++c) tot += sh.acc_tot[c];
-      for (int i = tid; i < per; i += NT) {
-        const uint32_t ab = pbits[i];
-        if (ab == SEL_INVALID) continue;
-        const float pr = tot > 0.0 ? (float)((double)__uint_as_float(ab) / tot) : 0.f;
-        probs[s0 + i] = pr;
-        const uint32_t bits = min(__float_as_uint(pr), SEL_ONE);
-        pbits[i] = bits;
-        hist_add(sh, bits >> 20, bits);
+      for (int qd = tid; qd < nq; qd += NT) {
+        const uint4 ab4 = *reinterpret_cast<const uint4 *>(pbits + 4 * qd);
+        const uint32_t ab[4] = {ab4.x, ab4.y, ab4.z, ab4.w};
+        uint32_t nb[4];
+        float pr[4];
+        bool whole = true;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          nb[e] = SEL_INVALID; pr[e] = 0.f;
+          if (ab[e] == SEL_INVALID) { whole = false; continue; }
+          pr[e] = tot > 0.0 ? (float)((double)__uint_as_float(ab[e]) / tot) : 0.f;
+          nb[e] = min(__float_as_uint(pr[e]), SEL_ONE);
+          hist_add(sh, nb[e] >> 20, nb[e]);
+        }
+        const int pos = s0 + 4 * qd;
+        if (whole) {
+          *reinterpret_cast<float4 *>(probs + pos) = make_float4(pr[0], pr[1], pr[2], pr[3]);
+        } else {
+#pragma unroll
+          for (int e = 0; e < 4; ++e)
+            if (nb[e] != SEL_INVALID) probs[pos + e] = pr[e];
+        }
+        *reinterpret_cast<uint4 *>(pbits + 4 * qd) = make_uint4(nb[0], nb[1], nb[2], nb[3]);
       }
       if (rank == 0 && tid == 0) P.st.ring_slot[unit] = (slot + 1) % P.accum_window;
     }
