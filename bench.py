@@ -445,9 +445,10 @@ def run_cuda(args):
     warm()
     torch.cuda.synchronize()
     barrier()
+    sh = stream.cuda_stream          # the caller of a per-token loop holds on to its stream handle
     t_e2e0 = time.perf_counter()
     for t in range(W, W + K):
-        eng.decode_step_host(states[t % L], q_h[t], k_h[t], v_h[t], wl.p, out_h)
+        eng.decode_step_host(states[t % L], q_h[t], k_h[t], v_h[t], wl.p, out_h, stream=sh)
         stream.synchronize()
     t_e2e_eager = time.perf_counter() - t_e2e0
     assert bool(torch.isfinite(out_h).all()), "non-finite output through the host entry"

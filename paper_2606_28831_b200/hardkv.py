@@ -250,13 +250,15 @@ class HardKV:
         return int(lib.hardkv_launch_count(self._ctx))
 
     def decode_step_host(self, st: DeviceState, q_host, k_new_host, v_new_host, p: float, out_host,
-                         do_select: bool = True):
-        """q_host / k_new_host / v_new_host / out_host: HOST (ideally pinned) torch tensors; see hardkv.h."""
+                         do_select: bool = True, stream: int | None = None):
+        """q_host / k_new_host / v_new_host / out_host: HOST (ideally pinned) torch tensors; see hardkv.h.
+        stream: raw cudaStream_t handle (torch.cuda.current_stream().cuda_stream) of a caller that holds on to its
+        stream -- saves the per-call lookup in a per-token loop; None = torch's current stream."""
         for t in (q_host, k_new_host, v_new_host, out_host):
             assert not t.is_cuda and t.is_contiguous()
-        _check(lib.hardkv_decode_step_host(self._ctx, C.byref(st.struct()), _ptr(q_host), _ptr(k_new_host),
-                                           _ptr(v_new_host), np.float32(p), int(do_select), _ptr(out_host),
-                                           _stream()))
+        _check(lib.hardkv_decode_step_host(self._ctx, C.byref(st.struct()), q_host.data_ptr(), k_new_host.data_ptr(),
+                                           v_new_host.data_ptr(), p, int(do_select), out_host.data_ptr(),
+                                           _stream() if stream is None else stream))
 
     def decode_step(self, st: DeviceState, q, k_new, v_new, p: float, out, lse=None, do_select: bool = True):
         _check(lib.hardkv_decode_step(self._ctx, C.byref(st.struct()), _ptr(q), _ptr(k_new), _ptr(v_new),
