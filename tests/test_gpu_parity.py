@@ -168,13 +168,14 @@ def test_fused_decode_step(name, teacher, P):
 
 
 @pytest.mark.parametrize("variant", [0, 2, 3, 4])
-@pytest.mark.parametrize("name", ["c1s", "c2s", "c3s", "c4s", "g1d64", "snap4"])
+@pytest.mark.parametrize("name", ["c1s", "c2s", "c3s", "c4s", "g1d64", "snap4", "qc4"])
 def test_kernel_variants(name, variant, P):
     """Variant 0 (generic fp32-FMA kernels), 2 (TMA-staged persistent score), 3 (score and selection fused into one
     persistent kernel: CTAs stream K pages and the CTA that retires a unit's last chunk runs its selection) and 4 (the
     publishing persistent score kernel with the select kernel co-resident behind it, longest unit first) against the
     oracle; the default is variant 1.  Variants 3 and 4 do not apply to configs with SNAPKV heads (the pooling pass sits
-    between score and select)."""
+    between score and select).  qc4 (query-cache heads): variant 0 runs the mma.sync form of the query-cache passes, the
+    others the tcgen05 form; with a query cache in the state variants 3 / 4 run their stages back to back."""
     from paper_2606_28831_b200 import hardkv
     wl = WL[name]
     pr = P(wl, want_mask=False)
