@@ -134,7 +134,13 @@ hardkv_status hardkv_set_select_geometry(hardkv_ctx *ctx, int32_t cluster, int32
 /* 1 (default): in hardkv_decode_step's compression steps on the bf16 paths the attention kernel is launched
  * programmatically behind the select kernel: its CTAs take the SMs that finished selections leave and wait per unit for
  * that unit's selection (flag published by the select kernel), units in the order their selections finish, so the
- * latency-bound selection of the long units hides under the attention of the short ones.  0: plain stream order. */
+ * latency-bound selection of the long units hides under the attention of the short ones.  In the same steps the
+ * append / retire kernel runs on a side branch BESIDE the score kernel (the score kernel computes the two scalars it
+ * needs itself and never reads the appended row) and joins before the select kernel: fork and join are event record /
+ * wait on a stream the ctx owns (created by hardkv_create, capturable, no device memory); during the step the new
+ * ctx_len / c_lo / dense_lo live in the workspace and the attention kernel writes them back, so when the call's work
+ * has completed the state is exactly that of plain stream order.  A ctx therefore serves ONE stream at a time.
+ * 0: plain stream order, one stream.  Results are bit-identical either way. */
 hardkv_status hardkv_set_overlap(hardkv_ctx *ctx, int32_t on);
 /* Measurement hook: while `slots` (DEVICE memory, 2 * capacity u64, the caller presets every pair to (~0, 0)) is set,
  * the i-th hot-kernel launch made through this ctx (append, score, select, score_select, attend; generic variants

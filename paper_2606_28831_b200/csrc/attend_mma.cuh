@@ -48,8 +48,16 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   constexpr int ROWB = D * 2;
   const int unit = P.wait_select == 1 ? P.unit_order[blockIdx.y]
                    : (P.wait_select == 2 ? P.unit_order[gridDim.y - 1 - blockIdx.y] : (int)blockIdx.y), b = unit / P.Hkv, h = unit % P.Hkv;
+  // forked append (common.cuh): nobody reads the in-place scalars during this launch -- one CTA writes them back
+  if (P.use_shadow && blockIdx.x == 0 && blockIdx.y == 0) {
+    for (int t = threadIdx.x; t < P.B; t += 256) {
+      P.st.ctx_len[t] = P.sh_scal[t];
+      P.st.c_lo[t] = P.sh_scal[P.B + t];
+      P.st.dense_lo[t] = P.sh_scal[2 * P.B + t];
+    }
+  }
   if (P.wait_select) wait_unit_selected(P, unit);
-  const int n = P.st.ctx_len[b];
+  const int n = P.use_shadow ? P.sh_scal[b] : P.st.ctx_len[b];
   int s_end, r_lo;
   if (!dense_bounds(P, b, n, s_end, r_lo)) {   // more reuse steps than cfg.reuse_max: flag, leave the unit untouched
     if (threadIdx.x == 0 && blockIdx.x == 0) atomicExch(P.st.err_flag, 2);

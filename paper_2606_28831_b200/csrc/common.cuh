@@ -37,6 +37,13 @@ struct Params {
   int32_t *epoch;        // [1] decode steps appended so far: the append kernel bumps it, select publishes it per unit
   int32_t *sel_flag;     // [units] == *epoch once the unit's selection of this step is complete and visible
   int32_t *unit_order;   // [units] units by increasing pool length (the order their selections finish in)
+  // Forked append (hardkv_decode_step): the append / retire kernel runs beside the score kernel and does NOT write the
+  // per-sequence scalars ctx_len / c_lo / dense_lo in place (the score kernel is reading them) but into sh_scal; the
+  // kernels after the join read them there (use_shadow), and the attention kernel writes them back in place.
+  int pre_append;        // score launch: pool bounds as the step's append kernel will leave them (pool_bounds)
+  int defer_commit;      // append launch: scalars -> sh_scal
+  int use_shadow;        // launches after the join: scalars <- sh_scal
+  int32_t *sh_scal;      // [3][B]: ctx_len, c_lo, dense_lo after this step's append / retirement
   int wait_select;       // attention launch: 1 = launched programmatically behind the select kernel: wait per unit, units by
                          // increasing pool length; 2 = the same behind the score || select pair: longest pool first
   int32_t *score_flag;   // [units] == *epoch once every logit / chunk statistic of the unit is stored (score || select overlap)
@@ -173,9 +180,21 @@ __device__ __forceinline__ const char *paged_row(const void *pool, const int32_t
 }
 
 // Pool bounds of sequence b (Tier-2 address range): [lo, hi).
+// pre_append: the arithmetic of append_retire_kernel on the scalars it has not written: n + 1 unless the context is
+// full, and c_lo pushed up until the pool fits l_upper (a compression step).
 __device__ __forceinline__ void pool_bounds(const Params &P, int b, int &n, int &lo, int &hi) {
-  n = P.st.ctx_len[b];
-  lo = P.st.c_lo[b];
+  if (P.use_shadow) {
+    n = P.sh_scal[b];
+    lo = P.sh_scal[P.B + b];
+  } else {
+    n = P.st.ctx_len[b];
+    lo = P.st.c_lo[b];
+    if (P.pre_append && n < P.max_ctx) {
+      n += 1;
+      const int over = n - P.recent - lo - P.st.l_upper[b];
+      if (over > 0) lo += over;
+    }
+  }
   hi = n - P.recent;
   if (hi < lo) hi = lo;
 }
@@ -200,7 +219,7 @@ __device__ __forceinline__ float warp_sum_f32(float v) {
 // recent + reuse_max rows the attention grid was sized for.
 __device__ __forceinline__ bool dense_bounds(const Params &P, int b, int n, int &s_end, int &r_lo) {
   s_end = min(P.sink, n);
-  r_lo = min(max(P.st.dense_lo[b], s_end), n);
+  r_lo = min(max(P.use_shadow ? P.sh_scal[2 * P.B + b] : P.st.dense_lo[b], s_end), n);
   return n - r_lo <= P.recent + P.reuse_max;
 }
 

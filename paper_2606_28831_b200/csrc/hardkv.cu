@@ -27,6 +27,8 @@ struct hardkv_ctx {
   int overlap;                   // 1 (default): the attention of a compression step starts while the select kernel runs
   int fused_ok;                  // the fused score -> select kernel applies to this config (score_select.cuh)
   int overlap_ok;                // the co-resident score || select pair (variant 4) applies to this config
+  cudaStream_t aux;              // hardkv_decode_step: the branch the append / retire kernel runs on beside the score kernel
+  cudaEvent_t ev_fork, ev_join;  // (fork / join by events: capturable; host-side driver objects, no device memory)
   unsigned long long *timing;    // hardkv_set_timing: per-launch (first CTA start, last CTA end), or NULL
   int timing_cap, timing_next;
   int pdl;                       // 1: launches carry the programmatic-stream-serialization attribute (hardkv_set_pdl)
@@ -60,7 +62,7 @@ WsLayout ws_layout(const hardkv_config &c) {
   size_t off = 0;
   w.arrive = off; off += align256(units * sizeof(int32_t));
   w.ss = off;     off += align256((units + 1) * sizeof(int32_t));
-  w.ovl = off;    off += align256((3 * units + 1) * sizeof(int32_t));   // sel_flag[units] | unit_order[units] | epoch | score_flag[units]
+  w.ovl = off;    off += align256((3 * units + 1 + 3 * (size_t)c.batch) * sizeof(int32_t));   // sel_flag[units] | unit_order[units] | epoch | score_flag[units] | sh_scal[3][B]
   w.part = off;   off += align256(units * att_chunks_of(c) * G * (c.head_dim + 2) * sizeof(float));
   w.stats = off;  off += align256(units * score_chunks_of(c) * 8 * sizeof(float2));
   const size_t qb = (size_t)c.batch * c.num_q_heads * c.head_dim, kb = units * c.head_dim;
@@ -567,6 +569,7 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
   P.unit_order = P.sel_flag + (size_t)cfg->batch * cfg->num_kv_heads;
   P.epoch = P.unit_order + (size_t)cfg->batch * cfg->num_kv_heads;
   P.score_flag = P.epoch + 1;
+  P.sh_scal = P.score_flag + (size_t)cfg->batch * cfg->num_kv_heads;
   P.wait_select = 0;
   P.part = reinterpret_cast<float *>(base + w.part);
   P.score_stats = reinterpret_cast<float2 *>(base + w.stats);
@@ -631,11 +634,30 @@ hardkv_status hardkv_create(const hardkv_config *cfg, void *workspace, size_t by
       ctx->fused_ok = 0;
     }
   }
+  // the side branch of hardkv_decode_step (without these driver objects the step runs in plain stream order)
+  {
+    int lo_p = 0, hi_p = 0;
+    cudaDeviceGetStreamPriorityRange(&lo_p, &hi_p);
+    if (cudaStreamCreateWithPriority(&ctx->aux, cudaStreamNonBlocking, hi_p) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ctx->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+      cudaGetLastError();
+      if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+      if (ctx->aux) cudaStreamDestroy(ctx->aux);
+      ctx->aux = nullptr; ctx->ev_fork = nullptr; ctx->ev_join = nullptr;
+    }
+  }
   *out = ctx;
   return HARDKV_OK;
 }
 
-void hardkv_destroy(hardkv_ctx *ctx) { delete ctx; }
+void hardkv_destroy(hardkv_ctx *ctx) {
+  if (!ctx) return;
+  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+  if (ctx->aux) cudaStreamDestroy(ctx->aux);
+  delete ctx;
+}
 
 hardkv_status hardkv_set_variant(hardkv_ctx *ctx, int32_t variant) {
   if (!ctx || variant < 0 || variant > 4) return HARDKV_ERR_INVALID_ARG;
@@ -837,7 +859,26 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   const Params P = params_of(ctx, s);
   if (do_select < 0 || do_select > 3) return HARDKV_ERR_INVALID_ARG;
   const bool compress = do_select == HARDKV_STEP_SELECT_REWRITE || do_select == HARDKV_STEP_SELECT_SPARSE;
-  launch_append(ctx, P, k_new, v_new, q, compress ? 1 : 0, st);   // between compressions: Step 1 only (L78, L274)
+  // The score kernel needs from the append / retire kernel only the two scalars n + 1 and the new c_lo, which it can
+  // compute itself (pool_bounds, pre_append), and never reads the appended row (it lies in the recent window, outside
+  // the pool, for W >= 1): on a compression step the append kernel runs on a forked branch BESIDE the score kernel and
+  // joins before the select kernel, which needs its step counter, unit order and re-armed counters.  While the score
+  // kernel reads the per-sequence scalars nobody may overwrite them: the forked append kernel leaves them in the
+  // workspace (sh_scal), the kernels after the join read them there, the attention kernel writes them back in place.
+  const bool fork = compress && ctx->overlap && ctx->aux && fast_path(ctx) && (ctx->variant == 1 || ctx->variant == 2) &&
+                    ctx->cfg.recent >= 1;
+  Params Pj = P;                 // launches after the join
+  if (fork) {
+    Params Pa = P;
+    Pa.defer_commit = 1;
+    Pj.use_shadow = 1;
+    cudaEventRecord(ctx->ev_fork, st);
+    cudaStreamWaitEvent(ctx->aux, ctx->ev_fork, 0);
+    launch_append(ctx, Pa, k_new, v_new, q, 1, ctx->aux);
+    cudaEventRecord(ctx->ev_join, ctx->aux);
+  } else {
+    launch_append(ctx, P, k_new, v_new, q, compress ? 1 : 0, st);   // between compressions: Step 1 only (L78, L274)
+  }
   launch_qcache_push(ctx, P, q, st);                              // the query window slides on every step (L448)
   // variant 4 overlaps the two kernels through the unit order the append kernel of THIS call has just written
   const bool ss_overlap = compress && ctx->variant == 4 && !P.st.qcache;
@@ -846,15 +887,22 @@ hardkv_status hardkv_decode_step(hardkv_ctx *ctx, const hardkv_state *s, const v
   } else if (ss_overlap) {
     launch_score_select_overlapped(ctx, P, q, p, st);
   } else if (compress) {
-    launch_score(ctx, P, q, st);
-    launch_pool(ctx, P, st);
-    launch_qcache_metric(ctx, P, st);
+    if (fork) {
+      Params Ps = P;
+      Ps.pre_append = 1;
+      launch_score(ctx, Ps, q, st);
+      cudaStreamWaitEvent(st, ctx->ev_join, 0);
+    } else {
+      launch_score(ctx, P, q, st);
+    }
+    launch_pool(ctx, Pj, st);
+    launch_qcache_metric(ctx, Pj, st);
     // the score kernel's chunk statistics describe the raw logits: configs with pooled heads take them in-kernel
-    launch_select(ctx, P, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
+    launch_select(ctx, Pj, p, (fast_path(ctx) && P.pool_kernel <= 1) ? 2 : 1, st);
   }
   // the select kernel (variants 1, 2: the last launch above) is followed by the attention of the same units: overlap them
   const int overlap = ss_overlap ? 2 : (compress && ctx->overlap && fast_path(ctx) && ctx->variant != 3);
-  launch_attend(ctx, P, q, out, lse, do_select == HARDKV_STEP_SELECT_REWRITE ? ATT_REWRITE
+  launch_attend(ctx, Pj, q, out, lse, do_select == HARDKV_STEP_SELECT_REWRITE ? ATT_REWRITE
                                      : (do_select == HARDKV_STEP_REUSE_TIER ? ATT_TIER : ATT_SPARSE), st, overlap);
   return launch_status();
 }

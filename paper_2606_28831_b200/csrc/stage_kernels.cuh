@@ -58,7 +58,10 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
   const int clo0 = P.st.c_lo[b];
   const int lup = P.st.l_upper[b];
   if (n >= P.max_ctx) {  // device-detected inconsistency: flag and leave the sequence untouched
-    if (threadIdx.x == 0) atomicExch(P.st.err_flag, 1);
+    if (threadIdx.x == 0) {
+      atomicExch(P.st.err_flag, 1);
+      if (P.defer_commit) { P.sh_scal[b] = n; P.sh_scal[P.B + b] = clo0; P.sh_scal[2 * P.B + b] = P.st.dense_lo[b]; }
+    }
     return;
   }
   const int n1 = n + 1;
@@ -213,9 +216,15 @@ __global__ void __launch_bounds__(256) append_retire_kernel(Params P, const void
   if (threadIdx.x == 0) {
     int c = clo0;
     if (do_retire && n1 - P.recent - c > lup) c = n1 - P.recent - lup;
-    P.st.ctx_len[b] = n1;
-    P.st.c_lo[b] = c;
-    if (do_retire) P.st.dense_lo[b] = max(min(P.sink, n1), n1 - P.recent);   // re-anchor the dense tier (L71)
+    if (P.defer_commit) {      // forked beside the score kernel, which is reading the scalars: into the shadow (common.cuh)
+      P.sh_scal[b] = n1;
+      P.sh_scal[P.B + b] = c;
+      P.sh_scal[2 * P.B + b] = do_retire ? max(min(P.sink, n1), n1 - P.recent) : P.st.dense_lo[b];
+    } else {
+      P.st.ctx_len[b] = n1;
+      P.st.c_lo[b] = c;
+      if (do_retire) P.st.dense_lo[b] = max(min(P.sink, n1), n1 - P.recent);   // re-anchor the dense tier (L71)
+    }
   }
 }
 

@@ -369,6 +369,14 @@ def test_error_paths(P):
     pr.eng.append_kv(pr.st, knd, vnd)                             # ctx_len == max_ctx: no room
     torch.cuda.synchronize()
     assert int(pr.st.err_flag.item()) == 1 and int(pr.st.ctx_len.item()) == 64
+    # the same through the fused step, whose append kernel runs on a forked branch beside the score kernel and leaves the
+    # per-sequence scalars to the attention kernel to write back: a full context stays exactly as it was
+    pr.st.err_flag.zero_()
+    before = (int(pr.st.ctx_len.item()), int(pr.st.c_lo.item()), int(pr.st.dense_lo.item()))
+    pr.eng.decode_step(pr.st, qd, knd, vnd, wl.p, pr.out, pr.lse)
+    torch.cuda.synchronize()
+    assert int(pr.st.err_flag.item()) == 1
+    assert (int(pr.st.ctx_len.item()), int(pr.st.c_lo.item()), int(pr.st.dense_lo.item())) == before
     with pytest.raises(hardkv.HardKVError):
         pr.eng.score(pr.st, None)
 
