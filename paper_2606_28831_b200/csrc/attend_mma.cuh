@@ -57,6 +57,20 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
     }
   }
   if (P.wait_select) wait_unit_selected(P, unit);
+  // Virtual row space of a unit: [selected | dense | condensed].  With the selected rows first, row v of the space is
+  // selected row v whatever the counts are: the two loads that start its resolution (sel_idx[v], sel_pages[v / 16]) are
+  // issued here, together with the loads of the counts, instead of behind them -- one dependent round trip less at the
+  // head of every CTA -- and a tile of 16 selected rows is exactly one page of the selected tier (write-through).
+  constexpr int RPL = ATT_TPW / 2;
+  const int32_t *stab = P.st.sel_pages + (size_t)unit * P.spu;
+  const int32_t *idx = P.st.sel_idx + (size_t)unit * P.k_cap;
+  int spec_pos[RPL], spec_page[RPL];
+#pragma unroll
+  for (int r = 0; r < RPL; ++r) {
+    const int v = (int)blockIdx.x * ATT_MMA_CHUNK + (int)(threadIdx.x >> 5) * (ATT_TPW * 16) + r * 32 + (int)(threadIdx.x & 31);
+    spec_pos[r] = (MODE != ATT_TIER && v < P.k_cap) ? __ldg(idx + v) : -1;
+    spec_page[r] = (MODE != ATT_SPARSE && v < P.k_cap) ? __ldg(stab + (v >> 4)) : -1;
+  }
   const int n = P.use_shadow ? P.sh_scal[b] : P.st.ctx_len[b];
   int s_end, r_lo;
   if (!dense_bounds(P, b, n, s_end, r_lo)) {   // more reuse steps than cfg.reuse_max: flag, leave the unit untouched
@@ -75,8 +89,6 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   const int G = P.G;
 
   const int32_t *tab = P.st.base_table + (size_t)unit * P.ppu;
-  const int32_t *stab = P.st.sel_pages + (size_t)unit * P.spu;
-  const int32_t *idx = P.st.sel_idx + (size_t)unit * P.k_cap;
   const char *kp0 = reinterpret_cast<const char *>(P.st.k_pool), *vp0 = reinterpret_cast<const char *>(P.st.v_pool);
   char *kp1 = reinterpret_cast<char *>(P.st.sel_k_pool), *vp1 = reinterpret_cast<char *>(P.st.sel_v_pool);
   const char *kp2 = reinterpret_cast<const char *>(P.st.cond_k), *vp2 = reinterpret_cast<const char *>(P.st.cond_v);
@@ -100,27 +112,26 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   const int v0 = c * ATT_MMA_CHUNK, v1 = min(total, v0 + ATT_MMA_CHUNK);
   // ---- the rows of all tiles of the warp are resolved up front: lane l holds rows l and l + 32 of the warp's
   //      ATT_TPW * 16 rows as source (tier << 30 | row) and rewrite destination ----
-  constexpr int RPL = ATT_TPW / 2;
   uint32_t srcs[RPL], dsts[RPL];
 #pragma unroll
   for (int r = 0; r < RPL; ++r) {
     srcs[r] = ROW_INVALID; dsts[r] = ROW_INVALID;
     const int v = v0 + warp * (ATT_TPW * 16) + r * 32 + lane;
-    if (v < n_dense) {                      // Tier 1: sinks + recent window, read in place
-      const int pos = v < s_end ? v : r_lo + (v - s_end);
-      srcs[r] = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
-    } else if (v < n_dense + k) {           // Tier 2: selected rows
-      const int j = v - n_dense;
-      const uint32_t srow = (uint32_t)(__ldg(stab + (j >> 4)) * PAGE + (j & 15));
+    if (v < k) {                            // Tier 2: selected rows (v = index into sel_idx)
+      const uint32_t srow = (uint32_t)(spec_page[r] * PAGE + (v & 15));
       if (MODE != ATT_TIER) {
-        const int pos = __ldg(idx + j);
+        const int pos = spec_pos[r];
         srcs[r] = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
         if (MODE == ATT_REWRITE) dsts[r] = srow;
       } else {
         srcs[r] = (1u << 30) | srow;
       }
+    } else if (v < k + n_dense) {           // Tier 1: sinks + recent window, read in place
+      const int dv = v - k;
+      const int pos = dv < s_end ? dv : r_lo + (dv - s_end);
+      srcs[r] = (uint32_t)(__ldg(tab + (pos >> 4)) * PAGE + (pos & 15));
     } else if (v < total) {                 // Tier 3: condensed residents
-      srcs[r] = (2u << 30) | (uint32_t)(unit * P.cond_cap + (v - n_dense - k));
+      srcs[r] = (2u << 30) | (uint32_t)(unit * P.cond_cap + (v - k - n_dense));
     }
   }
 #pragma unroll
@@ -239,7 +250,7 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
     }
   }
 
-  if (MODE == ATT_REWRITE && k > 0 && (n_dense + k - 1) >= v0 && (n_dense + k - 1) < v1) {
+  if (MODE == ATT_REWRITE && k > 0 && (k - 1) >= v0 && (k - 1) < v1) {
     // zero tail of the last valid page of the selected tier (DESIGN reading C9)
     constexpr int LPR = ROWB / 16;
     const int kend = (k + PAGE - 1) & ~(PAGE - 1);
@@ -286,15 +297,17 @@ __global__ void __launch_bounds__(256, 2) attend_mma_kernel(Params P, const void
   }
   // ---- the last CTA of the unit to arrive merges all chunk partials (Eq. 6): its 8 warps take
   //      chunks w, w + 8, ... in parallel (lanes over d), then combine through shared memory ----
-  __threadfence();
+  // every thread's partial stores are ordered before thread 0 by the barrier and thread 0's fence is cumulative: one
+  // fence per CTA instead of 256, each of which would wait for its thread's own streaming stores to drain
   __syncthreads();
   if (tid == 0) {
+    __threadfence();
     const int ticket = atomicAdd(P.att_arrive + unit, 1);
     s_last = (ticket == nchunks - 1);
+    if (s_last) __threadfence();
   }
   __syncthreads();
   if (!s_last) return;
-  __threadfence();
   {
     float mm[8], ll[8], aa[8][D / 32];
 #pragma unroll
